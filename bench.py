@@ -1,0 +1,394 @@
+#!/usr/bin/env python
+"""bench.py — RetroAttention decode hot path on B200: us per decode step per layer, HBM GB/s, overhead vs w=0.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c2|c5] [--layers L]
+
+A "step" is one decode step of an L-layer stack (default L = 32, Llama-3.1-8B depth): for every layer, in
+Alg. 1's order, digest refresh (S1) -> page score + top-k + mask (S2) -> fused multi-query
+sparse attention (S3) -> output-cache merge (S4), all through the C ABI.  Each layer has its own K/V pool,
+digests, mask and cache, so consecutive layer-steps do not share L2 (about 13 MB touched per layer-step, 430 MB
+per step >> 126 MB L2).  One step is captured in a CUDA graph (every step-varying value lives in device memory)
+and replayed K times between CUDA events.  Prints ONE JSON line (rank 0).
+
+`--impl reference` times the fp64 CPU oracle (oracle/retro_oracle.py, as it stands) on the host cores on a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "retro sparse-attn us/step/layer (HBM GB/s vs ~8 TB/s; overhead vs w=0)"
+UNIT = "us/step/layer"
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def measured_hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def workload_cfg(name: str, n_steps: int, window=None):
+    from paper_2508_09001_b200 import workload as wl
+    if name == "c2":
+        cfg = wl.c2(n_steps=n_steps)
+    elif name == "c5":
+        cfg = wl.c5(8, 4096, n_steps=n_steps)
+    elif name == "c1":
+        cfg = wl.c1()
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    if window is not None:
+        cfg = cfg.replace(window=window, name=cfg.name + f"_w{window}")
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.tmp.flush()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.tmp.name):
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        os.unlink(self.tmp.name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def time_graph(graph, iters: int):
+    import torch
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    start.record()
+    for _ in range(iters):
+        graph.replay()
+    end.record()
+    torch.cuda.synchronize()
+    return start.elapsed_time(end)   # ms
+
+
+def run_stack(cfg, n_layers, steps, warmup, seed_offset, dist_barrier, keep_inputs=False):
+    """Build the layer stack, warm up, time `steps` graph replays.  Returns (stack, graph, elapsed_ms)."""
+    import torch
+    from paper_2508_09001_b200 import harness as hs
+    pool = min(warmup + steps, 256)
+    stack = hs.DecodeStack(cfg, n_layers, pool, seed_offset=seed_offset, keep_inputs=keep_inputs)
+    graph = hs.capture_graph(stack.enqueue_step, warmup=1)      # 1 eager step, then capture
+    for _ in range(warmup - 1):
+        graph.replay()
+    torch.cuda.synchronize()
+    dist_barrier()
+    ms = time_graph(graph, steps)
+    dist_barrier()
+    return stack, graph, ms
+
+
+def oracle_sample(cfg, inp, n_steps: int):
+    """Time the oracle, as it stands, on `n_steps` decode steps of one layer (after an untimed digest prefill)."""
+    import numpy as np
+    from oracle import retro_oracle as orc
+    from paper_2508_09001_b200 import workload as wl
+    try:
+        from threadpoolctl import threadpool_limits
+    except Exception:
+        threadpool_limits = None
+    desc = orc.OracleDesc(batch=cfg.batch, num_q_heads=cfg.num_q_heads, num_kv_heads=cfg.num_kv_heads,
+                          head_dim=cfg.head_dim, page_size=cfg.page_size, max_pages_per_seq=cfg.max_pages_per_seq,
+                          max_sel_pages=max(1, cfg.budget_pages), window=cfg.window, sm_scale=cfg.sm_scale)
+    layer = orc.OracleLayer(desc, inp.k_pages.float().cpu().numpy(), inp.v_pages.float().cpu().numpy(),
+                            inp.block_table.cpu().numpy())
+    layer.prefill_bounds(np.asarray(cfg.prompt_lens))
+    budget = np.full(cfg.batch, cfg.budget_pages, dtype=np.int32)
+    q_all = inp.q_all.double().cpu()
+
+    def run():
+        t0 = time.perf_counter()
+        for s in range(n_steps):
+            q_win = np.zeros((cfg.batch, cfg.window + 1, cfg.num_q_heads, cfg.head_dim))
+            q_pos = np.full((cfg.batch, cfg.window + 1), -1, dtype=np.int32)
+            for b in range(cfg.batch):
+                for ss in wl.window_rows(cfg, s, b):
+                    pos = cfg.prompt_lens[b] + ss
+                    q_win[b, wl.ring_slot(cfg, pos)] = q_all[ss, b].numpy()
+                    q_pos[b, wl.ring_slot(cfg, pos)] = pos
+            layer.step(q_win, q_pos, q_all[s].numpy(), inp.seq_lens_at(s).cpu().numpy(), budget)
+        return time.perf_counter() - t0
+
+    if threadpool_limits is not None:
+        with threadpool_limits(limits=1):
+            sec = run()
+    else:
+        sec = run()
+    return sec / n_steps * 1e6   # us per layer-step
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, bounded sample, same metric / config / unit."""
+    ri_rank = int(os.environ.get("RANK", 0))
+    if ri_rank != 0:
+        return 0
+    from paper_2508_09001_b200 import workload as wl
+    n_sample = max(1, min(args.steps, 6))
+    cfg = workload_cfg(args.workload, n_steps=args.warmup + n_sample + 2)
+    inp = wl.make_layer_inputs(cfg, layer=0, device="cpu", q_steps=args.warmup + n_sample + 2)
+    oracle_sample(cfg, inp, min(args.warmup, 2))          # warm-up (numpy import, page cache)
+    us = oracle_sample(cfg, inp, n_sample)
+    sample = f"{n_sample} decode steps of 1 layer from the start of decoding (window ramp-up), 1 thread"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": us, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": us * args.layers / 1000.0, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": config_dict(cfg, args.layers),
+        "cpu_baseline": {"value": us, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": us, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def config_dict(cfg, n_layers):
+    return {"workload": cfg.name, "batch": cfg.batch, "num_q_heads": cfg.num_q_heads,
+            "num_kv_heads": cfg.num_kv_heads, "head_dim": cfg.head_dim, "page_size": cfg.page_size,
+            "context": max(cfg.prompt_lens), "budget_tokens": cfg.budget_tokens, "window": cfg.window,
+            "layers_per_step": n_layers,
+            "l2": "inputs larger than L2: each layer-step reads its own layer's digests+pages; "
+                  f"{n_layers} independent layer states per step"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=256)
+    ap.add_argument("--warmup", type=int, default=16)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--layers", type=int, default=32)
+    ap.add_argument("--no-extras", action="store_true", help="skip w=0 overhead run, stage timing, e2e, cpu baseline")
+    ap.add_argument("--oracle-steps", type=int, default=8)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2508_09001_b200 import binding as rb
+    from paper_2508_09001_b200 import harness as hs
+
+    ri = hs.rank_info()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(ri.local_rank)
+    dev = torch.device("cuda", ri.local_rank)
+    if ri.world_size > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if ri.world_size > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    warmup = max(args.warmup, 3)
+    steps, L = args.steps, args.layers
+    w_full = None
+    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 80)
+    warmup = max(warmup, cfg.window + 2)       # the retro window is full during the timed region
+    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 80)
+    seed_off = hs.rank_layer_seed_offset(ri.rank)
+
+    sampler = ClockSampler(ri.local_rank) if ri.rank == 0 else None
+    stack, graph, ms = run_stack(cfg, L, steps, warmup, seed_off, barrier, keep_inputs=True)
+    clocks = sampler.stop() if sampler is not None else None
+    ms = hs.max_over_ranks(ms, dev)
+    us_layer = ms * 1000.0 / (steps * L)
+    # the graph really advanced every layer
+    expect = [p + warmup + steps for p in cfg.prompt_lens]
+    assert stack.seq_lens_host() == expect, (stack.seq_lens_host(), expect)
+    assert torch.isfinite(stack.layers[-1].out.float()).all()
+
+    seq_now = stack.seq_lens_host()
+    bytes_model = hs.stage_bytes(cfg, seq_now)
+    peak, peak_src = measured_hbm_peak()
+    line = {
+        "metric": METRIC, "value": us_layer, "unit": UNIT, "n_gpus": ri.world_size, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms / steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": cfg.dtype, "data": "synthetic", "config": config_dict(cfg, L), "impl": "ours",
+        "gpu_launches": steps * L * hs.KERNELS_PER_LAYER_STEP,
+        "aggregate_layer_steps_per_s": ri.world_size * steps * L / (ms / 1000.0),
+        "path_hbm": {"algorithmic_bytes_per_layer_step": bytes_model["total"],
+                     "achieved_gbs": bytes_model["total"] / (us_layer * 1e-6) / 1e9,
+                     "frac_of_measured": bytes_model["total"] / (us_layer * 1e-6) / 1e9 / peak,
+                     "frac_of_nominal_8TBs": bytes_model["total"] / (us_layer * 1e-6) / 1e9 / NOMINAL_HBM_GBS},
+        "clocks": clocks,
+    }
+
+    if not args.no_extras:
+        # ---- per-stage device time (CUDA events around graphs of L back-to-back launches of one stage) ----
+        stages = {}
+        for st in ("bounds", "select", "attend", "merge"):
+            g = hs.capture_graph(lambda st=st: stack.enqueue_stage(st), warmup=1)
+            for _ in range(3):
+                g.replay()
+            it = 20
+            t = time_graph(g, it)
+            stages[st] = hs.max_over_ranks(t, dev) * 1000.0 / (it * L)      # us per launch(es) of that stage
+        key = {"bounds": "bounds", "select": None, "attend": "attend", "merge": "merge"}
+        sb = dict(bytes_model)
+        sb["select"] = bytes_model["score"] + bytes_model["topk"]
+        dom = max(stages, key=lambda k: stages[k])
+        ach = sb[dom] / (stages[dom] * 1e-6) / 1e9
+        line["stages_us"] = stages
+        line["stages_gbs"] = {k: sb[k] / (stages[k] * 1e-6) / 1e9 for k in stages}
+        line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
+                            "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom), "peak_source": peak_src,
+                            "algorithmic_bytes_per_launch": sb[dom], "launch_us": stages[dom],
+                            "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS}
+        line["attend_arith_intensity_flop_per_byte"] = hs.attend_flops(cfg, seq_now) / bytes_model["kv"]
+
+        # ---- end to end through the C ABI with HOST buffers (H2D of the step's inputs, D2H of its result) ----
+        e2e_steps = min(steps, 32)
+        e2e = run_e2e(stack, cfg, e2e_steps, dev)
+        e2e_ms = hs.max_over_ranks(e2e["ms"], dev)
+        line["e2e"] = {"value": e2e_ms * 1000.0 / (e2e_steps * L), "unit": UNIT,
+                       "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"], "steps": e2e_steps,
+                       "note": "retro_decode_step_host per layer: pinned-host q/k/v of the new token in, "
+                               "out[B][w+1][h_q][d] back, stream synchronised every step"}
+
+        # ---- CPU baseline: the oracle on this box's cores, bounded sample (rank 0, N = 1 only) ----
+        if ri.rank == 0 and ri.world_size == 1:
+            inp0 = stack.inputs[0]
+            n_or = args.oracle_steps
+            us_cpu = oracle_sample(cfg, inp0, n_or)
+            line["cpu_baseline"] = {"value": us_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": f"{n_or} decode steps of layer 0 from the start of decoding, 1 thread "
+                                              f"(host has {os.cpu_count()} cpus)"}
+        # ---- overhead vs w = 0 at the same budget (plain Quest through the same kernels) ----
+        del graph
+        stack_inputs_free(stack)
+        del stack
+        torch.cuda.empty_cache()
+        if cfg.window > 0:
+            cfg0 = workload_cfg(args.workload, n_steps=warmup + steps + 80, window=0)
+            stack0, graph0, ms0 = run_stack(cfg0, L, steps, warmup, seed_off, barrier)
+            ms0 = hs.max_over_ranks(ms0, dev)
+            us0 = ms0 * 1000.0 / (steps * L)
+            line["w0_us_per_layer_step"] = us0
+            line["overhead_vs_w0"] = us_layer / us0 - 1.0
+    else:
+        line["e2e"] = None
+
+    if ri.rank == 0:
+        print(json.dumps(line))
+    if ri.world_size > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def stack_inputs_free(stack):
+    stack.inputs.clear()
+
+
+def run_e2e(stack, cfg, n_steps, dev):
+    """retro_decode_step_host for every layer, n_steps steps, stream-synchronised per step."""
+    import torch
+    from paper_2508_09001_b200 import binding as rb
+    d = stack.desc
+    B, hq, hk, D, w = cfg.batch, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, cfg.window
+    dt = cfg.torch_dtype
+    P = cfg.page_size
+    seq0 = stack.seq_lens_host()
+    ios, hosts = [], []
+    for l, buf in enumerate(stack.layers):
+        inp = stack.inputs[l]
+        # host copies of this layer's next n_steps tokens (q from the pool, k/v rows from the trajectory)
+        ctr = int(stack.counters[l].item())
+        hq_new = torch.stack([stack.q_pools[l][(ctr + s) % stack.pool_steps] for s in range(n_steps)]).cpu().pin_memory()
+        hk_new = torch.empty((n_steps, B, hk, D), dtype=dt)
+        hv_new = torch.empty((n_steps, B, hk, D), dtype=dt)
+        for s in range(n_steps):
+            for b in range(B):
+                pos = seq0[b] + s
+                phys = int(inp.block_table[b, pos // P])
+                hk_new[s, b] = inp.k_pages[phys, :, pos % P].cpu()
+                hv_new[s, b] = inp.v_pages[phys, :, pos % P].cpu()
+        hk_new, hv_new = hk_new.pin_memory(), hv_new.pin_memory()
+        hout = torch.empty((B, w + 1, hq, D), dtype=dt).pin_memory()
+        dq = torch.empty((B, hq, D), dtype=dt, device=dev)
+        dk = torch.empty((B, hk, D), dtype=dt, device=dev)
+        dv = torch.empty((B, hk, D), dtype=dt, device=dev)
+        io = rb.RetroStepIO(dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(),
+                            buf.out.data_ptr())
+        ios.append((io, dq, dk, dv))
+        hosts.append((hq_new, hk_new, hv_new, hout))
+    torch.cuda.synchronize()
+    esz = 2 if cfg.dtype == "bf16" else 4
+    h2d = len(stack.layers) * (B * hq * D + 2 * B * hk * D) * esz
+    d2h = len(stack.layers) * B * (w + 1) * hq * D * esz
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start.record()
+    for s in range(n_steps):
+        for l, buf in enumerate(stack.layers):
+            hq_new, hk_new, hv_new, hout = hosts[l]
+            rb.retro_decode_step_host(d, buf.state, ios[l][0], hq_new[s], hk_new[s], hv_new[s], hout)
+        torch.cuda.current_stream().synchronize()      # the step's results are on the host
+    end.record()
+    torch.cuda.synchronize()
+    return {"ms": start.elapsed_time(end), "h2d": h2d, "d2h": d2h}
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,193 @@
+/* retro.h — C ABI of the B200-native (sm_100a) RetroAttention decode hot path.
+ *
+ * One decode step of retrospective sparse attention (arxiv 2508.09001, Alg. 1):
+ *   S1 retro_update_page_bounds  page digests Kmin/Kmax
+ *   S2 retro_select_pages        Eq. 1 page score + top-k + Alg. 2 mask
+ *   S3 retro_sparse_attend       one fused GQA pass, current + w past queries (Eq. 2/6/7)
+ *   S4 retro_merge_output_cache  LSE merge into the output cache              (Eq. 8-9; 83-85)
+ *
+ * Conventions (every function):
+ *   - Returns RETRO_OK (0) or a negative RETRO_ERR_* code; retro_error_string() names it.
+ *   - Unless a parameter is marked HOST, every pointer is a DEVICE pointer OWNED BY THE CALLER.  The library
+ *     never allocates, frees or retains device memory, never synchronises and never copies to the host; all
+ *     work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream) and is CUDA-graph
+ *     capturable: every step-varying quantity (seq_lens, q_pos, budgets, cache_pos) lives in device memory
+ *     and grids are sized from the descriptor's upper bounds only.
+ *   - Device pointers must be 16-byte aligned.  Validation is host-side only (null / shape / alignment).
+ *   - `w` = desc->window counts PAST queries (the paper's window counts the current one: w_paper = w + 1);
+ *     w = 0 is plain Quest sparse attention and needs no mask / cache buffers.
+ *   - t_b = seq_lens[b] - 1 is the position of sequence b's current token.  "Decode step" and "position of the
+ *     current token" are the same number, so the retrospective mask A stores positions.
+ *
+ * Layouts (row-major, innermost last; T = desc->dtype element, P = page_size, d = head_dim):
+ *   k_pages, v_pages [num_phys_pages][h_k][P][d] T   each (page, KV head) tile is contiguous (4 KB for bf16 d128).
+ *                                                   Slots at positions >= seq_len must hold FINITE values.
+ *   block_table      [B][max_pages_per_seq] int32   logical page j of sequence b -> physical page
+ *   seq_lens         [B] int32                      tokens valid in sequence b, current token included
+ *   bounds           [B][h_k][max_pages_per_seq][2][d] T   [..][0][:] = Kmax, [..][1][:] = Kmin
+ *   last_loaded (A)  [B][h_k][max_pages_per_seq] int32     last position whose step loaded the page, -1 = never
+ *   sel_pages        [B][h_k][max_sel_pages] int32  selected LOGICAL pages, ascending, -1 beyond sel_count
+ *   sel_prev  (M)    [B][h_k][max_sel_pages] int32  A[page] before this step's update, -1 beyond sel_count
+ *   sel_count        [B][h_k] int32
+ *   q_cur            [B][h_q][d] T                  the current query (drives selection)
+ *   q_win            [B][w+1][h_q][d] T             window rows in ANY order
+ *   q_pos            [B][w+1] int32                 position of each row, -1 = empty row; the row whose position
+ *                                                   is seq_lens[b]-1 is the current query; rows outside
+ *                                                   [t-w, t] are treated as empty
+ *   part_o           [B][w+1][h_q][d] float         normalised partial output of each row over its unseen pages
+ *   part_lse         [B][w+1][h_q] float            natural-log sum-exp of the same; empty set -> o = 0, lse = -inf
+ *   cache_o          [B][w][h_q][d] float           output cache ring, slot = position mod w
+ *   cache_lse        [B][w][h_q] float
+ *   cache_pos        [B][w] int32                   position held by each slot, -1 = empty
+ *   out              [B][w+1][h_q][d] T             merged outputs, row r belongs to q_pos[b][r]; empty rows = 0
+ *   out_lse          [B][w+1][h_q] float            optional (may be NULL)
+ */
+#ifndef RETRO_H_
+#define RETRO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RETRO_OK 0
+#define RETRO_ERR_ARG (-1)         /* null pointer, non-positive dim, h_q % h_k != 0, misaligned pointer      */
+#define RETRO_ERR_UNSUPPORTED (-2) /* (dtype, head_dim, page_size) not instantiated, or a size limit exceeded */
+#define RETRO_ERR_WORKSPACE (-3)   /* workspace smaller than retro_workspace_bytes()                          */
+#define RETRO_ERR_CUDA (-4)        /* launch / runtime error; retro_last_cuda_error() returns the cudaError_t */
+
+#define RETRO_F32 0
+#define RETRO_BF16 1
+#define RETRO_GROUP_SUM 0 /* Eq. 1 scores of a KV head's q heads are summed (default; reading Q2) */
+#define RETRO_GROUP_MAX 1
+
+/* Supported instantiations: {RETRO_F32, head_dim 64, page_size 16}, {RETRO_BF16, head_dim 128, page_size 16}.
+ * Limits: window <= 32, group (h_q / h_k) <= 8, max_pages_per_seq <= 24576. */
+typedef struct retro_desc {
+  int32_t batch;             /* B                                                              */
+  int32_t num_q_heads;       /* h_q                                                            */
+  int32_t num_kv_heads;      /* h_k, divides h_q                                               */
+  int32_t head_dim;          /* d                                                              */
+  int32_t page_size;         /* P tokens per page                                              */
+  int32_t max_pages_per_seq; /* row stride of block_table / bounds / last_loaded               */
+  int32_t max_sel_pages;     /* k_max: row stride of sel_pages / sel_prev, upper bound on k    */
+  int32_t num_phys_pages;    /* pages in the K/V pools                                         */
+  int32_t window;            /* w = number of PAST queries; 0 = plain Quest                    */
+  int32_t dtype;             /* RETRO_F32 | RETRO_BF16: q, K, V, bounds, out                   */
+  int32_t group_reduce;      /* RETRO_GROUP_SUM | RETRO_GROUP_MAX                              */
+  int32_t force_last_page;   /* 1: newest page always selected and counted in k (reading Q3)   */
+  float sm_scale;            /* softmax scale, 1/sqrt(head_dim)                  */
+} retro_desc_t;
+
+/* Bytes of scratch the S2/S3 entry points need for this descriptor (page scores, split-KV partials,
+ * arrival counters).  HOST pointers.  The workspace must be passed to retro_workspace_init() once after
+ * allocation; the library leaves it consistent after every call. */
+int retro_workspace_bytes(const retro_desc_t* desc /*HOST*/, size_t* bytes /*HOST out*/);
+int retro_workspace_init(const retro_desc_t* desc /*HOST*/, void* workspace, size_t ws_bytes, void* stream);
+
+const char* retro_error_string(int code);
+int retro_last_cuda_error(void);
+int retro_version(void);
+
+/* S1.  For every sequence b, recompute the digests of the logical pages that overlap positions
+ * [pos_begin[b], seq_lens[b]): per channel, max and min of K over the page's VALID tokens (l < seq_len).
+ * At most `max_touched_pages` pages per sequence are updated, starting at page pos_begin[b] / P (HOST int:
+ * 1 for a decode step with pos_begin = seq_len - 1; max_pages_per_seq for a rebuild after prefill).
+ * pos_begin == NULL means pos_begin[b] = seq_lens[b] - 1 (only the newest token's page).
+ * Bit-exact: min/max of T values is a T value. */
+int retro_update_page_bounds(const retro_desc_t* desc, const void* k_pages, const int32_t* block_table,
+                             const int32_t* seq_lens, const int32_t* pos_begin /*[B]*/,
+                             int32_t max_touched_pages /*HOST*/, void* bounds, void* stream);
+
+/* S2 (Eq. 1; top-k PAPER.md:42, 248; Alg. 2).  Per (b, KV head):
+ * score_j = reduce over the head's q heads g of sum_c max(q_gc * Kmin_jc, q_gc * Kmax_jc), accumulated in fp64;
+ * k = min(budget_pages[b], #pages, max_sel_pages); k == #pages selects every page, else the newest page (if
+ * force_last_page) plus the best of the others ordered by (score desc, index asc); emitted ascending.
+ * Then M_i = A[page_i] -> sel_prev and A[page_i] = seq_lens[b] - 1.  last_loaded may be NULL iff window == 0
+ * (sel_prev is then filled with -1).  scores_out (optional, [B][h_k][max_pages_per_seq] double, -inf for pages
+ * that do not exist) exposes the fp64 scores for tests. */
+int retro_select_pages(const retro_desc_t* desc, const void* q_cur, const void* bounds, const int32_t* seq_lens,
+                       const int32_t* budget_pages /*[B]*/, int32_t* last_loaded, int32_t* sel_pages,
+                       int32_t* sel_prev, int32_t* sel_count, double* scores_out, void* workspace,
+                       size_t ws_bytes, void* stream);
+
+/* S3 (Eq. 2 / 6 / 7; Alg. 1 line 6).  For every non-empty window row r at position p and
+ * every q head: softmax(q K^T * sm_scale) V over the tokens l of the selected pages j with sel_prev_j < p (page
+ * not yet seen by that query), l <= p and l < seq_len.  The current row (p = t) sees all of S_t (O_org); a past
+ * row sees only its unseen pages (O_sup).  Each selected page is read from HBM once and serves every row of the
+ * GQA group x (w+1) block.  fp32 accumulation and softmax.  A pure function of its inputs. */
+int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32_t* q_pos, const void* k_pages,
+                        const void* v_pages, const int32_t* block_table, const int32_t* seq_lens,
+                        const int32_t* sel_pages, const int32_t* sel_prev, const int32_t* sel_count,
+                        float* part_o, float* part_lse, void* workspace, size_t ws_bytes, void* stream);
+
+/* S4 (Eq. 8-9 with alpha = e^lse; push / update / pop; Alg. 1 lines 7-8).
+ * Past row at position p (t-w <= p < t): (o, lse) = merge(cache[p mod w] if cache_pos == p, part); emitted to
+ * `out`; written back to its slot unless p = t-w (popped after its last merge).  Current row: out = part, pushed
+ * into slot t mod w.  window == 0: out = part, cache_* may be NULL. */
+int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, const float* part_lse,
+                             const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                             int32_t* cache_pos, void* out, float* out_lse, void* stream);
+
+/* AppendKV (Alg. 1 line 3).  Writes k_new / v_new [B][h_k][d] T into position seq_lens[b] - 1 of
+ * each sequence (seq_lens already counts the new token). */
+int retro_append_kv(const retro_desc_t* desc, const void* k_new, const void* v_new, const int32_t* block_table,
+                    const int32_t* seq_lens, void* k_pages, void* v_pages, void* stream);
+
+/* One layer's persistent device state, for the whole-step entry points below. */
+typedef struct retro_layer_state {
+  void* k_pages;
+  void* v_pages;
+  int32_t* block_table;
+  int32_t* seq_lens;
+  int32_t* budget_pages; /* [B] */
+  void* bounds;
+  int32_t* last_loaded;
+  int32_t* sel_pages;
+  int32_t* sel_prev;
+  int32_t* sel_count;
+  float* part_o;
+  float* part_lse;
+  float* cache_o;
+  float* cache_lse;
+  int32_t* cache_pos;
+  void* workspace;
+  size_t workspace_bytes;
+} retro_layer_state_t;
+
+/* S1..S4 of Alg. 1 back to back on `stream` for one layer (digest refresh of the newest page, select, attend,
+ * merge).  seq_lens already counts the current token.  Same results as the four calls above. */
+int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st /*HOST struct of device ptrs*/,
+                      const void* q_win, const int32_t* q_pos, const void* q_cur, void* out, float* out_lse,
+                      void* stream);
+
+/* End-to-end step with HOST buffers (pinned for async copies): copies this step's inputs host->device
+ * (q_new, k_new, v_new: the new token's query [B][h_q][d] and key/value [B][h_k][d]), advances seq_lens and the
+ * query window ring on the device, appends the token to the KV pool, runs retro_decode_step, and copies
+ * out [B][w+1][h_q][d] device->host.  dev_io holds caller-owned device staging buffers. */
+typedef struct retro_step_io {
+  void* q_new;      /* device [B][h_q][d] T            */
+  void* k_new;      /* device [B][h_k][d] T            */
+  void* v_new;      /* device [B][h_k][d] T            */
+  void* q_win;      /* device [B][w+1][h_q][d] T ring  */
+  int32_t* q_pos;   /* device [B][w+1]                 */
+  void* out;        /* device [B][w+1][h_q][d] T       */
+} retro_step_io_t;
+int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* dev_io,
+                           const void* host_q_new, const void* host_k_new, const void* host_v_new,
+                           void* host_out, void* stream);
+
+/* Window-ring bookkeeping used by the two calls above and by the synthetic benchmark: seq_lens[b] += 1;
+ * row (new position mod (w+1)) of q_win <- q_new[b], q_pos <- new position.  q_new [B][h_q][d] T.
+ * If step_counter != NULL, q_new is taken as q_pool[(*step_counter) % pool_steps] ([pool][B][h_q][d]) and the
+ * counter is incremented (lets a captured CUDA graph replay successive steps of a pre-generated query stream). */
+int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, int32_t* step_counter,
+                         int32_t pool_steps /*HOST*/, int32_t* seq_lens, void* q_win, int32_t* q_pos,
+                         void* q_cur_out /*optional [B][h_q][d]*/, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RETRO_H_ */

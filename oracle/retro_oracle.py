@@ -216,8 +216,8 @@ def sparse_attend(desc, q_win, q_pos, k_pages, v_pages, block_table, seq_lens,
                 if toks:
                     phys = [int(block_table[b, l // P]) for l in toks]
                     offs = [l % P for l in toks]
-                    keys = k_pages[phys, h, offs, :]
-                    vals = v_pages[phys, h, offs, :]
+                    keys = np.asarray(k_pages[phys, h, offs, :], dtype=np.float64)
+                    vals = np.asarray(v_pages[phys, h, offs, :], dtype=np.float64)
                 else:
                     keys = np.zeros((0, d)); vals = np.zeros((0, d))
                 for g in range(G):
@@ -293,8 +293,10 @@ def merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_l
 class OracleLayer:
     def __init__(self, desc: OracleDesc, k_pages, v_pages, block_table):
         self.desc = desc
-        self.k_pages = np.asarray(k_pages, dtype=np.float64)
-        self.v_pages = np.asarray(v_pages, dtype=np.float64)
+        # pools may be float32 (every bf16 / fp32 input value is exact in it) to halve host memory at full
+        # size; all arithmetic upcasts to float64 first (min/max digests are exact in any float type)
+        self.k_pages = np.asarray(k_pages)
+        self.v_pages = np.asarray(v_pages)
         self.block_table = np.asarray(block_table, dtype=np.int64)
         B, hk, hq, d, w = desc.batch, desc.num_kv_heads, desc.num_q_heads, desc.head_dim, desc.window
         self.bounds = np.zeros((B, hk, desc.max_pages_per_seq, 2, d), dtype=np.float64)

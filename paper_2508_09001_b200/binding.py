@@ -1,0 +1,225 @@
+"""Thin ctypes binding of libretro.so (include/retro.h): argument marshalling only.
+
+Every function has the name of its C entry point and takes torch tensors (device memory, owned by the
+caller) whose data pointers are passed through; nothing is computed here.  If the library is missing it is
+built with nvcc; if that fails the import raises — there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+from typing import Optional
+
+import torch
+
+from . import build as _build
+
+RETRO_OK = 0
+RETRO_ERR_ARG, RETRO_ERR_UNSUPPORTED, RETRO_ERR_WORKSPACE, RETRO_ERR_CUDA = -1, -2, -3, -4
+RETRO_F32, RETRO_BF16 = 0, 1
+RETRO_GROUP_SUM, RETRO_GROUP_MAX = 0, 1
+
+EXPORTED = [
+    "retro_workspace_bytes", "retro_workspace_init", "retro_error_string", "retro_last_cuda_error",
+    "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
+    "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
+    "retro_window_advance",
+]
+
+
+class RetroDesc(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in (
+        "batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size", "max_pages_per_seq", "max_sel_pages",
+        "num_phys_pages", "window", "dtype", "group_reduce", "force_last_page")] + [("sm_scale", C.c_float)]
+
+    @property
+    def group(self):
+        return self.num_q_heads // self.num_kv_heads
+
+    @property
+    def torch_dtype(self):
+        return torch.bfloat16 if self.dtype == RETRO_BF16 else torch.float32
+
+
+class RetroLayerState(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in (
+        "k_pages", "v_pages", "block_table", "seq_lens", "budget_pages", "bounds", "last_loaded", "sel_pages",
+        "sel_prev", "sel_count", "part_o", "part_lse", "cache_o", "cache_lse", "cache_pos", "workspace")] + [
+        ("workspace_bytes", C.c_size_t)]
+
+
+class RetroStepIO(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("q_new", "k_new", "v_new", "q_win", "q_pos", "out")]
+
+
+class RetroError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = _lib().retro_error_string(code).decode()
+        extra = f" (cudaError {_lib().retro_last_cuda_error()})" if code == RETRO_ERR_CUDA else ""
+        super().__init__(f"{where}: {msg}{extra}")
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        path = _build.build()          # no-op when up to date; raises if nvcc fails
+        lib = C.CDLL(path)
+        lib.retro_error_string.restype = C.c_char_p
+        lib.retro_error_string.argtypes = [C.c_int]
+        for name in EXPORTED:
+            getattr(lib, name)          # fail loudly on a missing symbol
+        _LIB = lib
+    return _LIB
+
+
+def library_path() -> str:
+    _lib()
+    return _build.LIB_PATH
+
+
+def _p(t: Optional[torch.Tensor]):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_contiguous(), "libretro takes contiguous tensors"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> C.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _check(rc: int, where: str):
+    if rc != RETRO_OK:
+        raise RetroError(rc, where)
+
+
+def make_desc(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_pages_per_seq, max_sel_pages,
+              num_phys_pages, window, dtype, group_reduce=RETRO_GROUP_SUM, force_last_page=1,
+              sm_scale=None) -> RetroDesc:
+    if isinstance(dtype, torch.dtype):
+        dtype = RETRO_BF16 if dtype == torch.bfloat16 else RETRO_F32
+    elif isinstance(dtype, str):
+        dtype = RETRO_BF16 if dtype == "bf16" else RETRO_F32
+    return RetroDesc(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_pages_per_seq, max_sel_pages,
+                     num_phys_pages, window, dtype, group_reduce, int(force_last_page),
+                     1.0 / math.sqrt(head_dim) if sm_scale is None else sm_scale)
+
+
+def retro_version() -> int:
+    return _lib().retro_version()
+
+
+def retro_error_string(code: int) -> str:
+    return _lib().retro_error_string(code).decode()
+
+
+def retro_last_cuda_error() -> int:
+    return _lib().retro_last_cuda_error()
+
+
+def retro_workspace_bytes(desc: RetroDesc) -> int:
+    n = C.c_size_t(0)
+    _check(_lib().retro_workspace_bytes(C.byref(desc), C.byref(n)), "retro_workspace_bytes")
+    return n.value
+
+
+def retro_workspace_init(desc, workspace, stream=None):
+    _check(_lib().retro_workspace_init(C.byref(desc), _p(workspace), C.c_size_t(workspace.numel()),
+                                       _stream(stream)), "retro_workspace_init")
+
+
+def retro_update_page_bounds(desc, k_pages, block_table, seq_lens, pos_begin, max_touched_pages, bounds, stream=None):
+    _check(_lib().retro_update_page_bounds(C.byref(desc), _p(k_pages), _p(block_table), _p(seq_lens), _p(pos_begin),
+                                           C.c_int32(max_touched_pages), _p(bounds), _stream(stream)),
+           "retro_update_page_bounds")
+
+
+def retro_select_pages(desc, q_cur, bounds, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev, sel_count,
+                       scores_out, workspace, stream=None):
+    _check(_lib().retro_select_pages(C.byref(desc), _p(q_cur), _p(bounds), _p(seq_lens), _p(budget_pages),
+                                     _p(last_loaded), _p(sel_pages), _p(sel_prev), _p(sel_count), _p(scores_out),
+                                     _p(workspace), C.c_size_t(workspace.numel()), _stream(stream)),
+           "retro_select_pages")
+
+
+def retro_sparse_attend(desc, q_win, q_pos, k_pages, v_pages, block_table, seq_lens, sel_pages, sel_prev, sel_count,
+                        part_o, part_lse, workspace, stream=None):
+    _check(_lib().retro_sparse_attend(C.byref(desc), _p(q_win), _p(q_pos), _p(k_pages), _p(v_pages), _p(block_table),
+                                      _p(seq_lens), _p(sel_pages), _p(sel_prev), _p(sel_count), _p(part_o),
+                                      _p(part_lse), _p(workspace), C.c_size_t(workspace.numel()), _stream(stream)),
+           "retro_sparse_attend")
+
+
+def retro_merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse, cache_pos, out, out_lse,
+                             stream=None):
+    _check(_lib().retro_merge_output_cache(C.byref(desc), _p(part_o), _p(part_lse), _p(q_pos), _p(seq_lens),
+                                           _p(cache_o), _p(cache_lse), _p(cache_pos), _p(out), _p(out_lse),
+                                           _stream(stream)), "retro_merge_output_cache")
+
+
+def retro_append_kv(desc, k_new, v_new, block_table, seq_lens, k_pages, v_pages, stream=None):
+    _check(_lib().retro_append_kv(C.byref(desc), _p(k_new), _p(v_new), _p(block_table), _p(seq_lens), _p(k_pages),
+                                  _p(v_pages), _stream(stream)), "retro_append_kv")
+
+
+def retro_window_advance(desc, q_new_or_pool, step_counter, pool_steps, seq_lens, q_win, q_pos, q_cur_out,
+                         stream=None):
+    _check(_lib().retro_window_advance(C.byref(desc), _p(q_new_or_pool), _p(step_counter), C.c_int32(pool_steps),
+                                       _p(seq_lens), _p(q_win), _p(q_pos), _p(q_cur_out), _stream(stream)),
+           "retro_window_advance")
+
+
+def retro_decode_step(desc, state: RetroLayerState, q_win, q_pos, q_cur, out, out_lse=None, stream=None):
+    _check(_lib().retro_decode_step(C.byref(desc), C.byref(state), _p(q_win), _p(q_pos), _p(q_cur), _p(out),
+                                    _p(out_lse), _stream(stream)), "retro_decode_step")
+
+
+def retro_decode_step_host(desc, state: RetroLayerState, io: RetroStepIO, host_q_new, host_k_new, host_v_new,
+                           host_out, stream=None):
+    _check(_lib().retro_decode_step_host(C.byref(desc), C.byref(state), C.byref(io), _p(host_q_new), _p(host_k_new),
+                                         _p(host_v_new), _p(host_out), _stream(stream)), "retro_decode_step_host")
+
+
+class LayerBuffers:
+    """Caller-side allocation of one layer's device buffers (torch only allocates) + the C state struct."""
+
+    def __init__(self, desc: RetroDesc, k_pages, v_pages, block_table, seq_lens, budget_pages, device="cuda"):
+        d = desc
+        dev = torch.device(device)
+        dt = d.torch_dtype
+        B, hq, hk, D, w = d.batch, d.num_q_heads, d.num_kv_heads, d.head_dim, d.window
+        self.desc = d
+        self.k_pages, self.v_pages, self.block_table = k_pages, v_pages, block_table
+        self.seq_lens, self.budget_pages = seq_lens, budget_pages
+        self.bounds = torch.zeros((B, hk, d.max_pages_per_seq, 2, D), dtype=dt, device=dev)
+        self.last_loaded = torch.full((B, hk, d.max_pages_per_seq), -1, dtype=torch.int32, device=dev)
+        self.sel_pages = torch.full((B, hk, d.max_sel_pages), -1, dtype=torch.int32, device=dev)
+        self.sel_prev = torch.full((B, hk, d.max_sel_pages), -1, dtype=torch.int32, device=dev)
+        self.sel_count = torch.zeros((B, hk), dtype=torch.int32, device=dev)
+        self.part_o = torch.zeros((B, w + 1, hq, D), dtype=torch.float32, device=dev)
+        self.part_lse = torch.full((B, w + 1, hq), -math.inf, dtype=torch.float32, device=dev)
+        self.cache_o = torch.zeros((B, max(w, 1), hq, D), dtype=torch.float32, device=dev)
+        self.cache_lse = torch.full((B, max(w, 1), hq), -math.inf, dtype=torch.float32, device=dev)
+        self.cache_pos = torch.full((B, max(w, 1)), -1, dtype=torch.int32, device=dev)
+        self.out = torch.zeros((B, w + 1, hq, D), dtype=dt, device=dev)
+        self.out_lse = torch.zeros((B, w + 1, hq), dtype=torch.float32, device=dev)
+        self.q_win = torch.zeros((B, w + 1, hq, D), dtype=dt, device=dev)
+        self.q_pos = torch.full((B, w + 1), -1, dtype=torch.int32, device=dev)
+        self.q_cur = torch.zeros((B, hq, D), dtype=dt, device=dev)
+        self.workspace = torch.zeros(retro_workspace_bytes(d), dtype=torch.uint8, device=dev)
+        retro_workspace_init(d, self.workspace)
+        self.state = RetroLayerState(*[t.data_ptr() for t in (
+            self.k_pages, self.v_pages, self.block_table, self.seq_lens, self.budget_pages, self.bounds,
+            self.last_loaded, self.sel_pages, self.sel_prev, self.sel_count, self.part_o, self.part_lse,
+            self.cache_o, self.cache_lse, self.cache_pos, self.workspace)], self.workspace.numel())
+
+    def rebuild_bounds(self, stream=None):
+        zero = torch.zeros(self.desc.batch, dtype=torch.int32, device=self.seq_lens.device)
+        retro_update_page_bounds(self.desc, self.k_pages, self.block_table, self.seq_lens, zero,
+                                 self.desc.max_pages_per_seq, self.bounds, stream)

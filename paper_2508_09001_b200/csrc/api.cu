@@ -1,0 +1,235 @@
+// C ABI of libretro (include/retro.h): host-side validation, workspace layout, entry points.
+#include <atomic>
+
+#include "common.cuh"
+
+namespace retro {
+
+static std::atomic<int> g_last_cuda_error{0};
+void set_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
+
+int validate_desc(const retro_desc_t* d) {
+  if (d == nullptr) return RETRO_ERR_ARG;
+  if (d->batch <= 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->head_dim <= 0 || d->page_size <= 0 ||
+      d->max_pages_per_seq <= 0 || d->max_sel_pages < 1 || d->num_phys_pages <= 0 || d->window < 0)
+    return RETRO_ERR_ARG;
+  if (d->num_q_heads % d->num_kv_heads != 0) return RETRO_ERR_ARG;
+  if (d->group_reduce != RETRO_GROUP_SUM && d->group_reduce != RETRO_GROUP_MAX) return RETRO_ERR_ARG;
+  if (!(d->sm_scale > 0.f)) return RETRO_ERR_ARG;
+  const bool f32 = d->dtype == RETRO_F32 && d->head_dim == 64 && d->page_size == 16;
+  const bool bf16 = d->dtype == RETRO_BF16 && d->head_dim == 128 && d->page_size == 16;
+  if (!f32 && !bf16) return RETRO_ERR_UNSUPPORTED;
+  if (d->window > kMaxWindow || d->num_q_heads / d->num_kv_heads > kMaxGroup ||
+      d->max_pages_per_seq > kMaxPagesPerSeq || d->batch > 65535)
+    return RETRO_ERR_UNSUPPORTED;
+  return RETRO_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+WorkspaceLayout workspace_layout(const retro_desc_t* d) {
+  WorkspaceLayout wl;
+  const int units = d->batch * d->num_kv_heads;
+  wl.rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
+  // split-KV so that units * nsplit covers the 148 SMs about twice; at least 2 pages per split
+  int nsplit = ceil_div(2 * 148, units);
+  const int max_split = d->max_sel_pages >= 2 ? d->max_sel_pages / 2 : 1;
+  if (nsplit > max_split) nsplit = max_split;
+  if (nsplit < 1) nsplit = 1;
+  wl.pages_per_split = ceil_div(d->max_sel_pages, nsplit);
+  wl.nsplit = ceil_div(d->max_sel_pages, wl.pages_per_split);
+  size_t off = 0;
+  wl.scores_off = off;
+  off = align_up(off + (size_t)units * d->max_pages_per_seq * sizeof(double), 256);
+  wl.split_o_off = off;
+  off = align_up(off + (size_t)units * wl.nsplit * wl.rows * d->head_dim * sizeof(float), 256);
+  wl.split_lse_off = off;
+  off = align_up(off + (size_t)units * wl.nsplit * wl.rows * sizeof(float), 256);
+  wl.counters_off = off;
+  off = align_up(off + (size_t)2 * units * sizeof(unsigned int), 256);
+  wl.total = off;
+  return wl;
+}
+
+}  // namespace retro
+
+using namespace retro;
+
+#define RETRO_CHECK_DESC(d)              \
+  do {                                   \
+    const int rc__ = validate_desc(d);   \
+    if (rc__ != RETRO_OK) return rc__;   \
+  } while (0)
+#define RETRO_CHECK_PTR(p) \
+  if ((p) == nullptr || !aligned16(p)) return RETRO_ERR_ARG
+
+extern "C" {
+
+int retro_version(void) { return 100; }
+
+const char* retro_error_string(int code) {
+  switch (code) {
+    case RETRO_OK: return "ok";
+    case RETRO_ERR_ARG: return "invalid argument (null / misaligned pointer or bad dimension)";
+    case RETRO_ERR_UNSUPPORTED: return "unsupported (dtype, head_dim, page_size) combination or size limit";
+    case RETRO_ERR_WORKSPACE: return "workspace too small";
+    case RETRO_ERR_CUDA: return "CUDA error (see retro_last_cuda_error)";
+    default: return "unknown error code";
+  }
+}
+
+int retro_last_cuda_error(void) { return g_last_cuda_error.load(); }
+
+int retro_workspace_bytes(const retro_desc_t* desc, size_t* bytes) {
+  RETRO_CHECK_DESC(desc);
+  if (bytes == nullptr) return RETRO_ERR_ARG;
+  *bytes = workspace_layout(desc).total;
+  return RETRO_OK;
+}
+
+int retro_workspace_init(const retro_desc_t* desc, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(workspace);
+  const WorkspaceLayout wl = workspace_layout(desc);
+  if (ws_bytes < wl.total) return RETRO_ERR_WORKSPACE;
+  RETRO_CUDA_TRY(cudaMemsetAsync(static_cast<char*>(workspace) + wl.counters_off, 0, wl.total - wl.counters_off,
+                                 (cudaStream_t)stream));
+  return RETRO_OK;
+}
+
+int retro_update_page_bounds(const retro_desc_t* desc, const void* k_pages, const int32_t* block_table,
+                             const int32_t* seq_lens, const int32_t* pos_begin, int32_t max_touched_pages,
+                             void* bounds, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(bounds);
+  if (pos_begin != nullptr && !aligned16(pos_begin)) return RETRO_ERR_ARG;
+  if (max_touched_pages < 1) return RETRO_ERR_ARG;
+  return launch_update_page_bounds(desc, k_pages, block_table, seq_lens, pos_begin, max_touched_pages, bounds,
+                                   (cudaStream_t)stream);
+}
+
+int retro_select_pages(const retro_desc_t* desc, const void* q_cur, const void* bounds, const int32_t* seq_lens,
+                       const int32_t* budget_pages, int32_t* last_loaded, int32_t* sel_pages, int32_t* sel_prev,
+                       int32_t* sel_count, double* scores_out, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(q_cur); RETRO_CHECK_PTR(bounds); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(budget_pages);
+  RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(workspace);
+  if (last_loaded == nullptr && desc->window != 0) return RETRO_ERR_ARG;
+  if (last_loaded != nullptr && !aligned16(last_loaded)) return RETRO_ERR_ARG;
+  if (scores_out != nullptr && !aligned16(scores_out)) return RETRO_ERR_ARG;
+  const WorkspaceLayout wl = workspace_layout(desc);
+  if (ws_bytes < wl.total) return RETRO_ERR_WORKSPACE;
+  return launch_select_pages(desc, wl, q_cur, bounds, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev,
+                             sel_count, scores_out, workspace, (cudaStream_t)stream);
+}
+
+int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32_t* q_pos, const void* k_pages,
+                        const void* v_pages, const int32_t* block_table, const int32_t* seq_lens,
+                        const int32_t* sel_pages, const int32_t* sel_prev, const int32_t* sel_count, float* part_o,
+                        float* part_lse, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(q_win); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
+  RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev);
+  RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(part_o); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(workspace);
+  const WorkspaceLayout wl = workspace_layout(desc);
+  if (ws_bytes < wl.total) return RETRO_ERR_WORKSPACE;
+  return launch_sparse_attend(desc, wl, q_win, q_pos, k_pages, v_pages, block_table, seq_lens, sel_pages, sel_prev,
+                              sel_count, part_o, part_lse, workspace, (cudaStream_t)stream);
+}
+
+int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, const float* part_lse,
+                             const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                             int32_t* cache_pos, void* out, float* out_lse, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(part_o); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(seq_lens);
+  RETRO_CHECK_PTR(out);
+  if (desc->window > 0) { RETRO_CHECK_PTR(cache_o); RETRO_CHECK_PTR(cache_lse); RETRO_CHECK_PTR(cache_pos); }
+  if (out_lse != nullptr && !aligned16(out_lse)) return RETRO_ERR_ARG;
+  return launch_merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse, cache_pos, out,
+                                   out_lse, (cudaStream_t)stream);
+}
+
+int retro_append_kv(const retro_desc_t* desc, const void* k_new, const void* v_new, const int32_t* block_table,
+                    const int32_t* seq_lens, void* k_pages, void* v_pages, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(k_new); RETRO_CHECK_PTR(v_new); RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens);
+  RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
+  return launch_append_kv(desc, k_new, v_new, block_table, seq_lens, k_pages, v_pages, (cudaStream_t)stream);
+}
+
+int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, int32_t* step_counter,
+                         int32_t pool_steps, int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out,
+                         void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(q_new_or_pool); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(q_win); RETRO_CHECK_PTR(q_pos);
+  if (step_counter != nullptr && pool_steps < 1) return RETRO_ERR_ARG;
+  if (q_cur_out != nullptr && !aligned16(q_cur_out)) return RETRO_ERR_ARG;
+  return launch_window_advance(desc, q_new_or_pool, step_counter, pool_steps, seq_lens, q_win, q_pos, q_cur_out,
+                               (cudaStream_t)stream);
+}
+
+static int check_state(const retro_desc_t* desc, const retro_layer_state_t* st) {
+  if (st == nullptr) return RETRO_ERR_ARG;
+  RETRO_CHECK_PTR(st->k_pages); RETRO_CHECK_PTR(st->v_pages); RETRO_CHECK_PTR(st->block_table);
+  RETRO_CHECK_PTR(st->seq_lens); RETRO_CHECK_PTR(st->budget_pages); RETRO_CHECK_PTR(st->bounds);
+  RETRO_CHECK_PTR(st->sel_pages); RETRO_CHECK_PTR(st->sel_prev); RETRO_CHECK_PTR(st->sel_count);
+  RETRO_CHECK_PTR(st->part_o); RETRO_CHECK_PTR(st->part_lse); RETRO_CHECK_PTR(st->workspace);
+  if (desc->window > 0) {
+    RETRO_CHECK_PTR(st->last_loaded); RETRO_CHECK_PTR(st->cache_o); RETRO_CHECK_PTR(st->cache_lse);
+    RETRO_CHECK_PTR(st->cache_pos);
+  }
+  return RETRO_OK;
+}
+
+int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
+                      const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  int rc = check_state(desc, st);
+  if (rc != RETRO_OK) return rc;
+  RETRO_CHECK_PTR(q_win); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(q_cur); RETRO_CHECK_PTR(out);
+  const WorkspaceLayout wl = workspace_layout(desc);
+  if (st->workspace_bytes < wl.total) return RETRO_ERR_WORKSPACE;
+  cudaStream_t s = (cudaStream_t)stream;
+  // S1: the newest token's page.  pos_begin = seq_len - 1 is expressed by passing seq_lens with a -1 bias:
+  // the bounds kernel takes pos_begin from an array, so the per-step path uses the dedicated "tail" mode.
+  rc = launch_update_page_bounds(desc, st->k_pages, st->block_table, st->seq_lens, nullptr, 1, st->bounds, s);
+  if (rc != RETRO_OK) return rc;
+  rc = launch_select_pages(desc, wl, q_cur, st->bounds, st->seq_lens, st->budget_pages, st->last_loaded,
+                           st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s);
+  if (rc != RETRO_OK) return rc;
+  rc = launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
+                            st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s);
+  if (rc != RETRO_OK) return rc;
+  return launch_merge_output_cache(desc, st->part_o, st->part_lse, q_pos, st->seq_lens, st->cache_o, st->cache_lse,
+                                   st->cache_pos, out, out_lse, s);
+}
+
+int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* io,
+                           const void* host_q_new, const void* host_k_new, const void* host_v_new, void* host_out,
+                           void* stream) {
+  RETRO_CHECK_DESC(desc);
+  int rc = check_state(desc, st);
+  if (rc != RETRO_OK) return rc;
+  if (io == nullptr || host_q_new == nullptr || host_k_new == nullptr || host_v_new == nullptr ||
+      host_out == nullptr)
+    return RETRO_ERR_ARG;
+  RETRO_CHECK_PTR(io->q_new); RETRO_CHECK_PTR(io->k_new); RETRO_CHECK_PTR(io->v_new); RETRO_CHECK_PTR(io->q_win);
+  RETRO_CHECK_PTR(io->q_pos); RETRO_CHECK_PTR(io->out);
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t esz = desc->dtype == RETRO_BF16 ? 2 : 4;
+  const size_t q_bytes = (size_t)desc->batch * desc->num_q_heads * desc->head_dim * esz;
+  const size_t kv_bytes = (size_t)desc->batch * desc->num_kv_heads * desc->head_dim * esz;
+  RETRO_CUDA_TRY(cudaMemcpyAsync(io->q_new, host_q_new, q_bytes, cudaMemcpyHostToDevice, s));
+  RETRO_CUDA_TRY(cudaMemcpyAsync(io->k_new, host_k_new, kv_bytes, cudaMemcpyHostToDevice, s));
+  RETRO_CUDA_TRY(cudaMemcpyAsync(io->v_new, host_v_new, kv_bytes, cudaMemcpyHostToDevice, s));
+  rc = launch_window_advance(desc, io->q_new, nullptr, 1, st->seq_lens, io->q_win, io->q_pos, nullptr, s);
+  if (rc != RETRO_OK) return rc;
+  rc = launch_append_kv(desc, io->k_new, io->v_new, st->block_table, st->seq_lens, st->k_pages, st->v_pages, s);
+  if (rc != RETRO_OK) return rc;
+  rc = retro_decode_step(desc, st, io->q_win, io->q_pos, io->q_new, io->out, nullptr, stream);
+  if (rc != RETRO_OK) return rc;
+  RETRO_CUDA_TRY(cudaMemcpyAsync(host_out, io->out, q_bytes * (desc->window + 1), cudaMemcpyDeviceToHost, s));
+  return RETRO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,204 @@
+// S1  page-bound maintenance: per-channel max / min of K over each page's valid tokens.
+// Also AppendKV (Alg. 1 line 3) and the window-ring bookkeeping kernel.
+//
+// HBM-bound, comparisons only.  One warp per (sequence, KV head, touched page): a (page, head) K tile is
+// P*d*esize contiguous bytes; the warp streams it with 128-bit loads (a row of 256 B = 16 lanes), reduces
+// across the two half-warps with one shuffle and writes the [Kmax;Kmin] record (512 B) with 128-bit stores.
+#include "common.cuh"
+
+namespace retro {
+
+template <typename T> struct Vec16;
+template <> struct Vec16<float> {
+  __device__ static __forceinline__ uint4 vmax(uint4 a, uint4 b) {
+    uint4 r;
+    r.x = __float_as_uint(fmaxf(__uint_as_float(a.x), __uint_as_float(b.x)));
+    r.y = __float_as_uint(fmaxf(__uint_as_float(a.y), __uint_as_float(b.y)));
+    r.z = __float_as_uint(fmaxf(__uint_as_float(a.z), __uint_as_float(b.z)));
+    r.w = __float_as_uint(fmaxf(__uint_as_float(a.w), __uint_as_float(b.w)));
+    return r;
+  }
+  __device__ static __forceinline__ uint4 vmin(uint4 a, uint4 b) {
+    uint4 r;
+    r.x = __float_as_uint(fminf(__uint_as_float(a.x), __uint_as_float(b.x)));
+    r.y = __float_as_uint(fminf(__uint_as_float(a.y), __uint_as_float(b.y)));
+    r.z = __float_as_uint(fminf(__uint_as_float(a.z), __uint_as_float(b.z)));
+    r.w = __float_as_uint(fminf(__uint_as_float(a.w), __uint_as_float(b.w)));
+    return r;
+  }
+};
+template <> struct Vec16<__nv_bfloat16> {
+  __device__ static __forceinline__ uint32_t max2(uint32_t a, uint32_t b) {
+    __nv_bfloat162 r = __hmax2(*reinterpret_cast<__nv_bfloat162*>(&a), *reinterpret_cast<__nv_bfloat162*>(&b));
+    return *reinterpret_cast<uint32_t*>(&r);
+  }
+  __device__ static __forceinline__ uint32_t min2(uint32_t a, uint32_t b) {
+    __nv_bfloat162 r = __hmin2(*reinterpret_cast<__nv_bfloat162*>(&a), *reinterpret_cast<__nv_bfloat162*>(&b));
+    return *reinterpret_cast<uint32_t*>(&r);
+  }
+  __device__ static __forceinline__ uint4 vmax(uint4 a, uint4 b) {
+    return make_uint4(max2(a.x, b.x), max2(a.y, b.y), max2(a.z, b.z), max2(a.w, b.w));
+  }
+  __device__ static __forceinline__ uint4 vmin(uint4 a, uint4 b) {
+    return make_uint4(min2(a.x, b.x), min2(a.y, b.y), min2(a.z, b.z), min2(a.w, b.w));
+  }
+};
+
+__device__ __forceinline__ uint4 shfl_xor_u4(uint4 v, int m) {
+  v.x = __shfl_xor_sync(0xffffffffu, v.x, m);
+  v.y = __shfl_xor_sync(0xffffffffu, v.y, m);
+  v.z = __shfl_xor_sync(0xffffffffu, v.z, m);
+  v.w = __shfl_xor_sync(0xffffffffu, v.w, m);
+  return v;
+}
+
+// Row of D elements = kRowBytes; 16 lanes cover 256 B.  Instantiated for rows of exactly 256 B
+// ({f32, d64} and {bf16, d128}): two rows per warp pass.
+template <typename T, int D, int P>
+__global__ void __launch_bounds__(128) page_bounds_kernel(const T* __restrict__ k_pages,
+                                                          const int32_t* __restrict__ block_table,
+                                                          const int32_t* __restrict__ seq_lens,
+                                                          const int32_t* __restrict__ pos_begin, T* __restrict__ bounds,
+                                                          int B, int h_k, int max_pages, int max_touched) {
+  static_assert(D * sizeof(T) == 256, "one K row must be 256 bytes");
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  const int total = B * h_k * max_touched;
+  if (warp >= total) return;
+  const int jj = warp % max_touched;
+  const int h = (warp / max_touched) % h_k;
+  const int b = warp / (max_touched * h_k);
+  const int L = seq_lens[b];
+  if (L <= 0) return;
+  int pb = pos_begin != nullptr ? pos_begin[b] : L - 1;   // NULL: only the newest token's page
+  pb = pb < 0 ? 0 : pb;
+  const int j = pb / P + jj;
+  if (j > (L - 1) / P || j >= max_pages) return;
+  const int n_valid = min(P, L - j * P);
+  const int phys = block_table[(size_t)b * max_pages + j];
+  const uint4* tile = reinterpret_cast<const uint4*>(k_pages + ((size_t)phys * h_k + h) * P * D);
+  const int sub = lane >> 4;   // which of the two rows of a pass
+  const int col = lane & 15;   // 16-byte column within the row
+  uint4 vmax = make_uint4(0, 0, 0, 0), vmin = make_uint4(0, 0, 0, 0);
+  bool have = false;
+#pragma unroll
+  for (int r0 = 0; r0 < P; r0 += 2) {
+    const int row = r0 + sub;
+    if (row < n_valid) {
+      const uint4 v = __ldg(tile + row * 16 + col);
+      if (!have) {
+        vmax = v; vmin = v; have = true;
+      } else {
+        vmax = Vec16<T>::vmax(vmax, v);
+        vmin = Vec16<T>::vmin(vmin, v);
+      }
+    }
+  }
+  // combine the two half-warps; the odd half may be empty when n_valid == 1
+  uint4 omax = shfl_xor_u4(vmax, 16), omin = shfl_xor_u4(vmin, 16);
+  const bool ohave = __shfl_xor_sync(0xffffffffu, (int)have, 16) != 0;
+  if (have && ohave) {
+    vmax = Vec16<T>::vmax(vmax, omax);
+    vmin = Vec16<T>::vmin(vmin, omin);
+  } else if (!have) {
+    vmax = omax; vmin = omin;
+  }
+  uint4* rec = reinterpret_cast<uint4*>(bounds + (((size_t)b * h_k + h) * max_pages + j) * 2 * D);
+  rec[lane] = sub == 0 ? vmax : vmin;   // lanes 0..15 -> Kmax (256 B), lanes 16..31 -> Kmin (256 B)
+}
+
+int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const int32_t* block_table,
+                              const int32_t* seq_lens, const int32_t* pos_begin, int max_touched, void* bounds,
+                              cudaStream_t s) {
+  if (max_touched > d->max_pages_per_seq) max_touched = d->max_pages_per_seq;
+  const long long warps = (long long)d->batch * d->num_kv_heads * max_touched;
+  const int block = 128;
+  const unsigned grid = (unsigned)((warps * 32 + block - 1) / block);
+  if (d->dtype == RETRO_BF16) {
+    page_bounds_kernel<__nv_bfloat16, 128, 16><<<grid, block, 0, s>>>(
+        (const __nv_bfloat16*)k_pages, block_table, seq_lens, pos_begin, (__nv_bfloat16*)bounds, d->batch,
+        d->num_kv_heads, d->max_pages_per_seq, max_touched);
+  } else {
+    page_bounds_kernel<float, 64, 16><<<grid, block, 0, s>>>((const float*)k_pages, block_table, seq_lens, pos_begin,
+                                                             (float*)bounds, d->batch, d->num_kv_heads,
+                                                             d->max_pages_per_seq, max_touched);
+  }
+  RETRO_LAUNCH_CHECK();
+  return RETRO_OK;
+}
+
+// ---- AppendKV (Alg. 1 line 3): one token's K and V rows (256 B each) into the pool ----------------
+template <typename T, int D, int P>
+__global__ void append_kv_kernel(const T* __restrict__ k_new, const T* __restrict__ v_new,
+                                 const int32_t* __restrict__ block_table, const int32_t* __restrict__ seq_lens,
+                                 T* __restrict__ k_pages, T* __restrict__ v_pages, int B, int h_k, int max_pages) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // one 16 B chunk each: [B][h_k][2][16]
+  if (idx >= B * h_k * 32) return;
+  const int col = idx & 15, kv = (idx >> 4) & 1, h = (idx >> 5) % h_k, b = idx / (32 * h_k);
+  const int pos = seq_lens[b] - 1;
+  if (pos < 0) return;
+  const int phys = block_table[(size_t)b * max_pages + pos / P];
+  const T* src = (kv ? v_new : k_new) + ((size_t)b * h_k + h) * D;
+  T* dst = (kv ? v_pages : k_pages) + (((size_t)phys * h_k + h) * P + pos % P) * D;
+  reinterpret_cast<uint4*>(dst)[col] = reinterpret_cast<const uint4*>(src)[col];
+}
+
+int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
+                     const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s) {
+  const int n = d->batch * d->num_kv_heads * 32;
+  const int block = 128, grid = ceil_div(n, block);
+  if (d->dtype == RETRO_BF16) {
+    append_kv_kernel<__nv_bfloat16, 128, 16><<<grid, block, 0, s>>>(
+        (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new, block_table, seq_lens, (__nv_bfloat16*)k_pages,
+        (__nv_bfloat16*)v_pages, d->batch, d->num_kv_heads, d->max_pages_per_seq);
+  } else {
+    append_kv_kernel<float, 64, 16><<<grid, block, 0, s>>>((const float*)k_new, (const float*)v_new, block_table,
+                                                           seq_lens, (float*)k_pages, (float*)v_pages, d->batch,
+                                                           d->num_kv_heads, d->max_pages_per_seq);
+  }
+  RETRO_LAUNCH_CHECK();
+  return RETRO_OK;
+}
+
+// ---- window ring bookkeeping: seq_lens++, q_win[slot] <- q_new, q_pos[slot] <- new position -----------
+// Single CTA (the payload is B*h_q*256 bytes).  All threads read the step counter before thread 0 bumps it.
+__global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __restrict__ q_src, int32_t* step_counter,
+                                                               int pool_steps, int32_t* seq_lens, uint4* q_win,
+                                                               int32_t* q_pos, uint4* q_cur_out, int B, int h_q,
+                                                               int rows) {
+  __shared__ int s_pos[64];
+  const int row_chunks = h_q * 16;   // uint4 per [h_q][d] block (a q row is 256 B)
+  size_t src_off = 0;
+  if (step_counter != nullptr) src_off = (size_t)(*step_counter % pool_steps) * B * row_chunks;
+  for (int b = threadIdx.x; b < B; b += blockDim.x) {
+    const int pos = seq_lens[b];     // position of the token being appended
+    if (b < 64) s_pos[b] = pos;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < B * row_chunks; i += blockDim.x) {
+    const int b = i / row_chunks, c = i % row_chunks;
+    const int pos = s_pos[b];
+    const uint4 v = q_src[src_off + i];
+    q_win[((size_t)b * rows + pos % rows) * row_chunks + c] = v;
+    if (q_cur_out != nullptr) q_cur_out[i] = v;
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < B; b += blockDim.x) {
+    const int pos = s_pos[b];
+    q_pos[b * rows + pos % rows] = pos;
+    seq_lens[b] = pos + 1;
+  }
+  if (threadIdx.x == 0 && step_counter != nullptr) *step_counter += 1;
+}
+
+int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
+                          int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s) {
+  if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
+  window_advance_kernel<<<1, 1024, 0, s>>>((const uint4*)q_new_or_pool, step_counter, pool_steps, seq_lens,
+                                           (uint4*)q_win, q_pos, (uint4*)q_cur_out, d->batch, d->num_q_heads,
+                                           d->window + 1);
+  RETRO_LAUNCH_CHECK();
+  return RETRO_OK;
+}
+
+}  // namespace retro

@@ -1,0 +1,147 @@
+// Internal helpers of libretro (sm_100a).  Not part of the C ABI; see include/retro.h.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/retro.h"
+
+namespace retro {
+
+constexpr int kWarp = 32;
+constexpr int kMaxWindow = 32;
+constexpr int kMaxGroup = 8;
+constexpr int kMaxPagesPerSeq = 24576;
+
+// ---- error plumbing ---------------------------------------------------------------------------
+void set_cuda_error(cudaError_t e);
+#define RETRO_CUDA_TRY(expr)                      \
+  do {                                            \
+    cudaError_t e__ = (expr);                     \
+    if (e__ != cudaSuccess) {                     \
+      ::retro::set_cuda_error(e__);               \
+      return RETRO_ERR_CUDA;                      \
+    }                                             \
+  } while (0)
+#define RETRO_LAUNCH_CHECK() RETRO_CUDA_TRY(cudaGetLastError())
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+int validate_desc(const retro_desc_t* d);  // RETRO_OK / RETRO_ERR_ARG / RETRO_ERR_UNSUPPORTED
+
+// ---- workspace layout (host + device agree through this struct) --------------------------------
+struct WorkspaceLayout {
+  size_t scores_off;    // double [B][h_k][max_pages]
+  size_t split_o_off;   // float  [B][h_k][nsplit][rows][d]
+  size_t split_lse_off; // float  [B][h_k][nsplit][rows]
+  size_t counters_off;  // uint32 [B][h_k] split arrival counters (+ [B][h_k] score-chunk counters)
+  size_t total;
+  int nsplit;           // split-KV factor of the attend kernel
+  int pages_per_split;
+  int rows;             // G * (w+1)
+};
+WorkspaceLayout workspace_layout(const retro_desc_t* d);
+
+// ---- kernel launchers (one per stage; defined in the matching .cu) ------------------------------
+int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const int32_t* block_table,
+                              const int32_t* seq_lens, const int32_t* pos_begin, int max_touched, void* bounds,
+                              cudaStream_t s);
+int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
+                        const int32_t* seq_lens, const int32_t* budget_pages, int32_t* last_loaded,
+                        int32_t* sel_pages, int32_t* sel_prev, int32_t* sel_count, double* scores_out,
+                        void* workspace, cudaStream_t s);
+int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_win, const int32_t* q_pos,
+                         const void* k_pages, const void* v_pages, const int32_t* block_table,
+                         const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,
+                         const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s);
+int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
+                              const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                              int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
+int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
+                     const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s);
+int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
+                          int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s);
+
+#ifdef __CUDACC__
+// ---- device helpers ---------------------------------------------------------------------------
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+  static constexpr int kPer16B = 4;
+  __device__ static __forceinline__ float to_f32(float x) { return x; }
+  __device__ static __forceinline__ float from_f32(float x) { return x; }
+};
+template <> struct Elem<__nv_bfloat16> {
+  static constexpr int kPer16B = 8;
+  __device__ static __forceinline__ float to_f32(__nv_bfloat16 x) { return __bfloat162float(x); }
+  __device__ static __forceinline__ __nv_bfloat16 from_f32(float x) { return __float2bfloat16_rn(x); }
+};
+
+__device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+// mbarrier + 1-D bulk async copy (TMA unit, SASS UBLKCP): whole KV page tiles global -> shared.
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {
+  }
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// 128-bit read-only streaming load that does not allocate in L1 (digests are read once per step).
+__device__ __forceinline__ uint4 ldg_stream(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+#endif  // __CUDACC__
+
+}  // namespace retro

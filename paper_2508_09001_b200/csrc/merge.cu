@@ -1,0 +1,159 @@
+// S4  output-cache merge (Eq. 8-9 with alpha = e^lse) and the cache ring
+// (push / update / pop; Alg. 1 lines 7-8).
+//
+// One CTA per (sequence, cache slot): the slot's reader (the past row whose position maps to it) and its writer
+// (that row's merged value, or the current row when the slot is t mod w) are handled by the same CTA, so the
+// pop of position t-w and the push of position t never race.  One extra CTA per sequence writes the empty rows.
+// HBM-trivial: 2*w*h_q*(d+1) floats per sequence; 128-bit accesses.
+#include "common.cuh"
+
+namespace retro {
+
+template <typename T> struct OutVec;   // 4 consecutive outputs of type T from a float4
+template <> struct OutVec<float> {
+  __device__ static __forceinline__ void store(float* dst, float4 v) { *reinterpret_cast<float4*>(dst) = v; }
+};
+template <> struct OutVec<__nv_bfloat16> {
+  __device__ static __forceinline__ void store(__nv_bfloat16* dst, float4 v) {
+    __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), c = __floats2bfloat162_rn(v.z, v.w);
+    uint2 u;
+    u.x = *reinterpret_cast<uint32_t*>(&a);
+    u.y = *reinterpret_cast<uint32_t*>(&c);
+    *reinterpret_cast<uint2*>(dst) = u;
+  }
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restrict__ part_o,
+                                                          const float* __restrict__ part_lse,
+                                                          const int32_t* __restrict__ q_pos,
+                                                          const int32_t* __restrict__ seq_lens, float* cache_o,
+                                                          float* cache_lse, int32_t* cache_pos, T* __restrict__ out,
+                                                          float* __restrict__ out_lse, int h_q, int D, int w) {
+  const int b = blockIdx.y, x = blockIdx.x;
+  const int R = w + 1;
+  const int t = seq_lens[b] - 1;
+  const int vec_per_row = D / 4;
+  const int n_vec = h_q * vec_per_row;
+  __shared__ int s_past_row, s_cur_row, s_cached;
+
+  if (x == w) {   // empty rows -> zeros / -inf
+    for (int r = 0; r < R; ++r) {
+      const int p = q_pos[b * R + r];
+      if (p >= 0 && p <= t && p >= t - w) continue;
+      for (int i = threadIdx.x; i < n_vec; i += blockDim.x)
+        OutVec<T>::store(out + ((size_t)b * R + r) * h_q * D + (size_t)i * 4, make_float4(0.f, 0.f, 0.f, 0.f));
+      if (out_lse != nullptr)
+        for (int i = threadIdx.x; i < h_q; i += blockDim.x) out_lse[((size_t)b * R + r) * h_q + i] = -INFINITY;
+    }
+    if (w == 0) {   // plain Quest: out = part of the current row, no cache
+      for (int r = 0; r < R; ++r) {
+        if (q_pos[b * R + r] != t) continue;
+        for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
+          const size_t o = ((size_t)b * R + r) * h_q * D + (size_t)i * 4;
+          OutVec<T>::store(out + o, *reinterpret_cast<const float4*>(part_o + o));
+        }
+        if (out_lse != nullptr)
+          for (int i = threadIdx.x; i < h_q; i += blockDim.x)
+            out_lse[((size_t)b * R + r) * h_q + i] = part_lse[((size_t)b * R + r) * h_q + i];
+      }
+    }
+    return;
+  }
+
+  // slot x: the past position p in [t-w, t-1] with p mod w == x, and (if x == t mod w) the current row
+  const int slot = x;
+  if (threadIdx.x == 0) {
+    int past = -1, cur = -1;
+    for (int r = 0; r < R; ++r) {
+      const int p = q_pos[b * R + r];
+      if (p < 0 || p > t || p < t - w) continue;
+      if (p == t) { if (t % w == slot) cur = r; }
+      else if (p % w == slot) past = r;
+    }
+    s_past_row = past;
+    s_cur_row = cur;
+    s_cached = (past >= 0 && cache_pos[b * w + slot] == q_pos[b * R + past]) ? 1 : 0;
+  }
+  __syncthreads();
+  const int past = s_past_row, cur = s_cur_row;
+  const bool cached = s_cached != 0;
+  const int p_past = past >= 0 ? q_pos[b * R + past] : -1;
+  const bool evict = past >= 0 && p_past == t - w;   // popped after its last merge
+  float* c_o = cache_o + ((size_t)b * w + slot) * h_q * D;
+  float* c_l = cache_lse + ((size_t)b * w + slot) * h_q;
+
+  if (past >= 0) {
+    const float* po = part_o + ((size_t)b * R + past) * h_q * D;
+    const float* pl = part_lse + ((size_t)b * R + past) * h_q;
+    T* oo = out + ((size_t)b * R + past) * h_q * D;
+    for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
+      const int hh = i / vec_per_row;
+      const float lp = pl[hh];
+      const float lc = cached ? c_l[hh] : -INFINITY;
+      float4 vp = *reinterpret_cast<const float4*>(po + (size_t)i * 4);
+      float4 res;
+      if (lc == -INFINITY) res = vp;
+      else if (lp == -INFINITY) res = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4);
+      else {
+        const float4 vc = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4);
+        const float mx = fmaxf(lc, lp);
+        const float wc = __expf(lc - mx), wp = __expf(lp - mx);
+        const float inv = 1.f / (wc + wp);
+        res.x = (wc * vc.x + wp * vp.x) * inv; res.y = (wc * vc.y + wp * vp.y) * inv;
+        res.z = (wc * vc.z + wp * vp.z) * inv; res.w = (wc * vc.w + wp * vp.w) * inv;
+      }
+      OutVec<T>::store(oo + (size_t)i * 4, res);
+      if (!evict) *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = res;
+    }
+    __syncthreads();   // every thread has read c_l before it is rewritten
+    for (int hh = threadIdx.x; hh < h_q; hh += blockDim.x) {
+      const float lp = pl[hh];
+      const float lc = cached ? c_l[hh] : -INFINITY;
+      float lse;
+      if (lc == -INFINITY) lse = lp;
+      else if (lp == -INFINITY) lse = lc;
+      else {
+        const float mx = fmaxf(lc, lp);
+        lse = mx + __logf(__expf(lc - mx) + __expf(lp - mx));
+      }
+      if (out_lse != nullptr) out_lse[((size_t)b * R + past) * h_q + hh] = lse;
+      if (!evict) c_l[hh] = lse;
+    }
+    if (!evict && threadIdx.x == 0) cache_pos[b * w + slot] = p_past;
+  }
+  if (cur >= 0) {   // push O_org of the current query (after the popped row was read above)
+    __syncthreads();
+    const float* po = part_o + ((size_t)b * R + cur) * h_q * D;
+    const float* pl = part_lse + ((size_t)b * R + cur) * h_q;
+    T* oo = out + ((size_t)b * R + cur) * h_q * D;
+    for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
+      const float4 v = *reinterpret_cast<const float4*>(po + (size_t)i * 4);
+      OutVec<T>::store(oo + (size_t)i * 4, v);
+      *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = v;
+    }
+    for (int hh = threadIdx.x; hh < h_q; hh += blockDim.x) {
+      const float l = pl[hh];
+      if (out_lse != nullptr) out_lse[((size_t)b * R + cur) * h_q + hh] = l;
+      c_l[hh] = l;
+    }
+    if (threadIdx.x == 0) cache_pos[b * w + slot] = t;
+  }
+}
+
+int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
+                              const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                              int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s) {
+  dim3 grid(d->window + 1, d->batch);
+  if (d->dtype == RETRO_BF16)
+    merge_cache_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>(part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse,
+                                                          cache_pos, (__nv_bfloat16*)out, out_lse, d->num_q_heads,
+                                                          d->head_dim, d->window);
+  else
+    merge_cache_kernel<float><<<grid, 256, 0, s>>>(part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse, cache_pos,
+                                                   (float*)out, out_lse, d->num_q_heads, d->head_dim, d->window);
+  RETRO_LAUNCH_CHECK();
+  return RETRO_OK;
+}
+
+}  // namespace retro

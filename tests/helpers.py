@@ -26,7 +26,7 @@ def oracle_desc(cfg: wl.RetroConfig, **kw) -> orc.OracleDesc:
 
 def oracle_layer(inp: wl.LayerInputs, **kw) -> orc.OracleLayer:
     desc = oracle_desc(inp.cfg, **kw)
-    return orc.OracleLayer(desc, inp.k_pages.double().cpu().numpy(), inp.v_pages.double().cpu().numpy(),
+    return orc.OracleLayer(desc, inp.k_pages.float().cpu().numpy(), inp.v_pages.float().cpu().numpy(),
                            inp.block_table.cpu().numpy())
 
 

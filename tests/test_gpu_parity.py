@@ -1,0 +1,157 @@
+"""-m gpu: CUDA path vs the fp64 oracle, element by element, through the C ABI (teacher-forced lock-step).
+
+Shapes are the five BASELINE.json configs: C1 exactly; C2..C5 both shrunk to sizes the oracle finishes in
+seconds (several tiles, ragged tails, page roll-over) and at FULL context for a few sampled steps."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2508_09001_b200 import binding as rb
+from paper_2508_09001_b200 import workload as wl
+from tests import gpu_harness as GH
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def test_library_is_loaded_from_tree():
+    H.require_cuda()
+    assert rb.library_path().endswith("paper_2508_09001_b200/lib/libretro.so")
+    assert torch.cuda.get_device_capability()[0] >= 10, "needs sm_100"
+
+
+def test_c1_tiny_fp32_full_lockstep():
+    inp = wl.make_layer_inputs(wl.c1())
+    e = GH.lockstep(inp, 16)
+    assert e["out"] < 1e-4 and e["part_o"] < 1e-4
+    print("c1 errs", e)
+
+
+def test_c1_whole_step_entry_point():
+    """retro_decode_step (S1..S4 back to back) gives the same trajectory without teacher forcing."""
+    inp = wl.make_layer_inputs(wl.c1())
+    GH.lockstep(inp, 16, use_decode_step=True)
+
+
+@pytest.mark.parametrize("prompt", [2003, 2048])      # ragged tail / exactly page aligned
+def test_c2_shape_shrunk(prompt):
+    cfg = wl.shrink(wl.c2(), (prompt,), 40)
+    inp = wl.make_layer_inputs(cfg)
+    print("c2s errs", GH.lockstep(inp, 40))
+
+
+def test_c3_shape_shrunk_ragged_batch():
+    cfg = wl.shrink(wl.c3(), tuple(700 - 61 * b for b in range(4)), 36, batch=4, budget_tokens=256)
+    inp = wl.make_layer_inputs(cfg)
+    print("c3s errs", GH.lockstep(inp, 36))
+
+
+def test_c4_shape_shrunk_gqa7():
+    cfg = wl.shrink(wl.c4(), (3001, 2990), 20, batch=2, budget_tokens=512)
+    inp = wl.make_layer_inputs(cfg)
+    print("c4s errs", GH.lockstep(inp, 20))
+
+
+@pytest.mark.parametrize("w,budget", [(0, 512), (1, 1024), (32, 512)])
+def test_c5_shape_shrunk_sweep_points(w, budget):
+    cfg = wl.shrink(wl.c5(w, budget), (1500, 1490), w + 6, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    print("c5s errs", w, budget, GH.lockstep(inp, w + 6))
+
+
+def test_edge_budget_covers_whole_cache_is_dense():
+    cfg = wl.shrink(wl.c2(), (300,), 12, budget_tokens=16 * 64, window=4)
+    inp = wl.make_layer_inputs(cfg)
+    GH.lockstep(inp, 12)
+
+
+def test_edge_single_page_and_budget_one():
+    cfg = wl.shrink(wl.c2(), (5,), 14, budget_tokens=16, window=3)     # grows from 1 page to 2; k = 1
+    inp = wl.make_layer_inputs(cfg)
+    GH.lockstep(inp, 14)
+
+
+def test_edge_pure_topk_and_group_max():
+    cfg = wl.shrink(wl.c2(), (777,), 12, budget_tokens=128, window=4)
+    inp = wl.make_layer_inputs(cfg)
+    GH.lockstep(inp, 12, desc_kw=dict(force_last_page=0), oracle_kw=dict(force_last_page=False))
+    GH.lockstep(inp, 12, desc_kw=dict(group_reduce=rb.RETRO_GROUP_MAX), oracle_kw=dict(group_reduce="max"))
+
+
+def test_edge_exact_score_ties_resolve_to_lower_index():
+    """All keys identical => every page has the same score: top-k must be the k-1 lowest indices + newest page."""
+    cfg = wl.shrink(wl.c1(), (200,), 3, budget_tokens=64, window=2)
+    inp = wl.make_layer_inputs(cfg)
+    inp.k_pages[:] = inp.k_pages[0, 0, 0]
+    _, buf = GH.make_device_layer(inp)
+    # direct call, no oracle needed for the expectation
+    buf.seq_lens.fill_(201)
+    buf.rebuild_bounds()
+    buf.q_cur.copy_(inp.q_all[0])
+    desc = buf.desc
+    rb.retro_select_pages(desc, buf.q_cur, buf.bounds, buf.seq_lens, buf.budget_pages, buf.last_loaded,
+                          buf.sel_pages, buf.sel_prev, buf.sel_count, None, buf.workspace)
+    torch.cuda.synchronize()
+    assert buf.sel_pages[0, 0].tolist() == [0, 1, 2, 12]
+    GH.lockstep(inp, 3)
+
+
+def test_c2_full_context_sampled_steps():
+    """FULL C2 context (32768-token prompt), the launch configuration bench.py times; first steps + ramp-up."""
+    cfg = wl.c2(n_steps=12)
+    inp = wl.make_layer_inputs(cfg, device="cuda")
+    inp = _to_cpu(inp)
+    print("c2 full errs", GH.lockstep(inp, 12))
+
+
+def test_c4_full_context_sampled_steps():
+    cfg = wl.c4(n_steps=3)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c4 full errs", GH.lockstep(inp, 3))
+
+
+def test_c3_full_batch_sampled_steps():
+    cfg = wl.c3(n_steps=3)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c3 full errs", GH.lockstep(inp, 3))
+
+
+def test_c5_full_point_w8_budget4096():
+    cfg = wl.c5(8, 4096, n_steps=2)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c5 full errs", GH.lockstep(inp, 2))
+
+
+def test_append_kv_and_window_advance_match_pregenerated_pool():
+    """retro_append_kv / retro_window_advance (harness + host path plumbing) move bytes exactly."""
+    cfg = wl.shrink(wl.c2(), (100,), 6, window=3, budget_tokens=64)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    ref_k = buf.k_pages.clone()
+    ref_v = buf.v_pages.clone()
+    k_seq, v_seq = H.seq_tokens(inp, 0, 106)
+    # wipe the decode-phase tokens, then re-append them one by one
+    for pos in range(100, 106):
+        phys = int(inp.block_table[0, pos // 16])
+        buf.k_pages[phys, :, pos % 16] = 0
+        buf.v_pages[phys, :, pos % 16] = 0
+    buf.seq_lens.fill_(100)
+    for s in range(6):
+        pos = 100 + s
+        rb.retro_window_advance(desc, inp.q_all[s].cuda().contiguous(), None, 1, buf.seq_lens, buf.q_win, buf.q_pos,
+                                buf.q_cur)
+        kn = torch.from_numpy(k_seq[pos]).to(torch.bfloat16).cuda().contiguous()[None]
+        vn = torch.from_numpy(v_seq[pos]).to(torch.bfloat16).cuda().contiguous()[None]
+        rb.retro_append_kv(desc, kn, vn, buf.block_table, buf.seq_lens, buf.k_pages, buf.v_pages)
+        torch.cuda.synchronize()
+        assert int(buf.seq_lens[0]) == pos + 1
+        q_win, q_pos = wl.make_q_window(inp, s)
+        assert torch.equal(buf.q_pos.cpu(), q_pos)
+        assert torch.equal(buf.q_win.cpu()[q_pos >= 0], q_win[q_pos >= 0])
+        assert torch.equal(buf.q_cur.cpu(), inp.q_all[s])
+    assert torch.equal(buf.k_pages, ref_k) and torch.equal(buf.v_pages, ref_v)
+
+
+def _to_cpu(inp):
+    return wl.LayerInputs(inp.cfg, inp.k_pages.cpu(), inp.v_pages.cpu(), inp.block_table.cpu(), inp.q_all.cpu(),
+                          inp.prompt_lens.cpu(), inp.outlier_channels.cpu())
