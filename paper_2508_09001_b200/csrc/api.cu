@@ -31,12 +31,17 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   WorkspaceLayout wl;
   const int units = d->batch * d->num_kv_heads;
   wl.rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
-  // split-KV so that units * nsplit covers the 148 SMs about twice; at least 2 pages per split
-  int nsplit = ceil_div(2 * 148, units);
-  const int max_split = d->max_sel_pages >= 2 ? d->max_sel_pages / 2 : 1;
+  // split-KV so that units * nsplit covers the 148 SMs about twice; at least 2 pages per split.  The tensor-core
+  // path (bf16, rows <= 128) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per split, so
+  // its splits are whole blocks and at most one wave of CTAs.
+  const bool umma = d->dtype == RETRO_BF16 && wl.rows <= 128;
+  int nsplit = ceil_div((umma ? 1 : 2) * 148, units);
+  const int min_pages = umma ? 8 : 2;
+  const int max_split = d->max_sel_pages >= min_pages ? d->max_sel_pages / min_pages : 1;
   if (nsplit > max_split) nsplit = max_split;
   if (nsplit < 1) nsplit = 1;
   wl.pages_per_split = ceil_div(d->max_sel_pages, nsplit);
+  if (umma) wl.pages_per_split = ceil_div(wl.pages_per_split, 8) * 8;
   wl.nsplit = ceil_div(d->max_sel_pages, wl.pages_per_split);
   size_t off = 0;
   wl.scores_off = off;

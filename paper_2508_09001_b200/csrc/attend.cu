@@ -10,14 +10,14 @@
 // combines them (LSE merge, Eq. 8 applied to splits) into part_o / part_lse.
 //
 // This is the scalar-ALU path: exact fp32 products (C1's 1e-4 tolerance rules out TF32) and small row blocks.
-#include "common.cuh"
+#include <cstdlib>
+
+#include "attend_common.cuh"
 
 namespace retro {
 
 constexpr int kAttWarps = 8;
 constexpr int kStages = 4;
-constexpr float kLog2e = 1.4426950408889634f;
-constexpr float kLn2 = 0.6931471805599453f;
 
 template <typename T, int D> struct LaneSlice;   // a lane's D/32 channels of one row
 template <> struct LaneSlice<__nv_bfloat16, 128> {
@@ -31,15 +31,6 @@ template <> struct LaneSlice<float, 64> {
   static constexpr int kCh = 2;
   using Raw = float2;
   __device__ static __forceinline__ void unpack(Raw r, float* f) { f[0] = r.x; f[1] = r.y; }
-};
-
-struct AttendParams {
-  const void* q_win; const int32_t* q_pos; const void* k_pages; const void* v_pages;
-  const int32_t* block_table; const int32_t* seq_lens; const int32_t* sel_pages; const int32_t* sel_prev;
-  const int32_t* sel_count; float* part_o; float* part_lse; float* split_o; float* split_lse;
-  unsigned int* counters;
-  int B, h_q, h_k, max_pages, k_max, window, nsplit, pages_per_split;
-  float scale_log2;   // sm_scale * log2(e)
 };
 
 // Reduce 16 per-lane partial sums across the warp so that lane L ends with the total of token (L >> 1).
@@ -238,43 +229,8 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
   }
   if (p.nsplit == 1) return;
 
-  // last CTA of this (b, head) unit combines the splits
   __shared__ unsigned int s_ticket;
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_ticket = atomicAdd(&p.counters[unit], 1u);
-  __syncthreads();
-  if (s_ticket != (unsigned)(p.nsplit - 1)) return;
-  if (tid == 0) p.counters[unit] = 0;   // leave the workspace consistent for the next call
-  __threadfence();
-  for (int rho = warp; rho < rows; rho += kAttWarps) {
-    const float* lse_s = p.split_lse + unit * p.nsplit * rows + rho;
-    float mx = -INFINITY;
-    for (int s = lane; s < p.nsplit; s += 32) mx = fmaxf(mx, __ldcg(lse_s + (size_t)s * rows));
-    mx = warp_max(mx);
-    float o[kCh];
-#pragma unroll
-    for (int c = 0; c < kCh; ++c) o[c] = 0.f;
-    float wsum = 0.f;
-    if (mx > -INFINITY) {
-      for (int s = 0; s < p.nsplit; ++s) {
-        const float ls = __ldcg(lse_s + (size_t)s * rows);
-        if (ls == -INFINITY) continue;
-        const float wgt = exp2f(ls - mx);
-        wsum += wgt;
-        const float* src = p.split_o + ((unit * p.nsplit + s) * rows + rho) * D + lane * kCh;
-#pragma unroll
-        for (int c = 0; c < kCh; ++c) o[c] = fmaf(wgt, __ldcg(src + c), o[c]);
-      }
-    }
-    const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
-    const int r = rho / G, g = rho % G;
-    float* dst = p.part_o + (((size_t)b * R + r) * p.h_q + h * G + g) * D + lane * kCh;
-#pragma unroll
-    for (int c = 0; c < kCh; ++c) dst[c] = o[c] * inv;
-    if (lane == 0)
-      p.part_lse[((size_t)b * R + r) * p.h_q + h * G + g] = wsum > 0.f ? (mx + log2f(wsum)) * kLn2 : -INFINITY;
-  }
+  combine_splits_last_cta<D>(p, unit, b, h, rows, G, R, &s_ticket);
 }
 
 template <typename T, int D, int RPW>
@@ -322,7 +278,16 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
   prm.k_max = d->max_sel_pages; prm.window = d->window; prm.nsplit = wl.nsplit;
   prm.pages_per_split = wl.pages_per_split;
   prm.scale_log2 = d->sm_scale * kLog2e;
-  if (d->dtype == RETRO_BF16) return dispatch_rpw<__nv_bfloat16, 128>(d, prm, s);
+  if (d->dtype == RETRO_BF16) {
+    // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu).  The scalar
+    // path stays reachable for debugging (RETRO_ATTEND_PATH=simt) and for row blocks above one 128-row tile.
+    static const bool force_simt = [] {
+      const char* e = std::getenv("RETRO_ATTEND_PATH");
+      return e != nullptr && e[0] == 's';
+    }();
+    if (!force_simt && wl.rows <= 128) return launch_attend_umma(d, prm, s);
+    return dispatch_rpw<__nv_bfloat16, 128>(d, prm, s);
+  }
   return dispatch_rpw<float, 64>(d, prm, s);
 }
 
