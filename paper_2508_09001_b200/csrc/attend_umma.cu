@@ -12,8 +12,8 @@
 //               signalled to the other warps with tcgen05.commit on mbarriers.  Owns the TMEM allocation.
 //   warps 2..5  softmax: thread <-> TMEM lane <-> query row.  Reads its S row with tcgen05.ld, applies the
 //               retrospective mask (page j active for row at position p iff sel_prev_j < p; token l iff l <= p),
-//               keeps (m, l) in registers, writes P (bf16) into shared memory in the K-major 128B-swizzled
-//               operand layout, rescales O in TMEM only when the running max moved by more than 2^8.
+//               keeps (m, l) in registers, overwrites S in place with P (bf16 hi + lo, the TMEM A operand
+//               of the PV MMA), rescales O in TMEM only when the running max moved by more than 2^8.
 // S is double-buffered in TMEM so QK^T of block i+1 overlaps the softmax of block i.
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
@@ -84,10 +84,28 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
+// P is handed to the tensor core as a bf16 hi + bf16 lo pair (two MMAs per K step, 16 mantissa bits): a single
+// bf16 P (2^-9) leaves |err| ~ 2^-9 * |v| on the x8 outlier channels of V, outside the 2e-2 tolerance.
+__device__ __forceinline__ void split_bf16x2(float e0, float e1, uint32_t& hi, uint32_t& lo) {
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(hi) : "f"(e1), "f"(e0));
+  const float r0 = e0 - __uint_as_float(hi << 16), r1 = e1 - __uint_as_float(hi & 0xffff0000u);
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(lo) : "f"(r1), "f"(r0));
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+// A operand from TMEM (lanes = rows, one 32-bit column = two consecutive K elements), B from shared memory.
+__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
+                                             uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
 }
 
 // Shared-memory matrix descriptors (cute::UMMA::SmemDescriptor bit layout), 128B swizzle, version 1.
@@ -109,8 +127,7 @@ __device__ __forceinline__ uint32_t idesc_bf16(int n, bool b_mn_major) {
 
 struct UmmaSmem {   // offsets into dynamic shared memory (base aligned to 1024 B)
   static constexpr int q = 0;
-  static constexpr int p = q + kQBytes;
-  static constexpr int k = p + kQBytes;
+  static constexpr int k = q + kQBytes;
   static constexpr int v = k + kKvStages * kStageBytes;
   static constexpr int bars = v + kKvStages * kStageBytes;   // 16 mbarriers
   static constexpr int tmem_ptr = bars + 16 * 8;
@@ -166,7 +183,6 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
         }
         const int half = c >> 3, ch = c & 7;
         *reinterpret_cast<uint4*>(smem + UmmaSmem::q + half * 16384 + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
-        *reinterpret_cast<uint4*>(smem + UmmaSmem::p + half * 16384 + rho * 128 + (ch << 4)) = make_uint4(0, 0, 0, 0);
       }
     }
     if (tid == 0) {
@@ -214,7 +230,7 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
     } else if (warp == 1) {
       // ===== MMA issuer =====
       if (lane == 0) {
-        const uint32_t q_addr = smem_u32(smem + UmmaSmem::q), p_addr = smem_u32(smem + UmmaSmem::p);
+        const uint32_t q_addr = smem_u32(smem + UmmaSmem::q);
         auto issue_s = [&](int blk) {
           const int s = blk % kKvStages, n = blk / kKvStages;
           const int np = min(kPB, n_my - blk * kPB);
@@ -241,10 +257,11 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
           tc_fence_after();
           const uint32_t v_addr = smem_u32(smem + UmmaSmem::v + s * kStageBytes);
           const uint32_t idesc = idesc_bf16(128, true);
-          for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
-            const uint32_t a_off = (ks >> 2) * 16384 + (ks & 3) * 32;
-            umma_bf16(tmem_base + kColO, desc_kmajor_sw128(p_addr + a_off),
-                      desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride), idesc, (blk > 0 || ks > 0));
+          const uint32_t p_tmem = tmem_base + kColS + (blk & 1) * 128;   // P overwrote S in place: [hi 64 | lo 64]
+          for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step = 8 TMEM columns of A
+            const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
+            umma_bf16_ts(tmem_base + kColO, p_tmem + 8 * ks, vdesc, idesc, (blk > 0 || ks > 0));
+            umma_bf16_ts(tmem_base + kColO, p_tmem + 64 + 8 * ks, vdesc, idesc, 1u);
           }
           tc_commit(&v_empty[s]);
           tc_commit(o_full);
@@ -262,7 +279,6 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
       }
       const bool real = pos >= 0;
       float m_ref = -INFINITY, l_run = 0.f;               // running max (log2 units) used as exponent reference
-      unsigned char* p_row = smem + UmmaSmem::p + rho * 128;
       for (int blk = 0; blk < nblk; ++blk) {
         const int np = min(kPB, n_my - blk * kPB);
         // valid-token count of each page of the block for this row (0 = page masked for this query)
@@ -302,11 +318,9 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
         // the stale reference keeps P <= 2^8 and the final 1/l normalisation absorbs it.  While m_ref = -inf the
         // row's P has been all zeros, so its O row is exactly 0 and needs no rescale.
         const bool need = real && m_ref > -INFINITY && mx > m_ref + kRescaleThreshold;
-        if (blk > 0) {
-          mbar_wait(o_full, (blk - 1) & 1);                // PV(blk-1) retired: P buffer and O are ours
-          tc_fence_after();
-        }
         if (__any_sync(0xffffffffu, need)) {
+          mbar_wait(o_full, (blk - 1) & 1);                // PV(blk-1) retired: O is ours (need implies blk > 0)
+          tc_fence_after();
           float alpha = 1.f;
           if (need) {
             alpha = ex2_approx(m_ref - mx);
@@ -325,41 +339,38 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
           tmem_wait_st();
         }
         if (real && m_ref == -INFINITY && mx > -INFINITY) m_ref = mx;   // first visible keys of this row
-        // pass 2: P = 2^(s*scale - m_ref) -> bf16 -> shared memory (swizzled K-major operand), row sum
+        // pass 2: P = 2^(s*scale - m_ref) as bf16 hi + lo, written over S in place: hi of chunk c4 lands in
+        // columns [16 c4, 16 c4 + 16) (already read), lo is held back until every S chunk has been read.
         const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
         float lsum = 0.f;
+        uint32_t plo[4][16];
 #pragma unroll
         for (int c4 = 0; c4 < 4; ++c4) {
           if (c4 * 2 < np) {
             uint32_t sv[32];
             tmem_ld32(s_addr + c4 * 32, sv);
             tmem_wait_ld();
-            if (rho < rows) {
-              const int nv0 = nvalid(c4 * 2), nv1 = nvalid(c4 * 2 + 1);
-              uint32_t pk[16];
+            const int nv0 = nvalid(c4 * 2), nv1 = nvalid(c4 * 2 + 1);   // 0 for padding / empty rows
+            uint32_t phi[16];
 #pragma unroll
-              for (int c = 0; c < 32; c += 2) {
-                const int nv = c < 16 ? nv0 : nv1;
-                const int tk = c & 15;
-                float e0 = 0.f, e1 = 0.f;
-                if (tk < nv) e0 = ex2_approx(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use));
-                if (tk + 1 < nv) e1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use));
-                lsum += e0 + e1;
-                pk[c >> 1] = pack_bf16x2(e0, e1);
-              }
-              // 32 keys = 4 chunks of 16 B; key index kc = c4*32 + 8*q -> half = c4 >> 1, chunk = (c4 & 1)*4 + q
-#pragma unroll
-              for (int q4 = 0; q4 < 4; ++q4) {
-                const int ch = (c4 & 1) * 4 + q4;
-                *reinterpret_cast<uint4*>(p_row + (c4 >> 1) * 16384 + ((ch ^ (rho & 7)) << 4)) =
-                    make_uint4(pk[q4 * 4], pk[q4 * 4 + 1], pk[q4 * 4 + 2], pk[q4 * 4 + 3]);
-              }
+            for (int c = 0; c < 32; c += 2) {
+              const int nv = c < 16 ? nv0 : nv1;
+              const int tk = c & 15;
+              float e0 = 0.f, e1 = 0.f;
+              if (tk < nv) e0 = ex2_approx(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use));
+              if (tk + 1 < nv) e1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use));
+              lsum += e0 + e1;
+              split_bf16x2(e0, e1, phi[c >> 1], plo[c4][c >> 1]);
             }
+            tmem_st16(s_addr + c4 * 16, phi);
           }
         }
+#pragma unroll
+        for (int c4 = 0; c4 < 4; ++c4)
+          if (c4 * 2 < np) tmem_st16(s_addr + 64 + c4 * 16, plo[c4]);
+        tmem_wait_st();
         l_run += lsum;
         tc_fence_before();
-        fence_proxy_async();                               // P visible to the tensor core's async proxy
         mbar_arrive(p_ready);
       }
       // ---- epilogue: O / l and the base-2 lse of this split ----
