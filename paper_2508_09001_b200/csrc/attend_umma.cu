@@ -145,8 +145,9 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
   uint64_t* k_empty = bars + 4;     // [2]
   uint64_t* v_empty = bars + 6;     // [2]
   uint64_t* s_full = bars + 8;      // [2]
-  uint64_t* p_ready = bars + 10;
-  uint64_t* o_full = bars + 11;
+  uint64_t* p_ready = bars + 10;    // [2] one per S buffer: a fast warp may run one block ahead of a slow one
+  uint64_t* o_full = bars + 12;
+  uint64_t* o_done = bars + 13;     // last PV retired (a parity wait on o_full could alias two phases back)
   uint32_t* tmem_ptr_s = reinterpret_cast<uint32_t*>(smem + UmmaSmem::tmem_ptr);
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + UmmaSmem::list);
   __shared__ unsigned int s_ticket;
@@ -188,8 +189,9 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
     if (tid == 0) {
       for (int i = 0; i < 8; ++i) mbar_init(&bars[i], 1);
       mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
-      mbar_init(p_ready, 128);
+      mbar_init(&p_ready[0], 128); mbar_init(&p_ready[1], 128);
       mbar_init(o_full, 1);
+      mbar_init(o_done, 1);
       fence_mbar_init();
     }
     if (warp == 1) {
@@ -252,7 +254,7 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
           if (blk + 1 < nblk) issue_s(blk + 1);
           const int s = blk % kKvStages, n = blk / kKvStages;
           const int np = min(kPB, n_my - blk * kPB);
-          mbar_wait(p_ready, blk & 1);
+          mbar_wait(&p_ready[blk & 1], (blk >> 1) & 1);
           mbar_wait(&v_full[s], n & 1);
           tc_fence_after();
           const uint32_t v_addr = smem_u32(smem + UmmaSmem::v + s * kStageBytes);
@@ -265,6 +267,7 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
           }
           tc_commit(&v_empty[s]);
           tc_commit(o_full);
+          if (blk == nblk - 1) tc_commit(o_done);
         }
       }
     } else {
@@ -371,10 +374,10 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
         tmem_wait_st();
         l_run += lsum;
         tc_fence_before();
-        mbar_arrive(p_ready);
+        mbar_arrive(&p_ready[blk & 1]);
       }
       // ---- epilogue: O / l and the base-2 lse of this split ----
-      mbar_wait(o_full, (nblk - 1) & 1);
+      mbar_wait(o_done, 0);
       tc_fence_after();
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
       const float lse2 = l_run > 0.f ? m_ref + log2f(l_run) : -INFINITY;
