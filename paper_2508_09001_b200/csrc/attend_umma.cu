@@ -1,37 +1,43 @@
 // S3 on the 5th-generation tensor cores (bf16, d = 128, P = 16): the GQA group x (w+1) query block against
-// the selected pages is a dense [rows x 128] x [128 x keys] contraction followed by [rows x keys] x [keys x 128]
-// (Eq. 2 / 6 / 7; arithmetic intensity ~ rows flop/B), far above what
-// the fp32 ALUs sustain at HBM rate once rows > ~8.
+// the selected pages is a dense contraction (Eq. 2 / 6 / 7; arithmetic intensity ~ rows
+// flop per KV byte), far above what the fp32 ALUs sustain at HBM rate once rows > ~8.
 //
-// One CTA per (split, KV head, sequence), 192 threads, warp-specialised:
-//   warp 0      TMA producer: each selected (page, head) K tile and V tile arrives as two 64-column boxes with
-//               the 128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier), 8 pages = 128 keys per KV block,
-//               double-buffered (2 x 64 KB in flight per SM).
-//   warp 1      MMA issuer (one elected thread): S = Q K^T  -> TMEM (M = 128 rows, N = 16 * pages, K = 128) and
-//               O += P V -> TMEM (M = 128, N = 128, K = 16 * pages) with tcgen05.mma.kind::f16; completion is
-//               signalled to the other warps with tcgen05.commit on mbarriers.  Owns the TMEM allocation.
-//   warps 2..5  softmax: thread <-> TMEM lane <-> query row.  Reads its S row with tcgen05.ld, applies the
-//               retrospective mask (page j active for row at position p iff sel_prev_j < p; token l iff l <= p),
-//               keeps (m, l) in registers, overwrites S in place with P (bf16 hi + lo, the TMEM A operand
-//               of the PV MMA), rescales O in TMEM only when the running max moved by more than 2^8.
-// S is double-buffered in TMEM so QK^T of block i+1 overlaps the softmax of block i.
+// KEYS sit on the 128 TMEM lanes, query rows on the N dimension (N = rows padded to 16), so no tensor-core
+// or softmax work is spent on row padding and every softmax thread owns one key:
+//   S^T = K Q^T        A = K block [128 keys x 128 ch] (K-major, TMA SW128), B = Q [N x 128]   -> TMEM S  [key][row]
+//   O^T += V^T P^T     A = V block (MN-major),                               B = P [128 keys x N] -> TMEM O  [ch][row]
+//   L   += 1  P^T      A = ones,                                             B = P               -> TMEM L  [ * ][row]
+// Row sums (L) and the PV product both come from the tensor core; the softmax threads do element-wise work only:
+// P = 2^(s*scale - m_ref[row]) with the retrospective mask (page j is visible to the row at position p iff
+// sel_prev_j < p; token l iff l <= p), written to shared memory as bf16 hi + bf16 lo (MN-major SW128 B operand).
+// m_ref is a per-row reference kept in shared memory; it is raised (and O, L rescaled) only when some logit
+// exceeds it by more than 2^8, found by a cheap per-thread check, so the common block needs no reduction.
+//
+// One CTA per (split, KV head, sequence), 320 threads, warp-specialised:
+//   warp 0      TMA producer: every selected (page, head) K / V tile arrives as two 64-channel boxes with the
+//               128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier) into a ring of 32 KB slots
+//               (8 pages = 128 keys of K, then the same 128 keys of V, ...).
+//   warp 1      MMA issuer (one elected thread), owns the TMEM allocation; tcgen05.commit signals mbarriers.
+//   warps 2..9  softmax: lane quadrant = warp % 4 (32 keys), column half = (warp - 2) / 4.
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
+
+#include <cstdlib>
 
 #include "attend_common.cuh"
 
 namespace retro {
 
-constexpr int kUmmaThreads = 192;
-constexpr int kPB = 8;                    // pages per KV block
-constexpr int kKvStages = 2;
-constexpr int kTileHalfBytes = 16 * 128;  // one (page, head, 64-column half) box: 16 rows x 128 B
-constexpr int kHalfStride = kPB * kTileHalfBytes;          // 16 KB: [half][page][16][128 B]
-constexpr int kStageBytes = 2 * kHalfStride;               // 32 KB of K (or V) per stage
-constexpr int kQBytes = 2 * 128 * 128;                     // [half][128 rows][128 B] = 32 KB
+constexpr int kUmmaThreads = 320;
+constexpr int kSoftmaxThreads = 256;
+constexpr int kPB = 8;                        // pages per KV block (128 keys)
+constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel half) box: 16 rows x 128 B
+constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][128 B]
+constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
+constexpr int kOnesBytes = 4096;
 constexpr int kTmemCols = 512;
-constexpr int kColS = 0, kColO = 256;                      // S0: 0..127, S1: 128..255, O: 256..383
-constexpr float kRescaleThreshold = 8.f;                   // log2 units
+constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
+constexpr float kRescaleThreshold = 8.f;      // log2 units
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
@@ -125,57 +131,143 @@ __device__ __forceinline__ uint32_t idesc_bf16(int n, bool b_mn_major) {
          ((uint32_t)(128 >> 4) << 24);
 }
 
-struct UmmaSmem {   // offsets into dynamic shared memory (base aligned to 1024 B)
-  static constexpr int q = 0;
-  static constexpr int k = q + kQBytes;
-  static constexpr int v = k + kKvStages * kStageBytes;
-  static constexpr int bars = v + kKvStages * kStageBytes;   // 16 mbarriers
-  static constexpr int tmem_ptr = bars + 16 * 8;
-  static constexpr int list = tmem_ptr + 16;                  // int32 [3][pages_per_split]
+__device__ __forceinline__ uint32_t idesc_bf16_ab(int n, bool a_mn_major, bool b_mn_major) {
+  return idesc_bf16(n, b_mn_major) | ((a_mn_major ? 1u : 0u) << 15);
+}
+// K-major operand without swizzle: 8 x 16 B core matrices, LBO between the two K halves of a 16-deep step,
+// SBO between 8-row groups.  Used for the all-ones A operand of the row-sum MMA (its content is layout-free).
+__device__ __forceinline__ uint64_t desc_kmajor_none(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
+         ((uint64_t)(sbo_bytes >> 4) << 32) | ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
+}
+__device__ __forceinline__ void softmax_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+// order-preserving float <-> int image (signed compare), so a column max is one REDUX + one shared atomicMax
+__device__ __forceinline__ int f2o(float f) {
+  const int i = __float_as_int(f);
+  return i >= 0 ? i : i ^ 0x7fffffff;
+}
+__device__ __forceinline__ float o2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
+constexpr int kOrdNegInf = (int)0x807fffff;   // f2o(-inf)
+
+// Dynamic shared memory map (base aligned to 1024 B).  NT = padded rows, NS = ring slots, NP = P buffers.
+struct UmmaLayout {
+  int q, ones, p, ring, bars, meta, list, total;
+  int p_buf_bytes, p_hl_bytes;
+};
+__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
+  UmmaLayout L;
+  const int natom = (NT + 63) / 64;
+  L.q = 0;                                   // [half][NT rows][128 B]
+  L.ones = L.q + 2 * NT * 128;
+  L.p = L.ones + kOnesBytes;                 // [buf][hi|lo][atom][128 keys][128 B]
+  L.p_hl_bytes = natom * 16384;
+  L.p_buf_bytes = 2 * L.p_hl_bytes;
+  L.ring = L.p + NP * L.p_buf_bytes;
+  L.bars = L.ring + NS * kSlotBytes;         // up to 32 mbarriers
+  L.meta = L.bars + 32 * 8;                  // tmem ptr, flags, per-column arrays
+  L.list = L.meta + 64 + 5 * kMaxNT * 4;
+  L.total = L.list + 3 * pages_per_split * 4;
+  return L;
+}
+
+#ifdef RETRO_STAMPS
+__device__ unsigned long long g_stamps[32];
+__device__ __forceinline__ void stamp(int i) {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  g_stamps[i] = t;
+}
+#define STAMP(cond, i) do { if (cond) stamp(i); } while (0)
+#else
+#define STAMP(cond, i) do { } while (0)
+#endif
+
+struct UmmaCfg {
+  int NS;    // ring slots (32 KB each)
+  int NP;    // P buffers (1 or 2)
+  int NSB;   // S buffers in TMEM (1 or 2)
 };
 
+// NCH = NT / 16 = number of 8-column chunks each softmax thread owns (its half of the padded rows).
+template <int NCH>
 __global__ void __launch_bounds__(kUmmaThreads, 1)
-attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tmap_k,
+attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constant__ CUtensorMap tmap_k,
                    const __grid_constant__ CUtensorMap tmap_v) {
+  constexpr int NT = 16 * NCH;
+  constexpr int NHALF = 8 * NCH;
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + UmmaSmem::bars);
-  uint64_t* k_full = bars;          // [2]
-  uint64_t* v_full = bars + 2;      // [2]
-  uint64_t* k_empty = bars + 4;     // [2]
-  uint64_t* v_empty = bars + 6;     // [2]
-  uint64_t* s_full = bars + 8;      // [2]
-  uint64_t* p_ready = bars + 10;    // [2] one per S buffer: a fast warp may run one block ahead of a slow one
-  uint64_t* o_full = bars + 12;
-  uint64_t* o_done = bars + 13;     // last PV retired (a parity wait on o_full could alias two phases back)
-  uint32_t* tmem_ptr_s = reinterpret_cast<uint32_t*>(smem + UmmaSmem::tmem_ptr);
-  int32_t* s_list = reinterpret_cast<int32_t*>(smem + UmmaSmem::list);
+  const int pps = p.pages_per_split;
+  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, pps);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + lay.bars);
+  uint64_t* ring_full = bars;            // [NS <= 6]
+  uint64_t* ring_empty = bars + 6;       // [NS <= 6]
+  uint64_t* s_full = bars + 12;          // [2]
+  uint64_t* p_ready = bars + 14;         // [2]
+  uint64_t* o_full = bars + 16;          // [2] PV + L of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
+                                         // softmax warps run up to two blocks ahead: one barrier would alias)
+  uint32_t* tmem_ptr_s = reinterpret_cast<uint32_t*>(smem + lay.meta);
+  int* s_flag = reinterpret_cast<int*>(smem + lay.meta + 16);          // [3]
+  int* s_colpos = reinterpret_cast<int*>(smem + lay.meta + 64);        // [kMaxNT] position of the row, -1 = none
+  float* s_mref = reinterpret_cast<float*>(s_colpos + kMaxNT);         // running reference (log2 units)
+  int* s_colmax = reinterpret_cast<int*>(s_mref + kMaxNT);             // ordered-int block max (slow path)
+  float* s_alpha = reinterpret_cast<float*>(s_colmax + kMaxNT);
+  int* s_coloff = reinterpret_cast<int*>(s_alpha + kMaxNT);            // output offset (floats) of the row
+  int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
   __shared__ unsigned int s_ticket;
 
   const int split = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
+  STAMP(cta0 && tid == 0, 0);
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
   const int L = p.seq_lens[b];
   const int t = L - 1;
   const size_t unit = (size_t)b * p.h_k + h;
   const int count = p.sel_count[unit];
-  const int beg = min(split * p.pages_per_split, count);
-  const int end = min(beg + p.pages_per_split, count);
+  const int beg = min(split * pps, count);
+  const int end = min(beg + pps, count);
   const int n_my = end - beg;
   const int nblk = (n_my + kPB - 1) / kPB;
-  const int pps = p.pages_per_split;
+  const int colS = 0, colO = cfg.NSB * NT, colL = colO + NT;
 
   if (nblk > 0) {
-    // ---- prologue: page list, Q (swizzled K-major operand), zeroed P, barriers, TMEM ----------------------
+    // ---- prologue: page list, column metadata, Q (swizzled K-major B operand), ones, barriers, TMEM ------
     for (int i = tid; i < n_my; i += kUmmaThreads) {
       const int j = p.sel_pages[unit * p.k_max + beg + i];
       s_list[i] = j;
       s_list[pps + i] = p.sel_prev[unit * p.k_max + beg + i];
       s_list[2 * pps + i] = p.block_table[(size_t)b * p.max_pages + j];
     }
+    for (int c = tid; c < NT; c += kUmmaThreads) {
+      int pos = -1, off = 0;
+      if (c < rows) {
+        const int r = c / G, g = c % G;
+        pos = p.q_pos[b * R + r];
+        if (pos > t || pos < t - p.window) pos = -1;
+        off = p.nsplit > 1 ? c * 128 : (int)((((size_t)r) * p.h_q + h * G + g) * 128);
+      }
+      s_colpos[c] = pos;
+      s_coloff[c] = off;
+      s_mref[c] = -INFINITY;
+      s_colmax[c] = kOrdNegInf;
+      s_alpha[c] = 1.f;
+    }
+    if (tid < 3) s_flag[tid] = 0;
     {
       const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
-      for (int i = tid; i < 128 * 16; i += kUmmaThreads) {      // 128 rows x 16 chunks of 16 B
+      for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
         const int rho = i >> 4, c = i & 15;
         uint4 v = make_uint4(0, 0, 0, 0);
         if (rho < rows) {
@@ -183,15 +275,16 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
           v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
         }
         const int half = c >> 3, ch = c & 7;
-        *reinterpret_cast<uint4*>(smem + UmmaSmem::q + half * 16384 + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
+        *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
       }
+      uint32_t* ones = reinterpret_cast<uint32_t*>(smem + lay.ones);
+      for (int i = tid; i < kOnesBytes / 4; i += kUmmaThreads) ones[i] = 0x3F803F80u;   // bf16 1.0 pairs
     }
     if (tid == 0) {
-      for (int i = 0; i < 8; ++i) mbar_init(&bars[i], 1);
+      for (int i = 0; i < 6; ++i) { mbar_init(&ring_full[i], 1); mbar_init(&ring_empty[i], 1); }
       mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
-      mbar_init(&p_ready[0], 128); mbar_init(&p_ready[1], 128);
-      mbar_init(o_full, 1);
-      mbar_init(o_done, 1);
+      mbar_init(&p_ready[0], kSoftmaxThreads); mbar_init(&p_ready[1], kSoftmaxThreads);
+      mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
       fence_mbar_init();
     }
     if (warp == 1) {
@@ -199,215 +292,246 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
                    "n"(kTmemCols));
       asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
-    fence_proxy_async();          // Q / P written through the generic proxy, read by the tensor core (async proxy)
+    fence_proxy_async();          // Q / ones written through the generic proxy, read by the tensor core
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr_s;
+    STAMP(cta0 && tid == 0, 1);
 
     if (warp == 0) {
-      // ===== TMA producer =====
-      if (lane == 0) {
-        for (int blk = 0; blk < nblk; ++blk) {
-          const int s = blk % kKvStages, n = blk / kKvStages;
-          const int np = min(kPB, n_my - blk * kPB);
-          unsigned char* kdst = smem + UmmaSmem::k + s * kStageBytes;
-          unsigned char* vdst = smem + UmmaSmem::v + s * kStageBytes;
-          if (n > 0) mbar_wait(&k_empty[s], (n - 1) & 1);
-          mbar_expect_tx(&k_full[s], np * 2 * kTileHalfBytes);
-          for (int pg = 0; pg < np; ++pg) {
-            const int row0 = (s_list[2 * pps + blk * kPB + pg] * p.h_k + h) * 16;
-            tma_load_2d(kdst + pg * kTileHalfBytes, &tmap_k, 0, row0, &k_full[s]);
-            tma_load_2d(kdst + kHalfStride + pg * kTileHalfBytes, &tmap_k, 64, row0, &k_full[s]);
-          }
-          if (n > 0) mbar_wait(&v_empty[s], (n - 1) & 1);
-          mbar_expect_tx(&v_full[s], np * 2 * kTileHalfBytes);
-          for (int pg = 0; pg < np; ++pg) {
-            const int row0 = (s_list[2 * pps + blk * kPB + pg] * p.h_k + h) * 16;
-            tma_load_2d(vdst + pg * kTileHalfBytes, &tmap_v, 0, row0, &v_full[s]);
-            tma_load_2d(vdst + kHalfStride + pg * kTileHalfBytes, &tmap_v, 64, row0, &v_full[s]);
-          }
+      // ===== TMA producer: tile sequence K(0) V(0) K(1) V(1) ... through a ring of NS 32 KB slots =====
+      for (int q = 0; q < 2 * nblk; ++q) {
+        const int blk = q >> 1, slot = q % cfg.NS, n = q / cfg.NS;
+        const int np = min(kPB, n_my - blk * kPB);
+        unsigned char* dst = smem + lay.ring + slot * kSlotBytes;
+        const CUtensorMap* map = (q & 1) ? &tmap_v : &tmap_k;
+        if (n > 0) mbar_wait(&ring_empty[slot], (n - 1) & 1);
+        if (lane == 0) mbar_expect_tx(&ring_full[slot], np * 2 * kTileHalfBytes);
+        __syncwarp();
+        if (lane < np) {
+          const int row0 = (s_list[2 * pps + blk * kPB + lane] * p.h_k + h) * 16;
+          tma_load_2d(dst + lane * kTileHalfBytes, map, 0, row0, &ring_full[slot]);
+          tma_load_2d(dst + kHalfStride + lane * kTileHalfBytes, map, 64, row0, &ring_full[slot]);
         }
       }
     } else if (warp == 1) {
       // ===== MMA issuer =====
       if (lane == 0) {
-        const uint32_t q_addr = smem_u32(smem + UmmaSmem::q);
+        const uint32_t q_addr = smem_u32(smem + lay.q);
+        const uint32_t ones_addr = smem_u32(smem + lay.ones);
+        const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
+        const uint32_t idesc_o = idesc_bf16_ab(NT, true, true);
+        const uint32_t idesc_l = idesc_bf16_ab(NT, false, true);
+        const uint64_t ones_desc = desc_kmajor_none(ones_addr, 128, 256);
         auto issue_s = [&](int blk) {
-          const int s = blk % kKvStages, n = blk / kKvStages;
-          const int np = min(kPB, n_my - blk * kPB);
-          mbar_wait(&k_full[s], n & 1);
+          const int q = 2 * blk, slot = q % cfg.NS, n = q / cfg.NS;
+          mbar_wait(&ring_full[slot], n & 1);
+          STAMP(cta0 && blk == 0, 2);
           tc_fence_after();
-          const uint32_t k_addr = smem_u32(smem + UmmaSmem::k + s * kStageBytes);
-          const uint32_t idesc = idesc_bf16(16 * np, false);
-          const uint32_t d_tmem = tmem_base + kColS + (blk & 1) * 128;
+          const uint32_t k_addr = smem_u32(smem + lay.ring + slot * kSlotBytes);
+          const uint32_t d_tmem = tmem_base + colS + (blk % cfg.NSB) * NT;
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {    // K = 128 channels = 8 steps of 16; 4 steps per 64-column half
-            const uint32_t off = (ks >> 2) * 16384 + (ks & 3) * 32;
-            umma_bf16(d_tmem, desc_kmajor_sw128(q_addr + off), desc_kmajor_sw128(k_addr + off), idesc, ks > 0);
+          for (int ks = 0; ks < 8; ++ks) {    // K = 128 channels = 8 steps of 16; 4 steps per 64-channel half
+            const uint32_t koff = (ks >> 2) * kHalfStride + (ks & 3) * 32;
+            const uint32_t qoff = (ks >> 2) * (NT * 128) + (ks & 3) * 32;
+            umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff), idesc_s, ks > 0);
           }
-          tc_commit(&k_empty[s]);
-          tc_commit(&s_full[blk & 1]);
+          tc_commit(&ring_empty[slot]);
+          tc_commit(&s_full[blk % cfg.NSB]);
         };
-        issue_s(0);
+        if (cfg.NSB == 2) issue_s(0);
         for (int blk = 0; blk < nblk; ++blk) {
-          if (blk + 1 < nblk) issue_s(blk + 1);
-          const int s = blk % kKvStages, n = blk / kKvStages;
-          const int np = min(kPB, n_my - blk * kPB);
-          mbar_wait(&p_ready[blk & 1], (blk >> 1) & 1);
-          mbar_wait(&v_full[s], n & 1);
-          tc_fence_after();
-          const uint32_t v_addr = smem_u32(smem + UmmaSmem::v + s * kStageBytes);
-          const uint32_t idesc = idesc_bf16(128, true);
-          const uint32_t p_tmem = tmem_base + kColS + (blk & 1) * 128;   // P overwrote S in place: [hi 64 | lo 64]
-          for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step = 8 TMEM columns of A
-            const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
-            umma_bf16_ts(tmem_base + kColO, p_tmem + 8 * ks, vdesc, idesc, (blk > 0 || ks > 0));
-            umma_bf16_ts(tmem_base + kColO, p_tmem + 64 + 8 * ks, vdesc, idesc, 1u);
+          if (cfg.NSB == 2) {
+            if (blk + 1 < nblk) issue_s(blk + 1);
+          } else if (blk == 0) {
+            issue_s(0);
           }
-          tc_commit(&v_empty[s]);
-          tc_commit(o_full);
-          if (blk == nblk - 1) tc_commit(o_done);
+          const int q = 2 * blk + 1, slot = q % cfg.NS, n = q / cfg.NS;
+          const int np = min(kPB, n_my - blk * kPB);
+          mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
+          if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
+          mbar_wait(&ring_full[slot], n & 1);
+          tc_fence_after();
+          const uint32_t v_addr = smem_u32(smem + lay.ring + slot * kSlotBytes);
+          const uint32_t p_addr = smem_u32(smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes);
+          for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
+            const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
+            const uint64_t phi = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
+            const uint64_t plo = desc_mnmajor_sw128(p_addr + lay.p_hl_bytes + ks * 2048, 16384);
+            const uint32_t acc = (blk > 0 || ks > 0) ? 1u : 0u;
+            umma_bf16(tmem_base + colO, vdesc, phi, idesc_o, acc);
+            umma_bf16(tmem_base + colO, vdesc, plo, idesc_o, 1u);
+            umma_bf16(tmem_base + colL, ones_desc, phi, idesc_l, acc);
+            umma_bf16(tmem_base + colL, ones_desc, plo, idesc_l, 1u);
+          }
+          tc_commit(&ring_empty[slot]);
+          tc_commit(&o_full[blk & 1]);
         }
       }
     } else {
-      // ===== softmax warps: thread <-> TMEM lane <-> query row =====
-      const int quarter = warp & 3;                       // TMEM lanes a warp may touch: 32*(warp%4)..+31
-      const int rho = quarter * 32 + lane;
-      const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-      int pos = -1;
-      if (rho < rows) {
-        pos = p.q_pos[b * R + rho / G];
-        if (pos > t || pos < t - p.window) pos = -1;
-      }
-      const bool real = pos >= 0;
-      float m_ref = -INFINITY, l_run = 0.f;               // running max (log2 units) used as exponent reference
+      // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NHALF columns (rows) each =====
+      const int quadrant = warp & 3;                      // TMEM lanes a warp may touch: 32*(warp%4)..+31
+      const int half = (warp - 2) >> 2;
+      const int key = quadrant * 32 + lane;
+      const int cbeg = half * NHALF;
+      const int st = tid - 64;                            // 0..255
+      const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
+      constexpr int kActWords = (NHALF + 31) / 32;
       for (int blk = 0; blk < nblk; ++blk) {
         const int np = min(kPB, n_my - blk * kPB);
-        // valid-token count of each page of the block for this row (0 = page masked for this query)
-        uint32_t nv_lo = 0, nv_hi = 0;                    // 8 x 5 bits packed: pages 0..5 in lo, 6..7 in hi
-        if (real) {
-          for (int pg = 0; pg < np; ++pg) {
-            const int j = s_list[blk * kPB + pg], prev = s_list[pps + blk * kPB + pg];
-            int nv = (prev < pos) ? min(pos - j * 16 + 1, 16) : 0;
-            nv = max(nv, 0);
-            if (pg < 6) nv_lo |= (uint32_t)nv << (5 * pg); else nv_hi |= (uint32_t)nv << (5 * (pg - 6));
-          }
+        // key visible to the row at position pos  <=>  sel_prev < pos and token position <= pos  <=>  pos > thr
+        int thr = 0x7fffffff;
+        if ((key >> 4) < np) {
+          const int j = s_list[blk * kPB + (key >> 4)], prev = s_list[pps + blk * kPB + (key >> 4)];
+          thr = max(prev, j * 16 + (key & 15) - 1);
         }
-        auto nvalid = [&](int pg) -> int {
-          return pg < 6 ? (int)((nv_lo >> (5 * pg)) & 31u) : (int)((nv_hi >> (5 * (pg - 6))) & 31u);
-        };
-        mbar_wait(&s_full[blk & 1], (blk >> 1) & 1);
+        if (st == 0) s_flag[(blk + 1) % 3] = 0;
+        mbar_wait(&s_full[blk % cfg.NSB], (blk / cfg.NSB) & 1);
+        STAMP(cta0 && st == 0, 3 + 4 * min(blk, 3));
         tc_fence_after();
-        const uint32_t s_addr = lane_addr + kColS + (blk & 1) * 128;
-        // pass 1: row max over the unmasked columns
-        float mx = -INFINITY;
+        const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
+        float xs[NHALF];
+        {
+          uint32_t raw[NHALF];
 #pragma unroll
-        for (int c4 = 0; c4 < 4; ++c4) {
-          if (c4 * 2 < np) {                               // warp-uniform
-            uint32_t sv[32];
-            tmem_ld32(s_addr + c4 * 32, sv);
-            tmem_wait_ld();
-            const int nv0 = nvalid(c4 * 2), nv1 = nvalid(c4 * 2 + 1);
-#pragma unroll
-            for (int c = 0; c < 16; ++c) {
-              if (c < nv0) mx = fmaxf(mx, __uint_as_float(sv[c]));
-              if (c < nv1) mx = fmaxf(mx, __uint_as_float(sv[16 + c]));
-            }
-          }
-        }
-        mx *= p.scale_log2;                                // scale > 0: max commutes with the scaling; -inf stays
-        // O is rescaled only when some row of the warp moved its max by more than 2^kRescaleThreshold; otherwise
-        // the stale reference keeps P <= 2^8 and the final 1/l normalisation absorbs it.  While m_ref = -inf the
-        // row's P has been all zeros, so its O row is exactly 0 and needs no rescale.
-        const bool need = real && m_ref > -INFINITY && mx > m_ref + kRescaleThreshold;
-        if (__any_sync(0xffffffffu, need)) {
-          mbar_wait(o_full, (blk - 1) & 1);                // PV(blk-1) retired: O is ours (need implies blk > 0)
-          tc_fence_after();
-          float alpha = 1.f;
-          if (need) {
-            alpha = ex2_approx(m_ref - mx);
-            m_ref = mx;
-            l_run *= alpha;
-          }
-#pragma unroll
-          for (int c4 = 0; c4 < 4; ++c4) {
-            uint32_t ov[32];
-            tmem_ld32(lane_addr + kColO + c4 * 32, ov);
-            tmem_wait_ld();
-#pragma unroll
-            for (int c = 0; c < 32; ++c) ov[c] = __float_as_uint(__uint_as_float(ov[c]) * alpha);
-            tmem_st32(lane_addr + kColO + c4 * 32, ov);
-          }
-          tmem_wait_st();
-        }
-        if (real && m_ref == -INFINITY && mx > -INFINITY) m_ref = mx;   // first visible keys of this row
-        // pass 2: P = 2^(s*scale - m_ref) as bf16 hi + lo, written over S in place: hi of chunk c4 lands in
-        // columns [16 c4, 16 c4 + 16) (already read), lo is held back until every S chunk has been read.
-        const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
-        float lsum = 0.f;
-        uint32_t plo[4][16];
-#pragma unroll
-        for (int c4 = 0; c4 < 4; ++c4) {
-          if (c4 * 2 < np) {
-            uint32_t sv[32];
-            tmem_ld32(s_addr + c4 * 32, sv);
-            tmem_wait_ld();
-            const int nv0 = nvalid(c4 * 2), nv1 = nvalid(c4 * 2 + 1);   // 0 for padding / empty rows
-            uint32_t phi[16];
-#pragma unroll
-            for (int c = 0; c < 32; c += 2) {
-              const int nv = c < 16 ? nv0 : nv1;
-              const int tk = c & 15;
-              float e0 = 0.f, e1 = 0.f;
-              if (tk < nv) e0 = ex2_approx(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use));
-              if (tk + 1 < nv) e1 = ex2_approx(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use));
-              lsum += e0 + e1;
-              split_bf16x2(e0, e1, phi[c >> 1], plo[c4][c >> 1]);
-            }
-            tmem_st16(s_addr + c4 * 16, phi);
-          }
-        }
-#pragma unroll
-        for (int c4 = 0; c4 < 4; ++c4)
-          if (c4 * 2 < np) tmem_st16(s_addr + 64 + c4 * 16, plo[c4]);
-        tmem_wait_st();
-        l_run += lsum;
-        tc_fence_before();
-        mbar_arrive(&p_ready[blk & 1]);
-      }
-      // ---- epilogue: O / l and the base-2 lse of this split ----
-      mbar_wait(o_done, 0);
-      tc_fence_after();
-      const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
-      const float lse2 = l_run > 0.f ? m_ref + log2f(l_run) : -INFINITY;
-      float* dst;
-      if (p.nsplit > 1) {
-        dst = p.split_o + ((unit * p.nsplit + split) * rows + rho) * 128;
-        if (rho < rows) p.split_lse[(unit * p.nsplit + split) * rows + rho] = lse2;
-      } else {
-        const int r = rho / G, g = rho % G;
-        dst = p.part_o + (((size_t)b * R + r) * p.h_q + h * G + g) * 128;
-        if (rho < rows) p.part_lse[((size_t)b * R + r) * p.h_q + h * G + g] = lse2 * kLn2;
-      }
-      if (quarter * 32 < rows) {                           // warp-uniform: this warp owns at least one real row
-#pragma unroll
-        for (int c4 = 0; c4 < 4; ++c4) {
-          uint32_t ov[32];
-          tmem_ld32(lane_addr + kColO + c4 * 32, ov);
+          for (int i = 0; i < NCH; ++i) tmem_ld8(s_addr + 8 * i, raw + 8 * i);
           tmem_wait_ld();
-          if (rho < rows) {
 #pragma unroll
-            for (int c = 0; c < 32; c += 4)
-              *reinterpret_cast<float4*>(dst + c4 * 32 + c) =
-                  make_float4(__uint_as_float(ov[c]) * inv, __uint_as_float(ov[c + 1]) * inv,
-                              __uint_as_float(ov[c + 2]) * inv, __uint_as_float(ov[c + 3]) * inv);
+          for (int j = 0; j < NHALF; ++j) xs[j] = __uint_as_float(raw[j]) * p.scale_log2;
+        }
+        uint32_t act[kActWords];
+#pragma unroll
+        for (int i = 0; i < kActWords; ++i) act[i] = 0;
+        float tmax = -INFINITY;
+#pragma unroll
+        for (int j = 0; j < NHALF; j += 4) {
+          const int4 ps = *reinterpret_cast<const int4*>(s_colpos + cbeg + j);
+          const float4 mr = *reinterpret_cast<const float4*>(s_mref + cbeg + j);
+          const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
+          const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (pv[u] > thr) {
+              act[(j + u) >> 5] |= 1u << ((j + u) & 31);
+              tmax = fmaxf(tmax, xs[j + u] - mv[u]);      // m_ref = -inf (row not started) -> +inf
+            }
+          }
+        }
+        if (__any_sync(0xffffffffu, tmax > kRescaleThreshold) && lane == 0) s_flag[blk % 3] = 1;
+        softmax_bar();
+        STAMP(cta0 && st == 0, 4 + 4 * min(blk, 3));
+        if (s_flag[blk % 3] != 0) {
+          // ---- slow path: exact column max of this block, raise m_ref, rescale O and L ----
+          int mine = kOrdNegInf;
+#pragma unroll
+          for (int j = 0; j < NHALF; ++j) {
+            const bool a = (act[j >> 5] >> (j & 31)) & 1u;
+            const int r = __reduce_max_sync(0xffffffffu, a ? f2o(xs[j]) : kOrdNegInf);
+            if ((j & 31) == lane) mine = r;
+            if ((j & 31) == 31 || j == NHALF - 1) {
+              if (lane <= (j & 31)) atomicMax(&s_colmax[cbeg + (j & ~31) + lane], mine);
+            }
+          }
+          softmax_bar();
+          if (st < NT) {
+            const float bm = o2f(s_colmax[st]), old = s_mref[st];
+            const float nw = fmaxf(old, bm);
+            s_alpha[st] = (old == -INFINITY) ? 1.f : ex2_approx(old - nw);
+            s_mref[st] = nw;
+            s_colmax[st] = kOrdNegInf;
+          }
+          softmax_bar();
+          if (blk > 0) {
+            mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O and L are ours
+            tc_fence_after();
+#pragma unroll
+            for (int i = 0; i < NCH; ++i) {
+              uint32_t ov[8], lv[8];
+              tmem_ld8(lane_addr + colO + cbeg + 8 * i, ov);
+              tmem_ld8(lane_addr + colL + cbeg + 8 * i, lv);
+              tmem_wait_ld();
+#pragma unroll
+              for (int u = 0; u < 8; ++u) {
+                const float al = s_alpha[cbeg + 8 * i + u];
+                ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
+                lv[u] = __float_as_uint(__uint_as_float(lv[u]) * al);
+              }
+              tmem_st8(lane_addr + colO + cbeg + 8 * i, ov);
+              tmem_st8(lane_addr + colL + cbeg + 8 * i, lv);
+            }
+            tmem_wait_st();
+          }
+        }
+        if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // single P buffer: PV(blk-1) has read it
+        STAMP(cta0 && st == 0, 5 + 4 * min(blk, 3));
+        // ---- P = 2^(x - m_ref) as bf16 hi + lo into the MN-major SW128 B operand ----
+        unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
+#pragma unroll
+        for (int i = 0; i < NCH; ++i) {
+          const float4 m0 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i);
+          const float4 m1 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i + 4);
+          const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+          float e[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int j = 8 * i + u;
+            const bool a = (act[j >> 5] >> (j & 31)) & 1u;
+            e[u] = a ? ex2_approx(xs[j] - mv[u]) : 0.f;
+          }
+          uint4 hi, lo;
+          split_bf16x2(e[0], e[1], hi.x, lo.x);
+          split_bf16x2(e[2], e[3], hi.y, lo.y);
+          split_bf16x2(e[4], e[5], hi.z, lo.z);
+          split_bf16x2(e[6], e[7], hi.w, lo.w);
+          const int col0 = cbeg + 8 * i;
+          unsigned char* dst = p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4);
+          *reinterpret_cast<uint4*>(dst) = hi;
+          *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
+        }
+        fence_proxy_async();
+        tc_fence_before();
+        mbar_arrive(&p_ready[blk % cfg.NP]);
+        STAMP(cta0 && st == 0, 6 + 4 * min(blk, 3));
+      }
+      // ---- epilogue: O / L and the base-2 lse of this split (thread = channel `key`, NHALF rows) ----
+      mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
+      STAMP(cta0 && st == 0, 20);
+      tc_fence_after();
+      float* o_base;
+      float* lse_base;
+      if (p.nsplit > 1) {
+        o_base = p.split_o + (unit * p.nsplit + split) * rows * 128;
+        lse_base = p.split_lse + (unit * p.nsplit + split) * rows;
+      } else {
+        o_base = p.part_o + (size_t)b * R * p.h_q * 128;
+        lse_base = p.part_lse + (size_t)b * R * p.h_q;
+      }
+      const float lse_scale = p.nsplit > 1 ? 1.f : kLn2;
+#pragma unroll
+      for (int i = 0; i < NCH; ++i) {
+        if (cbeg + 8 * i < rows) {                          // warp-uniform
+          uint32_t ov[8], lv[8];
+          tmem_ld8(lane_addr + colO + cbeg + 8 * i, ov);
+          tmem_ld8(lane_addr + colL + cbeg + 8 * i, lv);
+          tmem_wait_ld();
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int c = cbeg + 8 * i + u;
+            if (c < rows) {
+              const float l = __uint_as_float(lv[u]);
+              const float inv = l > 0.f ? 1.f / l : 0.f;
+              const int off = s_coloff[c];
+              o_base[off + key] = __uint_as_float(ov[u]) * inv;
+              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + log2f(l)) * lse_scale : -INFINITY;
+            }
           }
         }
       }
     }
     tc_fence_before();
     __syncthreads();
+    STAMP(cta0 && tid == 0, 21);
     if (warp == 1) {
       tc_fence_after();
       asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
@@ -427,7 +551,14 @@ attend_umma_kernel(const AttendParams p, const __grid_constant__ CUtensorMap tma
   }
   if (p.nsplit == 1) return;
   combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket);
+  STAMP(cta0 && tid == 0, 22);
 }
+
+#ifdef RETRO_STAMPS
+extern "C" int retro_debug_read_stamps(unsigned long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_stamps, sizeof(unsigned long long) * 32);
+}
+#endif
 
 // ---- host: tensor maps over the K / V pools viewed as [(phys * h_k + head) * 16 rows][128 channels] ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -461,8 +592,22 @@ static int make_pool_map(CUtensorMap* map, const void* pool, const retro_desc_t*
   return RETRO_OK;
 }
 
+template <int NCH>
+static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const UmmaCfg& cfg, size_t smem,
+                      const CUtensorMap& mk, const CUtensorMap& mv, cudaStream_t s) {
+  auto kern = attend_umma_kernel<NCH>;
+  static size_t smem_allowed = 0;   // per instantiation; raised on demand (not a stream operation)
+  if (smem > smem_allowed) {
+    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    smem_allowed = smem;
+  }
+  kern<<<dim3(prm.nsplit, d->num_kv_heads, d->batch), kUmmaThreads, smem, s>>>(prm, cfg, mk, mv);
+  RETRO_LAUNCH_CHECK();
+  return RETRO_OK;
+}
+
 int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStream_t s) {
-  // the encode is pure host work (~1 us); cache the last pair of maps (one layer stack reuses its pools)
+  // the encode is pure host work (~1 us); cache the maps per (pool pair, shape)
   struct Cached { const void* k; const void* v; int phys, hk; CUtensorMap mk, mv; };
   constexpr int kCache = 64;
   static Cached cache[kCache];
@@ -483,15 +628,34 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
     cache[slot] = c;
     hit = &cache[slot];
   }
-  const size_t smem = 1024 + UmmaSmem::list + (size_t)3 * prm.pages_per_split * sizeof(int32_t);
-  static size_t smem_allowed = 0;
-  if (smem > smem_allowed) {
-    RETRO_CUDA_TRY(cudaFuncSetAttribute(attend_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    smem_allowed = smem;
+  const int rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
+  const int nch = ceil_div(rows, 16), NT = 16 * nch;
+  if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
+  // shared-memory plan: two P buffers when at least 4 ring slots still fit, else one; at least 3 slots
+  constexpr int kSmemMax = 232448 - 1024;
+  UmmaCfg cfg;
+  cfg.NSB = 2;
+  cfg.NP = 2;
+  cfg.NS = (kSmemMax - umma_layout(NT, 0, 2, prm.pages_per_split).total) / kSlotBytes;
+  static const int force_np = [] { const char* e = std::getenv("RETRO_UMMA_NP"); return e ? atoi(e) : 0; }();
+  if (cfg.NS < 4 || force_np == 1) {
+    cfg.NP = 1;
+    cfg.NS = (kSmemMax - umma_layout(NT, 0, 1, prm.pages_per_split).total) / kSlotBytes;
   }
-  attend_umma_kernel<<<dim3(prm.nsplit, d->num_kv_heads, d->batch), kUmmaThreads, smem, s>>>(prm, hit->mk, hit->mv);
-  RETRO_LAUNCH_CHECK();
-  return RETRO_OK;
+  if (cfg.NS < 3) return RETRO_ERR_UNSUPPORTED;
+  if (cfg.NS > 6) cfg.NS = 6;
+  const size_t smem = 1024 + (size_t)umma_layout(NT, cfg.NS, cfg.NP, prm.pages_per_split).total;
+  switch (nch) {
+    case 1: return launch_nch<1>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 2: return launch_nch<2>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 3: return launch_nch<3>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 4: return launch_nch<4>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 5: return launch_nch<5>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 6: return launch_nch<6>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 7: return launch_nch<7>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 8: return launch_nch<8>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+  }
+  return RETRO_ERR_UNSUPPORTED;
 }
 
 }  // namespace retro

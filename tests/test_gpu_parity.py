@@ -59,6 +59,13 @@ def test_c5_shape_shrunk_sweep_points(w, budget):
     print("c5s errs", w, budget, GH.lockstep(inp, w + 6))
 
 
+def test_multi_block_splits_shrunk():
+    """32 units x 128 pages: every attend CTA walks several 128-key blocks (ring reuse, lazy rescale, P buffers)."""
+    cfg = wl.shrink(wl.c5(8, 2048), (2500, 2491, 2333, 2100), 12, batch=4)
+    inp = wl.make_layer_inputs(cfg)
+    print("multi-block errs", GH.lockstep(inp, 12))
+
+
 def test_edge_budget_covers_whole_cache_is_dense():
     cfg = wl.shrink(wl.c2(), (300,), 12, budget_tokens=16 * 64, window=4)
     inp = wl.make_layer_inputs(cfg)
