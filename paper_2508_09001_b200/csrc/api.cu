@@ -31,11 +31,11 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   WorkspaceLayout wl;
   const int units = d->batch * d->num_kv_heads;
   wl.rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
-  // split-KV so that units * nsplit covers the 148 SMs about twice; at least 2 pages per split.  The tensor-core
-  // path (bf16, rows <= 128) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per split, so
-  // its splits are whole blocks and at most one wave of CTAs.
+  // split-KV.  Scalar path: units * nsplit covers the 148 SMs about twice, at least 2 pages per split.  The
+  // tensor-core path (bf16, rows <= 128) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per
+  // split: its splits are whole blocks and the grid is at most ONE wave of resident CTAs (148 x CTAs per SM).
   const bool umma = d->dtype == RETRO_BF16 && wl.rows <= 128;
-  int nsplit = ceil_div((umma ? 1 : 2) * 148, units);
+  int nsplit = umma ? (148 * umma_ctas_per_sm(wl.rows)) / units : ceil_div(2 * 148, units);
   const int min_pages = umma ? 8 : 2;
   const int max_split = d->max_sel_pages >= min_pages ? d->max_sel_pages / min_pages : 1;
   if (nsplit > max_split) nsplit = max_split;

@@ -17,6 +17,9 @@ struct AttendParams {
 };
 
 #ifdef __CUDACC__
+#ifndef RETRO_COMBINE_STAMP
+#define RETRO_COMBINE_STAMP(i) do { } while (0)
+#endif
 // Called by every thread of the CTA after it wrote its split partial (normalised o, base-2 lse) to the
 // workspace.  The last CTA of the (b, KV head) unit to arrive merges the nsplit partials (Eq. 8 applied to
 // splits: weights 2^(lse_s - max)) into part_o / part_lse (natural-log lse).  D = 128 or 64; one warp per row.
@@ -26,9 +29,11 @@ __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, s
   constexpr int kCh = D / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
   __threadfence();
+  RETRO_COMBINE_STAMP(24);
   __syncthreads();
   if (tid == 0) *s_ticket = atomicAdd(&p.counters[unit], 1u);
   __syncthreads();
+  RETRO_COMBINE_STAMP(25);
   if (*s_ticket != (unsigned)(p.nsplit - 1)) return;
   if (tid == 0) p.counters[unit] = 0;   // leave the workspace consistent for the next call
   __threadfence();

@@ -24,6 +24,11 @@
 
 #include <cstdlib>
 
+#ifdef RETRO_STAMPS
+namespace retro { __device__ void retro_stamp(int i); }
+#define RETRO_COMBINE_STAMP(i) \
+  do { if ((blockIdx.x | blockIdx.y | blockIdx.z) == 0 && threadIdx.x == 64) ::retro::retro_stamp(i); } while (0)
+#endif
 #include "attend_common.cuh"
 
 namespace retro {
@@ -34,7 +39,7 @@ constexpr int kPB = 8;                        // pages per KV block (128 keys)
 constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel half) box: 16 rows x 128 B
 constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][128 B]
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
-constexpr int kOnesBytes = 4096;
+constexpr int kOnesBytes = 256;        // one 8-row x 16-deep core-matrix pair; every row group aliases it
 constexpr int kTmemCols = 512;
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
 constexpr float kRescaleThreshold = 8.f;      // log2 units
@@ -131,8 +136,25 @@ __device__ __forceinline__ uint32_t idesc_bf16(int n, bool b_mn_major) {
          ((uint32_t)(128 >> 4) << 24);
 }
 
-__device__ __forceinline__ uint32_t idesc_bf16_ab(int n, bool a_mn_major, bool b_mn_major) {
-  return idesc_bf16(n, b_mn_major) | ((a_mn_major ? 1u : 0u) << 15);
+// b_f16: the B operand holds fp16 (A stays bf16): kind::f16 takes the two formats independently.
+__device__ __forceinline__ uint32_t idesc_bf16_ab(int n, bool a_mn_major, bool b_mn_major, bool b_f16 = false) {
+  return (1u << 4) | (1u << 7) | ((b_f16 ? 0u : 1u) << 10) | ((a_mn_major ? 1u : 0u) << 15) |
+         ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 // K-major operand without swizzle: 8 x 16 B core matrices, LBO between the two K halves of a 16-deep step,
 // SBO between 8-row groups.  Used for the all-ones A operand of the row-sum MMA (its content is layout-free).
@@ -160,23 +182,22 @@ __device__ __forceinline__ int f2o(float f) {
 __device__ __forceinline__ float o2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
 constexpr int kOrdNegInf = (int)0x807fffff;   // f2o(-inf)
 
-// Dynamic shared memory map (base aligned to 1024 B).  NT = padded rows, NS = ring slots, NP = P buffers.
+// Dynamic shared memory map (1024 B aligned).  NT = padded rows, NS = ring slots, NP = P buffers,
+// PLO = 1: P as bf16 hi + bf16 lo (two B operands), 0: P as one fp16 B operand.
 struct UmmaLayout {
-  int q, ones, p, ring, bars, meta, list, total;
+  int q, ones, p, ring, list, total;
   int p_buf_bytes, p_hl_bytes;
 };
-__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
+__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int PLO, int pages_per_split) {
   UmmaLayout L;
   const int natom = (NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
-  L.ones = L.q + 2 * NT * 128;
-  L.p = L.ones + kOnesBytes;                 // [buf][hi|lo][atom][128 keys][128 B]
+  L.p = L.q + 2 * NT * 128;                  // [buf][hi|lo][atom][128 keys][128 B]
   L.p_hl_bytes = natom * 16384;
-  L.p_buf_bytes = 2 * L.p_hl_bytes;
+  L.p_buf_bytes = (1 + PLO) * L.p_hl_bytes;
   L.ring = L.p + NP * L.p_buf_bytes;
-  L.bars = L.ring + NS * kSlotBytes;         // up to 32 mbarriers
-  L.meta = L.bars + 32 * 8;                  // tmem ptr, flags, per-column arrays
-  L.list = L.meta + 64 + 5 * kMaxNT * 4;
+  L.ones = L.ring + NS * kSlotBytes;
+  L.list = L.ones + kOnesBytes;              // int32 [3][pages_per_split]
   L.total = L.list + 3 * pages_per_split * 4;
   return L;
 }
@@ -185,57 +206,60 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
 __device__ unsigned long long g_stamps[32];
 __device__ __forceinline__ void stamp(int i) {
   unsigned long long t;
-  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
   g_stamps[i] = t;
 }
 #define STAMP(cond, i) do { if (cond) stamp(i); } while (0)
+__device__ void retro_stamp(int i) { stamp(i); }
 #else
 #define STAMP(cond, i) do { } while (0)
 #endif
 
 struct UmmaCfg {
-  int NS;    // ring slots (32 KB each)
-  int NP;    // P buffers (1 or 2)
-  int NSB;   // S buffers in TMEM (1 or 2)
+  int NS;         // ring slots (32 KB each)
+  int NP;         // P buffers (1 or 2)
+  int NSB;        // S buffers in TMEM (1 or 2)
+  int PLO;        // 1: P = bf16 hi + lo, 0: P = fp16
+  int tmem_cols;  // power of two >= (NSB + 2) * NT
 };
 
 // NCH = NT / 16 = number of 8-column chunks each softmax thread owns (its half of the padded rows).
+// Two CTAs share an SM when NT <= 48 (TMA gather throughput per CTA saturates well below the SM's share of HBM).
 template <int NCH>
-__global__ void __launch_bounds__(kUmmaThreads, 1)
+__global__ void __launch_bounds__(kUmmaThreads, NCH <= 3 ? 2 : 1)
 attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constant__ CUtensorMap tmap_k,
                    const __grid_constant__ CUtensorMap tmap_v) {
   constexpr int NT = 16 * NCH;
   constexpr int NHALF = 8 * NCH;
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  extern __shared__ __align__(1024) unsigned char smem[];
+  __shared__ __align__(8) uint64_t bars[24];
+  __shared__ uint32_t tmem_ptr_s;
+  __shared__ int s_flag[3];
+  __shared__ unsigned int s_ticket;
+  __shared__ __align__(16) int s_colpos[NT];     // position of the row, -1 = none
+  __shared__ __align__(16) float s_mref[NT];     // running reference (log2 units)
+  __shared__ __align__(16) int s_colmax[NT];     // ordered-int block max (slow path)
+  __shared__ __align__(16) float s_alpha[NT];
+  __shared__ __align__(16) int s_coloff[NT];     // output offset (floats) of the row
   const int pps = p.pages_per_split;
-  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, pps);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + lay.bars);
+  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, cfg.PLO, pps);
   uint64_t* ring_full = bars;            // [NS <= 6]
   uint64_t* ring_empty = bars + 6;       // [NS <= 6]
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
   uint64_t* o_full = bars + 16;          // [2] PV + L of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
-  uint32_t* tmem_ptr_s = reinterpret_cast<uint32_t*>(smem + lay.meta);
-  int* s_flag = reinterpret_cast<int*>(smem + lay.meta + 16);          // [3]
-  int* s_colpos = reinterpret_cast<int*>(smem + lay.meta + 64);        // [kMaxNT] position of the row, -1 = none
-  float* s_mref = reinterpret_cast<float*>(s_colpos + kMaxNT);         // running reference (log2 units)
-  int* s_colmax = reinterpret_cast<int*>(s_mref + kMaxNT);             // ordered-int block max (slow path)
-  float* s_alpha = reinterpret_cast<float*>(s_colmax + kMaxNT);
-  int* s_coloff = reinterpret_cast<int*>(s_alpha + kMaxNT);            // output offset (floats) of the row
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
-  __shared__ unsigned int s_ticket;
 
   const int split = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
   STAMP(cta0 && tid == 0, 0);
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
-  const int L = p.seq_lens[b];
-  const int t = L - 1;
   const size_t unit = (size_t)b * p.h_k + h;
   const int count = p.sel_count[unit];
+  const int L = p.seq_lens[b];
+  const int t = L - 1;
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
   const int n_my = end - beg;
@@ -243,42 +267,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   const int colS = 0, colO = cfg.NSB * NT, colL = colO + NT;
 
   if (nblk > 0) {
-    // ---- prologue: page list, column metadata, Q (swizzled K-major B operand), ones, barriers, TMEM ------
+    // ---- prologue: page list (two dependent loads: start them first), barriers, TMEM, Q, column metadata ----
     for (int i = tid; i < n_my; i += kUmmaThreads) {
       const int j = p.sel_pages[unit * p.k_max + beg + i];
       s_list[i] = j;
       s_list[pps + i] = p.sel_prev[unit * p.k_max + beg + i];
       s_list[2 * pps + i] = p.block_table[(size_t)b * p.max_pages + j];
-    }
-    for (int c = tid; c < NT; c += kUmmaThreads) {
-      int pos = -1, off = 0;
-      if (c < rows) {
-        const int r = c / G, g = c % G;
-        pos = p.q_pos[b * R + r];
-        if (pos > t || pos < t - p.window) pos = -1;
-        off = p.nsplit > 1 ? c * 128 : (int)((((size_t)r) * p.h_q + h * G + g) * 128);
-      }
-      s_colpos[c] = pos;
-      s_coloff[c] = off;
-      s_mref[c] = -INFINITY;
-      s_colmax[c] = kOrdNegInf;
-      s_alpha[c] = 1.f;
-    }
-    if (tid < 3) s_flag[tid] = 0;
-    {
-      const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
-      for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
-        const int rho = i >> 4, c = i & 15;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (rho < rows) {
-          const int r = rho / G, g = rho % G;
-          v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
-        }
-        const int half = c >> 3, ch = c & 7;
-        *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
-      }
-      uint32_t* ones = reinterpret_cast<uint32_t*>(smem + lay.ones);
-      for (int i = tid; i < kOnesBytes / 4; i += kUmmaThreads) ones[i] = 0x3F803F80u;   // bf16 1.0 pairs
     }
     if (tid == 0) {
       for (int i = 0; i < 6; ++i) { mbar_init(&ring_full[i], 1); mbar_init(&ring_empty[i], 1); }
@@ -288,15 +282,45 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       fence_mbar_init();
     }
     if (warp == 1) {
-      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_ptr_s)),
-                   "n"(kTmemCols));
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_ptr_s)),
+                   "r"(cfg.tmem_cols));
       asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    if (tid < 3) s_flag[tid] = 0;
+    for (int c = tid; c < NT; c += kUmmaThreads) {
+      int pos = -1, off = 0;
+      if (c < rows) {
+        const int r = c / G, g = c - r * G;
+        pos = p.q_pos[b * R + r];
+        if (pos > t || pos < t - p.window) pos = -1;
+        off = p.nsplit > 1 ? c * 128 : (r * p.h_q + h * G + g) * 128;
+      }
+      s_colpos[c] = pos;
+      s_coloff[c] = off;
+      s_mref[c] = -INFINITY;
+      s_colmax[c] = kOrdNegInf;
+      s_alpha[c] = 1.f;
+    }
+    {
+      const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
+      for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
+        const int rho = i >> 4, c = i & 15;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (rho < rows) {
+          const int r = rho / G, g = rho - r * G;
+          v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
+        }
+        const int half = c >> 3, ch = c & 7;
+        *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
+      }
+      uint32_t* ones = reinterpret_cast<uint32_t*>(smem + lay.ones);
+      for (int i = tid; i < kOnesBytes / 4; i += kUmmaThreads) ones[i] = 0x3F803F80u;   // bf16 1.0 pairs
     }
     fence_proxy_async();          // Q / ones written through the generic proxy, read by the tensor core
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_ptr_s;
+    const uint32_t tmem_base = tmem_ptr_s;
     STAMP(cta0 && tid == 0, 1);
 
     if (warp == 0) {
@@ -309,10 +333,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         if (n > 0) mbar_wait(&ring_empty[slot], (n - 1) & 1);
         if (lane == 0) mbar_expect_tx(&ring_full[slot], np * 2 * kTileHalfBytes);
         __syncwarp();
-        if (lane < np) {
-          const int row0 = (s_list[2 * pps + blk * kPB + lane] * p.h_k + h) * 16;
-          tma_load_2d(dst + lane * kTileHalfBytes, map, 0, row0, &ring_full[slot]);
-          tma_load_2d(dst + kHalfStride + lane * kTileHalfBytes, map, 64, row0, &ring_full[slot]);
+        if (lane < 2 * np) {                  // lane = 2 * page + channel half: 16 boxes in flight at once
+          const int pg = lane >> 1, hf = lane & 1;
+          const int row0 = (s_list[2 * pps + blk * kPB + pg] * p.h_k + h) * 16;
+          tma_load_2d(dst + hf * kHalfStride + pg * kTileHalfBytes, map, hf * 64, row0, &ring_full[slot]);
         }
       }
     } else if (warp == 1) {
@@ -320,10 +344,11 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       if (lane == 0) {
         const uint32_t q_addr = smem_u32(smem + lay.q);
         const uint32_t ones_addr = smem_u32(smem + lay.ones);
+        const bool f16p = cfg.PLO == 0;
         const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
-        const uint32_t idesc_o = idesc_bf16_ab(NT, true, true);
-        const uint32_t idesc_l = idesc_bf16_ab(NT, false, true);
-        const uint64_t ones_desc = desc_kmajor_none(ones_addr, 128, 256);
+        const uint32_t idesc_o = idesc_bf16_ab(NT, true, true, f16p);
+        const uint32_t idesc_l = idesc_bf16_ab(NT, false, true, f16p);
+        const uint64_t ones_desc = desc_kmajor_none(ones_addr, 128, 0);   // SBO = 0: all 16 row groups alias
         auto issue_s = [&](int blk) {
           const int q = 2 * blk, slot = q % cfg.NS, n = q / cfg.NS;
           mbar_wait(&ring_full[slot], n & 1);
@@ -358,12 +383,14 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
             const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
             const uint64_t phi = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
-            const uint64_t plo = desc_mnmajor_sw128(p_addr + lay.p_hl_bytes + ks * 2048, 16384);
             const uint32_t acc = (blk > 0 || ks > 0) ? 1u : 0u;
             umma_bf16(tmem_base + colO, vdesc, phi, idesc_o, acc);
-            umma_bf16(tmem_base + colO, vdesc, plo, idesc_o, 1u);
             umma_bf16(tmem_base + colL, ones_desc, phi, idesc_l, acc);
-            umma_bf16(tmem_base + colL, ones_desc, plo, idesc_l, 1u);
+            if (!f16p) {
+              const uint64_t plo = desc_mnmajor_sw128(p_addr + lay.p_hl_bytes + ks * 2048, 16384);
+              umma_bf16(tmem_base + colO, vdesc, plo, idesc_o, 1u);
+              umma_bf16(tmem_base + colL, ones_desc, plo, idesc_l, 1u);
+            }
           }
           tc_commit(&ring_empty[slot]);
           tc_commit(&o_full[blk & 1]);
@@ -463,9 +490,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             tmem_wait_st();
           }
         }
-        if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // single P buffer: PV(blk-1) has read it
+        if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) has read P
         STAMP(cta0 && st == 0, 5 + 4 * min(blk, 3));
-        // ---- P = 2^(x - m_ref) as bf16 hi + lo into the MN-major SW128 B operand ----
+        // ---- P = 2^(x - m_ref): fp16, or bf16 hi + lo, into the MN-major SW128 B operand ----
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
@@ -479,15 +506,20 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             const bool a = (act[j >> 5] >> (j & 31)) & 1u;
             e[u] = a ? ex2_approx(xs[j] - mv[u]) : 0.f;
           }
-          uint4 hi, lo;
-          split_bf16x2(e[0], e[1], hi.x, lo.x);
-          split_bf16x2(e[2], e[3], hi.y, lo.y);
-          split_bf16x2(e[4], e[5], hi.z, lo.z);
-          split_bf16x2(e[6], e[7], hi.w, lo.w);
           const int col0 = cbeg + 8 * i;
           unsigned char* dst = p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4);
-          *reinterpret_cast<uint4*>(dst) = hi;
-          *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
+          if (cfg.PLO) {
+            uint4 hi, lo;
+            split_bf16x2(e[0], e[1], hi.x, lo.x);
+            split_bf16x2(e[2], e[3], hi.y, lo.y);
+            split_bf16x2(e[4], e[5], hi.z, lo.z);
+            split_bf16x2(e[6], e[7], hi.w, lo.w);
+            *reinterpret_cast<uint4*>(dst) = hi;
+            *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
+          } else {
+            *reinterpret_cast<uint4*>(dst) = make_uint4(pack_f16x2(e[0], e[1]), pack_f16x2(e[2], e[3]),
+                                                        pack_f16x2(e[4], e[5]), pack_f16x2(e[6], e[7]));
+          }
         }
         fence_proxy_async();
         tc_fence_before();
@@ -515,26 +547,29 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           tmem_ld8(lane_addr + colO + cbeg + 8 * i, ov);
           tmem_ld8(lane_addr + colL + cbeg + 8 * i, lv);
           tmem_wait_ld();
+          STAMP(cta0 && st == 0 && i < 2, 26 + 2 * i);
 #pragma unroll
           for (int u = 0; u < 8; ++u) {
             const int c = cbeg + 8 * i + u;
             if (c < rows) {
               const float l = __uint_as_float(lv[u]);
-              const float inv = l > 0.f ? 1.f / l : 0.f;
+              const float inv = l > 0.f ? rcp_approx(l) : 0.f;
               const int off = s_coloff[c];
               o_base[off + key] = __uint_as_float(ov[u]) * inv;
-              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + log2f(l)) * lse_scale : -INFINITY;
+              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + lg2_approx(l)) * lse_scale : -INFINITY;
             }
           }
+          STAMP(cta0 && st == 0 && i == 0, 27);
         }
       }
+      STAMP(cta0 && st == 0, 23);
     }
     tc_fence_before();
     __syncthreads();
     STAMP(cta0 && tid == 0, 21);
     if (warp == 1) {
       tc_fence_after();
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols));
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
     }
   } else {
     // no page for this split: empty partial for every row
@@ -599,6 +634,8 @@ static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const Umma
   static size_t smem_allowed = 0;   // per instantiation; raised on demand (not a stream operation)
   if (smem > smem_allowed) {
     RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                        cudaSharedmemCarveoutMaxShared));
     smem_allowed = smem;
   }
   kern<<<dim3(prm.nsplit, d->num_kv_heads, d->batch), kUmmaThreads, smem, s>>>(prm, cfg, mk, mv);
@@ -631,20 +668,35 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   const int rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
   const int nch = ceil_div(rows, 16), NT = 16 * nch;
   if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
-  // shared-memory plan: two P buffers when at least 4 ring slots still fit, else one; at least 3 slots
-  constexpr int kSmemMax = 232448 - 1024;
+  // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~1.5 KB static; two CTAs per SM up to
+  // 64 padded rows.  Prefer two P buffers and two S buffers; the ring takes what is left (>= 2 slots: K and V of
+  // one block in flight per CTA).
+  const int per_sm = umma_ctas_per_sm(rows);
   UmmaCfg cfg;
+  cfg.PLO = 1;     // a bf16 A (V) with an fp16 B (P) operand is rejected by the hardware (illegal instruction)
   cfg.NSB = 2;
-  cfg.NP = 2;
-  cfg.NS = (kSmemMax - umma_layout(NT, 0, 2, prm.pages_per_split).total) / kSlotBytes;
-  static const int force_np = [] { const char* e = std::getenv("RETRO_UMMA_NP"); return e ? atoi(e) : 0; }();
-  if (cfg.NS < 4 || force_np == 1) {
-    cfg.NP = 1;
-    cfg.NS = (kSmemMax - umma_layout(NT, 0, 1, prm.pages_per_split).total) / kSlotBytes;
-  }
-  if (cfg.NS < 3) return RETRO_ERR_UNSUPPORTED;
+  auto plan = [&](int budget) {
+    cfg.NP = 2;
+    cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, cfg.PLO, prm.pages_per_split).total) / kSlotBytes;
+    if (cfg.NS < 2) {
+      cfg.NP = 1;
+      cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, cfg.PLO, prm.pages_per_split).total) / kSlotBytes;
+    }
+  };
+  plan((per_sm == 2 ? 233472 / 2 : 232448) - 1024 - 2048);
+  if (cfg.NS < 2 && per_sm == 2) plan(232448 - 1024 - 2048);     // does not fit twice: one CTA per SM
+  if (cfg.NS < 2) return RETRO_ERR_UNSUPPORTED;
   if (cfg.NS > 6) cfg.NS = 6;
-  const size_t smem = 1024 + (size_t)umma_layout(NT, cfg.NS, cfg.NP, prm.pages_per_split).total;
+  int cols = 32;
+  while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
+  if (cols > kTmemCols / per_sm) {
+    cfg.NSB = 1;
+    cols = 32;
+    while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
+  }
+  if (cols > kTmemCols / per_sm) return RETRO_ERR_UNSUPPORTED;
+  cfg.tmem_cols = cols;
+  const size_t smem = (size_t)umma_layout(NT, cfg.NS, cfg.NP, cfg.PLO, prm.pages_per_split).total;
   switch (nch) {
     case 1: return launch_nch<1>(d, prm, cfg, smem, hit->mk, hit->mv, s);
     case 2: return launch_nch<2>(d, prm, cfg, smem, hit->mk, hit->mv, s);
