@@ -2,23 +2,26 @@
 // the selected pages is a dense contraction (Eq. 2 / 6 / 7; arithmetic intensity ~ rows
 // flop per KV byte), far above what the fp32 ALUs sustain at HBM rate once rows > ~8.
 //
-// KEYS sit on the 128 TMEM lanes, query rows on the N dimension (N = rows padded to 16), so no tensor-core
-// or softmax work is spent on row padding and every softmax thread owns one key:
-//   S^T = K Q^T        A = K block [128 keys x 128 ch] (K-major, TMA SW128), B = Q [N x 128]   -> TMEM S  [key][row]
-//   O^T += V^T P^T     A = V block (MN-major),                               B = P [128 keys x N] -> TMEM O  [ch][row]
-//   L   += 1  P^T      A = ones,                                             B = P               -> TMEM L  [ * ][row]
-// Row sums (L) and the PV product both come from the tensor core; the softmax threads do element-wise work only:
+// Per block of 8 pages (128 keys), two tensor-core passes, each reading the 32 KB K or V block from shared
+// memory exactly once (small-N tcgen05.mma is bound by the operand fetch from shared memory, not by the math):
+//   S^T = K Q^T    A = K block [128 keys x 128 ch] (K-major, TMA SW128), B = Q [NT rows x 128 ch], N = NT
+//                  -> TMEM S [lane = key][column = row]: every softmax thread owns one key, no row padding.
+//   O  += P V      A = [P_hi ; P_lo] stacked on M (64 rows of bf16 hi, 64 rows of bf16 lo, MN-major),
+//                  B = V block [128 keys x 128 ch] (MN-major), N = 128
+//                  -> TMEM O [lane = row (hi) | 64 + row (lo)][column = channel]; O = O_hi + O_lo in the epilogue.
 // P = 2^(s*scale - m_ref[row]) with the retrospective mask (page j is visible to the row at position p iff
-// sel_prev_j < p; token l iff l <= p), written to shared memory as bf16 hi + bf16 lo (MN-major SW128 B operand).
-// m_ref is a per-row reference kept in shared memory; it is raised (and O, L rescaled) only when some logit
-// exceeds it by more than 2^8, found by a cheap per-thread check, so the common block needs no reduction.
+// sel_prev_j < p; token l iff l <= p) goes to shared memory as bf16 hi + bf16 lo: a single bf16 P (2^-9) leaves
+// |err| ~ 2^-9 |v| on the x8 outlier channels of V, outside the 2e-2 tolerance, and the hardware rejects a bf16
+// A with an fp16 B operand.  Row sums L are accumulated by the softmax threads themselves (a 3-level halving
+// shuffle per block, finished once per CTA).  m_ref is a per-row reference in shared memory; it is raised (and
+// O, L rescaled) only when some logit exceeds it by more than 2^8, so the common block needs no reduction.
 //
 // One CTA per (split, KV head, sequence), 320 threads, warp-specialised:
 //   warp 0      TMA producer: every selected (page, head) K / V tile arrives as two 64-channel boxes with the
 //               128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier) into a ring of 32 KB slots
 //               (8 pages = 128 keys of K, then the same 128 keys of V, ...).
 //   warp 1      MMA issuer (one elected thread), owns the TMEM allocation; tcgen05.commit signals mbarriers.
-//   warps 2..9  softmax: lane quadrant = warp % 4 (32 keys), column half = (warp - 2) / 4.
+//   warps 2..9  softmax: TMEM lane quadrant = warp % 4 (32 keys), column half = (warp - 2) / 4.
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
 
@@ -39,9 +42,9 @@ constexpr int kPB = 8;                        // pages per KV block (128 keys)
 constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel half) box: 16 rows x 128 B
 constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][128 B]
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
-constexpr int kOnesBytes = 256;        // one 8-row x 16-deep core-matrix pair; every row group aliases it
 constexpr int kTmemCols = 512;
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
+constexpr int kStageStride = 132;             // floats per staged output row (conflict-free 128-bit accesses)
 constexpr float kRescaleThreshold = 8.f;      // log2 units
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
@@ -102,23 +105,6 @@ __device__ __forceinline__ void split_bf16x2(float e0, float e1, uint32_t& hi, u
   const float r0 = e0 - __uint_as_float(hi << 16), r1 = e1 - __uint_as_float(hi & 0xffff0000u);
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(lo) : "f"(r1), "f"(r0));
 }
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
-        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-      : "memory");
-}
-// A operand from TMEM (lanes = rows, one 32-bit column = two consecutive K elements), B from shared memory.
-__device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc,
-                                             uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
-
 // Shared-memory matrix descriptors (cute::UMMA::SmemDescriptor bit layout), 128B swizzle, version 1.
 // K-major operand (rows of 128 B = 64 bf16 along K; 8-row groups SBO = 1024 B apart).
 __device__ __forceinline__ uint64_t desc_kmajor_sw128(uint32_t saddr) {
@@ -130,21 +116,10 @@ __device__ __forceinline__ uint64_t desc_mnmajor_sw128(uint32_t saddr, uint32_t 
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) |
          ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
-// Instruction descriptor (cute::UMMA::InstrDescriptor): D = f32, A = B = bf16, M = 128.
-__device__ __forceinline__ uint32_t idesc_bf16(int n, bool b_mn_major) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) |
-         ((uint32_t)(128 >> 4) << 24);
-}
-
-// b_f16: the B operand holds fp16 (A stays bf16): kind::f16 takes the two formats independently.
-__device__ __forceinline__ uint32_t idesc_bf16_ab(int n, bool a_mn_major, bool b_mn_major, bool b_f16 = false) {
-  return (1u << 4) | (1u << 7) | ((b_f16 ? 0u : 1u) << 10) | ((a_mn_major ? 1u : 0u) << 15) |
+// Instruction descriptor (cute::UMMA::InstrDescriptor): D = f32, A = B = bf16, M = 128, N = n.
+__device__ __forceinline__ uint32_t idesc_bf16_ab(int n, bool a_mn_major, bool b_mn_major) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((a_mn_major ? 1u : 0u) << 15) |
          ((b_mn_major ? 1u : 0u) << 16) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-}
-__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
 }
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
@@ -156,21 +131,10 @@ __device__ __forceinline__ float lg2_approx(float x) {
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// K-major operand without swizzle: 8 x 16 B core matrices, LBO between the two K halves of a 16-deep step,
-// SBO between 8-row groups.  Used for the all-ones A operand of the row-sum MMA (its content is layout-free).
-__device__ __forceinline__ uint64_t desc_kmajor_none(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) |
-         ((uint64_t)(sbo_bytes >> 4) << 32) | ((uint64_t)1 << 46);
-}
 __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                : "r"(taddr)
-               : "memory");
-}
-__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r) {
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
-               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
                : "memory");
 }
 __device__ __forceinline__ void softmax_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
@@ -182,22 +146,20 @@ __device__ __forceinline__ int f2o(float f) {
 __device__ __forceinline__ float o2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff); }
 constexpr int kOrdNegInf = (int)0x807fffff;   // f2o(-inf)
 
-// Dynamic shared memory map (1024 B aligned).  NT = padded rows, NS = ring slots, NP = P buffers,
-// PLO = 1: P as bf16 hi + bf16 lo (two B operands), 0: P as one fp16 B operand.
+// Dynamic shared memory map (1024 B aligned).  NT = padded rows, NS = ring slots, NP = P buffers.
 struct UmmaLayout {
-  int q, ones, p, ring, list, total;
+  int q, p, ring, list, total;
   int p_buf_bytes, p_hl_bytes;
 };
-__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int PLO, int pages_per_split) {
+__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
   UmmaLayout L;
   const int natom = (NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
-  L.p = L.q + 2 * NT * 128;                  // [buf][hi|lo][atom][128 keys][128 B]
+  L.p = L.q + 2 * NT * 128;                  // [buf][hi|lo][atom][128 keys][128 B = 64 rows]
   L.p_hl_bytes = natom * 16384;
-  L.p_buf_bytes = (1 + PLO) * L.p_hl_bytes;
-  L.ring = L.p + NP * L.p_buf_bytes;
-  L.ones = L.ring + NS * kSlotBytes;
-  L.list = L.ones + kOnesBytes;              // int32 [3][pages_per_split]
+  L.p_buf_bytes = 2 * L.p_hl_bytes;
+  L.ring = L.p + NP * L.p_buf_bytes;         // the first 33 KB double as the epilogue's output staging
+  L.list = L.ring + NS * kSlotBytes;         // int32 [3][pages_per_split]
   L.total = L.list + 3 * pages_per_split * 4;
   return L;
 }
@@ -219,18 +181,19 @@ struct UmmaCfg {
   int NS;         // ring slots (32 KB each)
   int NP;         // P buffers (1 or 2)
   int NSB;        // S buffers in TMEM (1 or 2)
-  int PLO;        // 1: P = bf16 hi + lo, 0: P = fp16
-  int tmem_cols;  // power of two >= (NSB + 2) * NT
+  int tmem_cols;  // power of two >= NSB * NT + 128 * atoms
 };
 
 // NCH = NT / 16 = number of 8-column chunks each softmax thread owns (its half of the padded rows).
-// Two CTAs share an SM when NT <= 48 (TMA gather throughput per CTA saturates well below the SM's share of HBM).
+// Two CTAs share an SM when NT <= 48 (shared memory and TMEM columns allow it; the second CTA hides the
+// per-block latency chain TMA -> MMA -> softmax -> MMA of the first).
 template <int NCH>
 __global__ void __launch_bounds__(kUmmaThreads, NCH <= 3 ? 2 : 1)
 attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constant__ CUtensorMap tmap_k,
                    const __grid_constant__ CUtensorMap tmap_v) {
   constexpr int NT = 16 * NCH;
   constexpr int NHALF = 8 * NCH;
+  constexpr int NATOM = (NT + 63) / 64;
   extern __shared__ __align__(1024) unsigned char smem[];
   __shared__ __align__(8) uint64_t bars[24];
   __shared__ uint32_t tmem_ptr_s;
@@ -241,88 +204,96 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(16) int s_colmax[NT];     // ordered-int block max (slow path)
   __shared__ __align__(16) float s_alpha[NT];
   __shared__ __align__(16) int s_coloff[NT];     // output offset (floats) of the row
+  __shared__ __align__(16) float s_L[NT];        // row sums (epilogue)
   const int pps = p.pages_per_split;
-  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, cfg.PLO, pps);
+  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, pps);
   uint64_t* ring_full = bars;            // [NS <= 6]
   uint64_t* ring_empty = bars + 6;       // [NS <= 6]
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
-  uint64_t* o_full = bars + 16;          // [2] PV + L of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
+  uint64_t* o_full = bars + 16;          // [2] PV of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
 
   const int split = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
+  [[maybe_unused]] const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
   STAMP(cta0 && tid == 0, 0);
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
   const size_t unit = (size_t)b * p.h_k + h;
+
+  // ---- prologue.  Global loads that depend on nothing are issued first (count, length, the list entries of
+  // this split, Q); only block_table[j] is a second round trip.
   const int count = p.sel_count[unit];
   const int L = p.seq_lens[b];
+  if (tid == 0) {
+    for (int i = 0; i < 6; ++i) { mbar_init(&ring_full[i], 1); mbar_init(&ring_empty[i], 1); }
+    mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
+    mbar_init(&p_ready[0], kSoftmaxThreads); mbar_init(&p_ready[1], kSoftmaxThreads);
+    mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
+    fence_mbar_init();
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_ptr_s)),
+                 "r"(cfg.tmem_cols));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  for (int i = tid; i < pps; i += kUmmaThreads) {
+    const int idx = split * pps + i;
+    int j = 0, prev = 0;
+    if (idx < p.k_max) {
+      j = p.sel_pages[unit * p.k_max + idx];
+      prev = p.sel_prev[unit * p.k_max + idx];
+    }
+    int phys = 0;
+    if (idx < count) phys = p.block_table[(size_t)b * p.max_pages + j];
+    s_list[i] = j;
+    s_list[pps + i] = prev;
+    s_list[2 * pps + i] = phys;
+  }
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
+    for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
+      const int rho = i >> 4, c = i & 15;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (rho < rows) {
+        const int r = rho / G, g = rho - r * G;
+        v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
+      }
+      const int half = c >> 3, ch = c & 7;
+      *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
+    }
+  }
   const int t = L - 1;
+  if (tid < 3) s_flag[tid] = 0;
+  for (int c = tid; c < NT; c += kUmmaThreads) {
+    int pos = -1, off = 0;
+    if (c < rows) {
+      const int r = c / G, g = c - r * G;
+      pos = p.q_pos[b * R + r];
+      if (pos > t || pos < t - p.window) pos = -1;
+      off = p.nsplit > 1 ? c * 128 : (r * p.h_q + h * G + g) * 128;
+    }
+    s_colpos[c] = pos;
+    s_coloff[c] = off;
+    s_mref[c] = -INFINITY;
+    s_colmax[c] = kOrdNegInf;
+    s_alpha[c] = 1.f;
+    s_L[c] = 0.f;
+  }
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
   const int n_my = end - beg;
   const int nblk = (n_my + kPB - 1) / kPB;
-  const int colS = 0, colO = cfg.NSB * NT, colL = colO + NT;
+  const int colS = 0, colO = cfg.NSB * NT;
+  fence_proxy_async();          // Q written through the generic proxy, read by the tensor core
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_ptr_s;
+  STAMP(cta0 && tid == 0, 1);
 
   if (nblk > 0) {
-    // ---- prologue: page list (two dependent loads: start them first), barriers, TMEM, Q, column metadata ----
-    for (int i = tid; i < n_my; i += kUmmaThreads) {
-      const int j = p.sel_pages[unit * p.k_max + beg + i];
-      s_list[i] = j;
-      s_list[pps + i] = p.sel_prev[unit * p.k_max + beg + i];
-      s_list[2 * pps + i] = p.block_table[(size_t)b * p.max_pages + j];
-    }
-    if (tid == 0) {
-      for (int i = 0; i < 6; ++i) { mbar_init(&ring_full[i], 1); mbar_init(&ring_empty[i], 1); }
-      mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
-      mbar_init(&p_ready[0], kSoftmaxThreads); mbar_init(&p_ready[1], kSoftmaxThreads);
-      mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
-      fence_mbar_init();
-    }
-    if (warp == 1) {
-      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_ptr_s)),
-                   "r"(cfg.tmem_cols));
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    if (tid < 3) s_flag[tid] = 0;
-    for (int c = tid; c < NT; c += kUmmaThreads) {
-      int pos = -1, off = 0;
-      if (c < rows) {
-        const int r = c / G, g = c - r * G;
-        pos = p.q_pos[b * R + r];
-        if (pos > t || pos < t - p.window) pos = -1;
-        off = p.nsplit > 1 ? c * 128 : (r * p.h_q + h * G + g) * 128;
-      }
-      s_colpos[c] = pos;
-      s_coloff[c] = off;
-      s_mref[c] = -INFINITY;
-      s_colmax[c] = kOrdNegInf;
-      s_alpha[c] = 1.f;
-    }
-    {
-      const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
-      for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
-        const int rho = i >> 4, c = i & 15;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (rho < rows) {
-          const int r = rho / G, g = rho - r * G;
-          v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
-        }
-        const int half = c >> 3, ch = c & 7;
-        *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
-      }
-      uint32_t* ones = reinterpret_cast<uint32_t*>(smem + lay.ones);
-      for (int i = tid; i < kOnesBytes / 4; i += kUmmaThreads) ones[i] = 0x3F803F80u;   // bf16 1.0 pairs
-    }
-    fence_proxy_async();          // Q / ones written through the generic proxy, read by the tensor core
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    const uint32_t tmem_base = tmem_ptr_s;
-    STAMP(cta0 && tid == 0, 1);
-
     if (warp == 0) {
       // ===== TMA producer: tile sequence K(0) V(0) K(1) V(1) ... through a ring of NS 32 KB slots =====
       for (int q = 0; q < 2 * nblk; ++q) {
@@ -343,12 +314,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       // ===== MMA issuer =====
       if (lane == 0) {
         const uint32_t q_addr = smem_u32(smem + lay.q);
-        const uint32_t ones_addr = smem_u32(smem + lay.ones);
-        const bool f16p = cfg.PLO == 0;
         const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
-        const uint32_t idesc_o = idesc_bf16_ab(NT, true, true, f16p);
-        const uint32_t idesc_l = idesc_bf16_ab(NT, false, true, f16p);
-        const uint64_t ones_desc = desc_kmajor_none(ones_addr, 128, 0);   // SBO = 0: all 16 row groups alias
+        const uint32_t idesc_o = idesc_bf16_ab(128, true, true);
         auto issue_s = [&](int blk) {
           const int q = 2 * blk, slot = q % cfg.NS, n = q / cfg.NS;
           mbar_wait(&ring_full[slot], n & 1);
@@ -382,14 +349,11 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           const uint32_t p_addr = smem_u32(smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes);
           for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
             const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
-            const uint64_t phi = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
             const uint32_t acc = (blk > 0 || ks > 0) ? 1u : 0u;
-            umma_bf16(tmem_base + colO, vdesc, phi, idesc_o, acc);
-            umma_bf16(tmem_base + colL, ones_desc, phi, idesc_l, acc);
-            if (!f16p) {
-              const uint64_t plo = desc_mnmajor_sw128(p_addr + lay.p_hl_bytes + ks * 2048, 16384);
-              umma_bf16(tmem_base + colO, vdesc, plo, idesc_o, 1u);
-              umma_bf16(tmem_base + colL, ones_desc, plo, idesc_l, 1u);
+#pragma unroll
+            for (int a = 0; a < NATOM; ++a) {   // M = 128: 64 rows of P_hi then the same 64 rows of P_lo
+              const uint64_t pdesc = desc_mnmajor_sw128(p_addr + a * 16384 + ks * 2048, lay.p_hl_bytes);
+              umma_bf16(tmem_base + colO + a * 128, pdesc, vdesc, idesc_o, acc);
             }
           }
           tc_commit(&ring_empty[slot]);
@@ -404,7 +368,11 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       const int cbeg = half * NHALF;
       const int st = tid - 64;                            // 0..255
       const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
+      const int lcol0 = cbeg + ((lane >> 2) & 7) * NCH;   // first column of this lane's partial row sums
       constexpr int kActWords = (NHALF + 31) / 32;
+      float l_part[NCH];
+#pragma unroll
+      for (int i = 0; i < NCH; ++i) l_part[i] = 0.f;
       for (int blk = 0; blk < nblk; ++blk) {
         const int np = min(kPB, n_my - blk * kPB);
         // key visible to the row at position pos  <=>  sel_prev < pos and token position <= pos  <=>  pos > thr
@@ -470,66 +438,95 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           }
           softmax_bar();
           if (blk > 0) {
-            mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O and L are ours
+#pragma unroll
+            for (int i = 0; i < NCH; ++i) l_part[i] *= s_alpha[lcol0 + i];
+            mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O is ours
             tc_fence_after();
 #pragma unroll
-            for (int i = 0; i < NCH; ++i) {
-              uint32_t ov[8], lv[8];
-              tmem_ld8(lane_addr + colO + cbeg + 8 * i, ov);
-              tmem_ld8(lane_addr + colL + cbeg + 8 * i, lv);
-              tmem_wait_ld();
+            for (int a = 0; a < NATOM; ++a) {
+              const int row = a * 64 + (key & 63);          // lanes 64..127 hold the lo part of the same rows
+              const float al = s_alpha[min(row, NT - 1)];
 #pragma unroll
-              for (int u = 0; u < 8; ++u) {
-                const float al = s_alpha[cbeg + 8 * i + u];
-                ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
-                lv[u] = __float_as_uint(__uint_as_float(lv[u]) * al);
+              for (int c = 0; c < 2; ++c) {
+                uint32_t ov[32];
+                const uint32_t addr = lane_addr + colO + a * 128 + half * 64 + c * 32;
+                tmem_ld32(addr, ov);
+                tmem_wait_ld();
+#pragma unroll
+                for (int u = 0; u < 32; ++u) ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
+                tmem_st32(addr, ov);
               }
-              tmem_st8(lane_addr + colO + cbeg + 8 * i, ov);
-              tmem_st8(lane_addr + colL + cbeg + 8 * i, lv);
             }
             tmem_wait_st();
           }
         }
         if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) has read P
         STAMP(cta0 && st == 0, 5 + 4 * min(blk, 3));
-        // ---- P = 2^(x - m_ref): fp16, or bf16 hi + lo, into the MN-major SW128 B operand ----
+        // ---- P = 2^(x - m_ref) as bf16 hi + lo into the MN-major SW128 operand ----
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
           const float4 m0 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i);
           const float4 m1 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i + 4);
           const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
-          float e[8];
 #pragma unroll
           for (int u = 0; u < 8; ++u) {
             const int j = 8 * i + u;
             const bool a = (act[j >> 5] >> (j & 31)) & 1u;
-            e[u] = a ? ex2_approx(xs[j] - mv[u]) : 0.f;
+            xs[j] = a ? ex2_approx(xs[j] - mv[u]) : 0.f;
           }
           const int col0 = cbeg + 8 * i;
           unsigned char* dst = p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4);
-          if (cfg.PLO) {
-            uint4 hi, lo;
-            split_bf16x2(e[0], e[1], hi.x, lo.x);
-            split_bf16x2(e[2], e[3], hi.y, lo.y);
-            split_bf16x2(e[4], e[5], hi.z, lo.z);
-            split_bf16x2(e[6], e[7], hi.w, lo.w);
-            *reinterpret_cast<uint4*>(dst) = hi;
-            *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
-          } else {
-            *reinterpret_cast<uint4*>(dst) = make_uint4(pack_f16x2(e[0], e[1]), pack_f16x2(e[2], e[3]),
-                                                        pack_f16x2(e[4], e[5]), pack_f16x2(e[6], e[7]));
-          }
+          uint4 hi, lo;
+          split_bf16x2(xs[8 * i + 0], xs[8 * i + 1], hi.x, lo.x);
+          split_bf16x2(xs[8 * i + 2], xs[8 * i + 3], hi.y, lo.y);
+          split_bf16x2(xs[8 * i + 4], xs[8 * i + 5], hi.z, lo.z);
+          split_bf16x2(xs[8 * i + 6], xs[8 * i + 7], hi.w, lo.w);
+          *reinterpret_cast<uint4*>(dst) = hi;
+          *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
         }
         fence_proxy_async();
         tc_fence_before();
         mbar_arrive(&p_ready[blk % cfg.NP]);
         STAMP(cta0 && st == 0, 6 + 4 * min(blk, 3));
+        // ---- row sums: three halving shuffle levels leave NCH partial sums per lane (columns lcol0 ...) ----
+        {
+          const bool up = lane & 16;
+#pragma unroll
+          for (int i = 0; i < 4 * NCH; ++i) {
+            const float send = up ? xs[i] : xs[i + 4 * NCH], keep = up ? xs[i + 4 * NCH] : xs[i];
+            xs[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+          }
+        }
+        {
+          const bool up = lane & 8;
+#pragma unroll
+          for (int i = 0; i < 2 * NCH; ++i) {
+            const float send = up ? xs[i] : xs[i + 2 * NCH], keep = up ? xs[i + 2 * NCH] : xs[i];
+            xs[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+          }
+        }
+        {
+          const bool up = lane & 4;
+#pragma unroll
+          for (int i = 0; i < NCH; ++i) {
+            const float send = up ? xs[i] : xs[i + NCH], keep = up ? xs[i + NCH] : xs[i];
+            l_part[i] += keep + __shfl_xor_sync(0xffffffffu, send, 4);
+          }
+        }
       }
-      // ---- epilogue: O / L and the base-2 lse of this split (thread = channel `key`, NHALF rows) ----
+      // ---- epilogue: L per row, O = (O_hi + O_lo) / L through a shared-memory stage, coalesced stores ----
+#pragma unroll
+      for (int i = 0; i < NCH; ++i) {
+        float v = l_part[i];
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        if ((lane & 3) == 0) atomicAdd(&s_L[lcol0 + i], v);
+      }
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
       STAMP(cta0 && st == 0, 20);
       tc_fence_after();
+      softmax_bar();                                       // s_L complete; every PV retired (ring is free)
       float* o_base;
       float* lse_base;
       if (p.nsplit > 1) {
@@ -540,36 +537,61 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         lse_base = p.part_lse + (size_t)b * R * p.h_q;
       }
       const float lse_scale = p.nsplit > 1 ? 1.f : kLn2;
+      float* stage = reinterpret_cast<float*>(smem + lay.ring);
+      const int rl = key & 63;
+      const bool is_lo = key >= 64;
+      float* my_stage = stage + rl * kStageStride + half * 64;
 #pragma unroll
-      for (int i = 0; i < NCH; ++i) {
-        if (cbeg + 8 * i < rows) {                          // warp-uniform
-          uint32_t ov[8], lv[8];
-          tmem_ld8(lane_addr + colO + cbeg + 8 * i, ov);
-          tmem_ld8(lane_addr + colL + cbeg + 8 * i, lv);
-          tmem_wait_ld();
-          STAMP(cta0 && st == 0 && i < 2, 26 + 2 * i);
+      for (int a = 0; a < NATOM; ++a) {
+        if (a * 64 < rows) {                                // CTA-uniform
+          const int row = a * 64 + rl;
+          const float l = s_L[min(row, NT - 1)];
+          const float inv = (row < rows && l > 0.f) ? rcp_approx(l) : 0.f;
+          if (a > 0) softmax_bar();                         // previous atom's stage fully written out
+          if (is_lo) {                                      // warp-uniform (quadrants 2, 3)
 #pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const int c = cbeg + 8 * i + u;
-            if (c < rows) {
-              const float l = __uint_as_float(lv[u]);
-              const float inv = l > 0.f ? rcp_approx(l) : 0.f;
-              const int off = s_coloff[c];
-              o_base[off + key] = __uint_as_float(ov[u]) * inv;
-              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + lg2_approx(l)) * lse_scale : -INFINITY;
+            for (int cc = 0; cc < 2; ++cc) {
+              uint32_t ov[32];
+              tmem_ld32(lane_addr + colO + a * 128 + half * 64 + 32 * cc, ov);
+              tmem_wait_ld();
+#pragma unroll
+              for (int c = 0; c < 8; ++c)
+                *reinterpret_cast<uint4*>(my_stage + 32 * cc + 4 * c) =
+                    make_uint4(ov[4 * c], ov[4 * c + 1], ov[4 * c + 2], ov[4 * c + 3]);
             }
           }
-          STAMP(cta0 && st == 0 && i == 0, 27);
+          softmax_bar();
+          if (!is_lo) {
+#pragma unroll
+            for (int cc = 0; cc < 2; ++cc) {
+              uint32_t ov[32];
+              tmem_ld32(lane_addr + colO + a * 128 + half * 64 + 32 * cc, ov);
+              tmem_wait_ld();
+#pragma unroll
+              for (int c = 0; c < 8; ++c) {
+                float4 v = *reinterpret_cast<float4*>(my_stage + 32 * cc + 4 * c);
+                v.x = (v.x + __uint_as_float(ov[4 * c])) * inv;
+                v.y = (v.y + __uint_as_float(ov[4 * c + 1])) * inv;
+                v.z = (v.z + __uint_as_float(ov[4 * c + 2])) * inv;
+                v.w = (v.w + __uint_as_float(ov[4 * c + 3])) * inv;
+                *reinterpret_cast<float4*>(my_stage + 32 * cc + 4 * c) = v;
+              }
+            }
+          }
+          softmax_bar();
+          STAMP(cta0 && st == 0 && a == 0, 26);
+          const int nrow = min(64, rows - a * 64);
+          for (int rr = st >> 5; rr < nrow; rr += kSoftmaxThreads / 32)
+            *reinterpret_cast<float4*>(o_base + s_coloff[a * 64 + rr] + 4 * lane) =
+                *reinterpret_cast<const float4*>(stage + rr * kStageStride + 4 * lane);
+          if (st < nrow) {
+            const int c = a * 64 + st;
+            const float lc = s_L[c];
+            lse_base[s_coloff[c] >> 7] = lc > 0.f ? (s_mref[c] + lg2_approx(lc)) * lse_scale : -INFINITY;
+          }
         }
       }
       STAMP(cta0 && st == 0, 23);
-    }
-    tc_fence_before();
-    __syncthreads();
-    STAMP(cta0 && tid == 0, 21);
-    if (warp == 1) {
-      tc_fence_after();
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
     }
   } else {
     // no page for this split: empty partial for every row
@@ -583,6 +605,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         p.part_lse[((size_t)b * R + r) * p.h_q + h * G + g] = -INFINITY;
       }
     }
+  }
+  tc_fence_before();
+  __syncthreads();
+  STAMP(cta0 && tid == 0, 21);
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
   }
   if (p.nsplit == 1) return;
   combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket);
@@ -668,35 +697,30 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   const int rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
   const int nch = ceil_div(rows, 16), NT = 16 * nch;
   if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
-  // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~1.5 KB static; two CTAs per SM up to
-  // 64 padded rows.  Prefer two P buffers and two S buffers; the ring takes what is left (>= 2 slots: K and V of
-  // one block in flight per CTA).
+  // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~2-3 KB static; two CTAs per SM up to
+  // 48 padded rows.  Prefer two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in
+  // flight per CTA, and room for the epilogue's 33 KB output stage).
   const int per_sm = umma_ctas_per_sm(rows);
+  const int natom = (NT + 63) / 64;
   UmmaCfg cfg;
-  cfg.PLO = 1;     // a bf16 A (V) with an fp16 B (P) operand is rejected by the hardware (illegal instruction)
   cfg.NSB = 2;
   auto plan = [&](int budget) {
     cfg.NP = 2;
-    cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, cfg.PLO, prm.pages_per_split).total) / kSlotBytes;
-    if (cfg.NS < 2) {
+    cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
+    if (cfg.NS < 3) {
       cfg.NP = 1;
-      cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, cfg.PLO, prm.pages_per_split).total) / kSlotBytes;
+      cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
     }
   };
-  plan((per_sm == 2 ? 233472 / 2 : 232448) - 1024 - 2048);
-  if (cfg.NS < 2 && per_sm == 2) plan(232448 - 1024 - 2048);     // does not fit twice: one CTA per SM
+  plan((per_sm == 2 ? 233472 / 2 : 232448) - 1024 - 3072);
+  if (cfg.NS < 2 && per_sm == 2) plan(232448 - 1024 - 3072);     // does not fit twice: one CTA per SM
   if (cfg.NS < 2) return RETRO_ERR_UNSUPPORTED;
   if (cfg.NS > 6) cfg.NS = 6;
   int cols = 32;
-  while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
-  if (cols > kTmemCols / per_sm) {
-    cfg.NSB = 1;
-    cols = 32;
-    while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
-  }
+  while (cols < cfg.NSB * NT + 128 * natom) cols <<= 1;
   if (cols > kTmemCols / per_sm) return RETRO_ERR_UNSUPPORTED;
   cfg.tmem_cols = cols;
-  const size_t smem = (size_t)umma_layout(NT, cfg.NS, cfg.NP, cfg.PLO, prm.pages_per_split).total;
+  const size_t smem = (size_t)umma_layout(NT, cfg.NS, cfg.NP, prm.pages_per_split).total;
   switch (nch) {
     case 1: return launch_nch<1>(d, prm, cfg, smem, hit->mk, hit->mv, s);
     case 2: return launch_nch<2>(d, prm, cfg, smem, hit->mk, hit->mv, s);
