@@ -16,12 +16,12 @@
 // shuffle per block, finished once per CTA).  m_ref is a per-row reference in shared memory; it is raised (and
 // O, L rescaled) only when some logit exceeds it by more than 2^8, so the common block needs no reduction.
 //
-// One CTA per (split, KV head, sequence), 320 threads, warp-specialised:
+// One CTA per (split, KV head, sequence), 576 threads, warp-specialised:
 //   warp 0      TMA producer: every selected (page, head) K / V tile arrives as two 64-channel boxes with the
 //               128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier) into a ring of 32 KB slots
 //               (8 pages = 128 keys of K, then the same 128 keys of V, ...).
 //   warp 1      MMA issuer (one elected thread), owns the TMEM allocation; tcgen05.commit signals mbarriers.
-//   warps 2..9  softmax: TMEM lane quadrant = warp % 4 (32 keys), column half = (warp - 2) / 4.
+//   warps 2..17 softmax: TMEM lane quadrant = warp % 4 (32 keys), column group = (warp - 2) / 4 (a quarter of the rows).
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
 
@@ -36,8 +36,8 @@ namespace retro { __device__ void retro_stamp(int i); }
 
 namespace retro {
 
-constexpr int kUmmaThreads = 320;
-constexpr int kSoftmaxThreads = 256;
+constexpr int kUmmaThreads = 576;
+constexpr int kSoftmaxThreads = 512;
 constexpr int kPB = 8;                        // pages per KV block (128 keys)
 constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel half) box: 16 rows x 128 B
 constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][128 B]
@@ -46,6 +46,7 @@ constexpr int kTmemCols = 512;
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
 constexpr int kStageStride = 132;             // floats per staged output row (conflict-free 128-bit accesses)
 constexpr float kRescaleThreshold = 8.f;      // log2 units
+constexpr float kMrefInit = -1.0e30f;         // finite "row not started" reference: -inf - kMrefInit stays -inf
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) {
@@ -131,13 +132,19 @@ __device__ __forceinline__ float lg2_approx(float x) {
   asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t* r) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(taddr)
+               : "memory");
+}
 __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                : "r"(taddr)
                : "memory");
 }
-__device__ __forceinline__ void softmax_bar() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ void softmax_bar() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 // order-preserving float <-> int image (signed compare), so a column max is one REDUX + one shared atomicMax
 __device__ __forceinline__ int f2o(float f) {
   const int i = __float_as_int(f);
@@ -184,15 +191,13 @@ struct UmmaCfg {
   int tmem_cols;  // power of two >= NSB * NT + 128 * atoms
 };
 
-// NCH = NT / 16 = number of 8-column chunks each softmax thread owns (its half of the padded rows).
-// Two CTAs share an SM when NT <= 48 (shared memory and TMEM columns allow it; the second CTA hides the
-// per-block latency chain TMA -> MMA -> softmax -> MMA of the first).
+// NCH = NT / 16; every softmax thread owns one key and NC = 4 * NCH of the padded rows (four column groups).
 template <int NCH>
-__global__ void __launch_bounds__(kUmmaThreads, NCH <= 3 ? 2 : 1)
+__global__ void __launch_bounds__(kUmmaThreads, 1)
 attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constant__ CUtensorMap tmap_k,
                    const __grid_constant__ CUtensorMap tmap_v) {
   constexpr int NT = 16 * NCH;
-  constexpr int NHALF = 8 * NCH;
+  constexpr int NC = 4 * NCH;
   constexpr int NATOM = (NT + 63) / 64;
   extern __shared__ __align__(1024) unsigned char smem[];
   __shared__ __align__(8) uint64_t bars[24];
@@ -276,7 +281,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     }
     s_colpos[c] = pos;
     s_coloff[c] = off;
-    s_mref[c] = -INFINITY;
+    s_mref[c] = kMrefInit;
     s_colmax[c] = kOrdNegInf;
     s_alpha[c] = 1.f;
     s_L[c] = 0.f;
@@ -361,18 +366,17 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         }
       }
     } else {
-      // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NHALF columns (rows) each =====
+      // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NC = NT / 4 columns (rows) each =====
+      const int sw = warp - 2;                            // 0..15
       const int quadrant = warp & 3;                      // TMEM lanes a warp may touch: 32*(warp%4)..+31
-      const int half = (warp - 2) >> 2;
+      const int cg = sw >> 2;                             // column group
       const int key = quadrant * 32 + lane;
-      const int cbeg = half * NHALF;
-      const int st = tid - 64;                            // 0..255
+      const int cbeg = cg * NC;
+      const int st = tid - 64;                            // 0..511
       const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
-      const int lcol0 = cbeg + ((lane >> 2) & 7) * NCH;   // first column of this lane's partial row sums
-      constexpr int kActWords = (NHALF + 31) / 32;
-      float l_part[NCH];
+      float l_acc[NC];                                    // this key-thread's share of the row sums
 #pragma unroll
-      for (int i = 0; i < NCH; ++i) l_part[i] = 0.f;
+      for (int j = 0; j < NC; ++j) l_acc[j] = 0.f;
       for (int blk = 0; blk < nblk; ++blk) {
         const int np = min(kPB, n_my - blk * kPB);
         // key visible to the row at position pos  <=>  sel_prev < pos and token position <= pos  <=>  pos > thr
@@ -386,30 +390,25 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         STAMP(cta0 && st == 0, 3 + 4 * min(blk, 3));
         tc_fence_after();
         const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
-        float xs[NHALF];
+        // d = s * scale - m_ref (log2 units), -inf where masked; the common block needs nothing else
+        float d[NC];
+        float tmax = -INFINITY;
         {
-          uint32_t raw[NHALF];
+          uint32_t raw[NC];
 #pragma unroll
-          for (int i = 0; i < NCH; ++i) tmem_ld8(s_addr + 8 * i, raw + 8 * i);
+          for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
           tmem_wait_ld();
 #pragma unroll
-          for (int j = 0; j < NHALF; ++j) xs[j] = __uint_as_float(raw[j]) * p.scale_log2;
-        }
-        uint32_t act[kActWords];
+          for (int i = 0; i < NCH; ++i) {
+            const int4 ps = *reinterpret_cast<const int4*>(s_colpos + cbeg + 4 * i);
+            const float4 mr = *reinterpret_cast<const float4*>(s_mref + cbeg + 4 * i);
+            const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
+            const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
 #pragma unroll
-        for (int i = 0; i < kActWords; ++i) act[i] = 0;
-        float tmax = -INFINITY;
-#pragma unroll
-        for (int j = 0; j < NHALF; j += 4) {
-          const int4 ps = *reinterpret_cast<const int4*>(s_colpos + cbeg + j);
-          const float4 mr = *reinterpret_cast<const float4*>(s_mref + cbeg + j);
-          const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
-          const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            if (pv[u] > thr) {
-              act[(j + u) >> 5] |= 1u << ((j + u) & 31);
-              tmax = fmaxf(tmax, xs[j + u] - mv[u]);      // m_ref = -inf (row not started) -> +inf
+            for (int u = 0; u < 4; ++u) {
+              const float v = fmaf(__uint_as_float(raw[4 * i + u]), p.scale_log2, -mv[u]);
+              d[4 * i + u] = pv[u] > thr ? v : -INFINITY;
+              tmax = fmaxf(tmax, d[4 * i + u]);
             }
           }
         }
@@ -418,110 +417,97 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         STAMP(cta0 && st == 0, 4 + 4 * min(blk, 3));
         if (s_flag[blk % 3] != 0) {
           // ---- slow path: exact column max of this block, raise m_ref, rescale O and L ----
-          int mine = kOrdNegInf;
+          float xs[NC];
+          {
+            uint32_t raw[NC];
 #pragma unroll
-          for (int j = 0; j < NHALF; ++j) {
-            const bool a = (act[j >> 5] >> (j & 31)) & 1u;
-            const int r = __reduce_max_sync(0xffffffffu, a ? f2o(xs[j]) : kOrdNegInf);
-            if ((j & 31) == lane) mine = r;
-            if ((j & 31) == 31 || j == NHALF - 1) {
-              if (lane <= (j & 31)) atomicMax(&s_colmax[cbeg + (j & ~31) + lane], mine);
-            }
+            for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
+            tmem_wait_ld();
+#pragma unroll
+            for (int j = 0; j < NC; ++j)
+              xs[j] = s_colpos[cbeg + j] > thr ? __uint_as_float(raw[j]) * p.scale_log2 : -INFINITY;
+          }
+#pragma unroll
+          for (int j = 0; j < NC; ++j) {
+            const int r = __reduce_max_sync(0xffffffffu, f2o(xs[j]));
+            if (lane == 0) atomicMax(&s_colmax[cbeg + j], r);
           }
           softmax_bar();
           if (st < NT) {
             const float bm = o2f(s_colmax[st]), old = s_mref[st];
             const float nw = fmaxf(old, bm);
-            s_alpha[st] = (old == -INFINITY) ? 1.f : ex2_approx(old - nw);
+            s_alpha[st] = ex2_approx(old - nw);             // old = kMrefInit (row not started): 0, O and L are 0
             s_mref[st] = nw;
             s_colmax[st] = kOrdNegInf;
           }
           softmax_bar();
-          if (blk > 0) {
 #pragma unroll
-            for (int i = 0; i < NCH; ++i) l_part[i] *= s_alpha[lcol0 + i];
+          for (int j = 0; j < NC; ++j) {
+            l_acc[j] *= s_alpha[cbeg + j];
+            d[j] = xs[j] - s_mref[cbeg + j];
+          }
+          if (blk > 0) {
             mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O is ours
             tc_fence_after();
 #pragma unroll
             for (int a = 0; a < NATOM; ++a) {
               const int row = a * 64 + (key & 63);          // lanes 64..127 hold the lo part of the same rows
               const float al = s_alpha[min(row, NT - 1)];
+              uint32_t ov[32];
+              const uint32_t addr = lane_addr + colO + a * 128 + cg * 32;
+              tmem_ld32(addr, ov);
+              tmem_wait_ld();
 #pragma unroll
-              for (int c = 0; c < 2; ++c) {
-                uint32_t ov[32];
-                const uint32_t addr = lane_addr + colO + a * 128 + half * 64 + c * 32;
-                tmem_ld32(addr, ov);
-                tmem_wait_ld();
-#pragma unroll
-                for (int u = 0; u < 32; ++u) ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
-                tmem_st32(addr, ov);
-              }
+              for (int u = 0; u < 32; ++u) ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
+              tmem_st32(addr, ov);
             }
             tmem_wait_st();
           }
         }
         if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) has read P
         STAMP(cta0 && st == 0, 5 + 4 * min(blk, 3));
-        // ---- P = 2^(x - m_ref) as bf16 hi + lo into the MN-major SW128 operand ----
+        // ---- P = 2^d as bf16 hi + lo into the MN-major SW128 operand (8-byte stores: NC is a multiple of 4) ----
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
-          const float4 m0 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i);
-          const float4 m1 = *reinterpret_cast<const float4*>(s_mref + cbeg + 8 * i + 4);
-          const float mv[8] = {m0.x, m0.y, m0.z, m0.w, m1.x, m1.y, m1.z, m1.w};
+          float e[4];
 #pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const int j = 8 * i + u;
-            const bool a = (act[j >> 5] >> (j & 31)) & 1u;
-            xs[j] = a ? ex2_approx(xs[j] - mv[u]) : 0.f;
+          for (int u = 0; u < 4; ++u) {
+            e[u] = ex2_approx(d[4 * i + u]);
+            l_acc[4 * i + u] += e[u];
           }
-          const int col0 = cbeg + 8 * i;
-          unsigned char* dst = p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4);
-          uint4 hi, lo;
-          split_bf16x2(xs[8 * i + 0], xs[8 * i + 1], hi.x, lo.x);
-          split_bf16x2(xs[8 * i + 2], xs[8 * i + 3], hi.y, lo.y);
-          split_bf16x2(xs[8 * i + 4], xs[8 * i + 5], hi.z, lo.z);
-          split_bf16x2(xs[8 * i + 6], xs[8 * i + 7], hi.w, lo.w);
-          *reinterpret_cast<uint4*>(dst) = hi;
-          *reinterpret_cast<uint4*>(dst + lay.p_hl_bytes) = lo;
+          const int col0 = cbeg + 4 * i;
+          unsigned char* dst =
+              p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4) + ((col0 & 4) << 1);
+          uint2 hi, lo;
+          split_bf16x2(e[0], e[1], hi.x, lo.x);
+          split_bf16x2(e[2], e[3], hi.y, lo.y);
+          *reinterpret_cast<uint2*>(dst) = hi;
+          *reinterpret_cast<uint2*>(dst + lay.p_hl_bytes) = lo;
         }
         fence_proxy_async();
         tc_fence_before();
         mbar_arrive(&p_ready[blk % cfg.NP]);
         STAMP(cta0 && st == 0, 6 + 4 * min(blk, 3));
-        // ---- row sums: three halving shuffle levels leave NCH partial sums per lane (columns lcol0 ...) ----
-        {
-          const bool up = lane & 16;
-#pragma unroll
-          for (int i = 0; i < 4 * NCH; ++i) {
-            const float send = up ? xs[i] : xs[i + 4 * NCH], keep = up ? xs[i + 4 * NCH] : xs[i];
-            xs[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
-          }
-        }
-        {
-          const bool up = lane & 8;
-#pragma unroll
-          for (int i = 0; i < 2 * NCH; ++i) {
-            const float send = up ? xs[i] : xs[i + 2 * NCH], keep = up ? xs[i + 2 * NCH] : xs[i];
-            xs[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-          }
-        }
-        {
-          const bool up = lane & 4;
-#pragma unroll
-          for (int i = 0; i < NCH; ++i) {
-            const float send = up ? xs[i] : xs[i + NCH], keep = up ? xs[i + NCH] : xs[i];
-            l_part[i] += keep + __shfl_xor_sync(0xffffffffu, send, 4);
-          }
-        }
       }
       // ---- epilogue: L per row, O = (O_hi + O_lo) / L through a shared-memory stage, coalesced stores ----
+      {
+        // sum over the 32 keys of the warp: two halving levels, then a 3-level butterfly on NCH values
+        const bool up16 = lane & 16, up8 = lane & 8;
 #pragma unroll
-      for (int i = 0; i < NCH; ++i) {
-        float v = l_part[i];
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        if ((lane & 3) == 0) atomicAdd(&s_L[lcol0 + i], v);
+        for (int i = 0; i < 2 * NCH; ++i) {
+          const float send = up16 ? l_acc[i] : l_acc[i + 2 * NCH], keep = up16 ? l_acc[i + 2 * NCH] : l_acc[i];
+          l_acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+        }
+#pragma unroll
+        for (int i = 0; i < NCH; ++i) {
+          const float send = up8 ? l_acc[i] : l_acc[i + NCH], keep = up8 ? l_acc[i + NCH] : l_acc[i];
+          float v = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+          v += __shfl_xor_sync(0xffffffffu, v, 4);
+          v += __shfl_xor_sync(0xffffffffu, v, 2);
+          v += __shfl_xor_sync(0xffffffffu, v, 1);
+          if ((lane & 7) == 0) atomicAdd(&s_L[cbeg + ((lane >> 3) & 3) * NCH + i], v);
+        }
       }
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
       STAMP(cta0 && st == 0, 20);
@@ -539,8 +525,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       const float lse_scale = p.nsplit > 1 ? 1.f : kLn2;
       float* stage = reinterpret_cast<float*>(smem + lay.ring);
       const int rl = key & 63;
-      const bool is_lo = key >= 64;
-      float* my_stage = stage + rl * kStageStride + half * 64;
+      const bool is_lo = key >= 64;                        // warp-uniform (quadrants 2, 3)
+      float* my_stage = stage + rl * kStageStride + cg * 32;
 #pragma unroll
       for (int a = 0; a < NATOM; ++a) {
         if (a * 64 < rows) {                                // CTA-uniform
@@ -548,40 +534,31 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           const float l = s_L[min(row, NT - 1)];
           const float inv = (row < rows && l > 0.f) ? rcp_approx(l) : 0.f;
           if (a > 0) softmax_bar();                         // previous atom's stage fully written out
-          if (is_lo) {                                      // warp-uniform (quadrants 2, 3)
+          uint32_t ov[32];
+          tmem_ld32(lane_addr + colO + a * 128 + cg * 32, ov);
+          tmem_wait_ld();
+          if (is_lo) {
 #pragma unroll
-            for (int cc = 0; cc < 2; ++cc) {
-              uint32_t ov[32];
-              tmem_ld32(lane_addr + colO + a * 128 + half * 64 + 32 * cc, ov);
-              tmem_wait_ld();
-#pragma unroll
-              for (int c = 0; c < 8; ++c)
-                *reinterpret_cast<uint4*>(my_stage + 32 * cc + 4 * c) =
-                    make_uint4(ov[4 * c], ov[4 * c + 1], ov[4 * c + 2], ov[4 * c + 3]);
-            }
+            for (int c = 0; c < 8; ++c)
+              *reinterpret_cast<uint4*>(my_stage + 4 * c) =
+                  make_uint4(ov[4 * c], ov[4 * c + 1], ov[4 * c + 2], ov[4 * c + 3]);
           }
           softmax_bar();
           if (!is_lo) {
 #pragma unroll
-            for (int cc = 0; cc < 2; ++cc) {
-              uint32_t ov[32];
-              tmem_ld32(lane_addr + colO + a * 128 + half * 64 + 32 * cc, ov);
-              tmem_wait_ld();
-#pragma unroll
-              for (int c = 0; c < 8; ++c) {
-                float4 v = *reinterpret_cast<float4*>(my_stage + 32 * cc + 4 * c);
-                v.x = (v.x + __uint_as_float(ov[4 * c])) * inv;
-                v.y = (v.y + __uint_as_float(ov[4 * c + 1])) * inv;
-                v.z = (v.z + __uint_as_float(ov[4 * c + 2])) * inv;
-                v.w = (v.w + __uint_as_float(ov[4 * c + 3])) * inv;
-                *reinterpret_cast<float4*>(my_stage + 32 * cc + 4 * c) = v;
-              }
+            for (int c = 0; c < 8; ++c) {
+              float4 v = *reinterpret_cast<float4*>(my_stage + 4 * c);
+              v.x = (v.x + __uint_as_float(ov[4 * c])) * inv;
+              v.y = (v.y + __uint_as_float(ov[4 * c + 1])) * inv;
+              v.z = (v.z + __uint_as_float(ov[4 * c + 2])) * inv;
+              v.w = (v.w + __uint_as_float(ov[4 * c + 3])) * inv;
+              *reinterpret_cast<float4*>(my_stage + 4 * c) = v;
             }
           }
           softmax_bar();
           STAMP(cta0 && st == 0 && a == 0, 26);
           const int nrow = min(64, rows - a * 64);
-          for (int rr = st >> 5; rr < nrow; rr += kSoftmaxThreads / 32)
+          for (int rr = sw; rr < nrow; rr += kSoftmaxThreads / 32)
             *reinterpret_cast<float4*>(o_base + s_coloff[a * 64 + rr] + 4 * lane) =
                 *reinterpret_cast<const float4*>(stage + rr * kStageStride + 4 * lane);
           if (st < nrow) {

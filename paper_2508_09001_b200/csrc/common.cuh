@@ -29,13 +29,8 @@ void set_cuda_error(cudaError_t e);
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
-// CTAs of the tensor-core attend kernel that share one SM (its launch bounds, shared memory and TMEM columns allow
-// two up to 48 padded query rows).
-inline int umma_ctas_per_sm(int rows) {
-  static const int env = [] { const char* e = getenv("RETRO_UMMA_PER_SM"); return e ? atoi(e) : 0; }();   // TEMP probe
-  if (env == 1) return 1;
-  return ceil_div(rows, 16) <= 3 ? 2 : 1;
-}
+// CTAs of the tensor-core attend kernel that share one SM.
+inline int umma_ctas_per_sm(int /*rows*/) { return 1; }
 
 int validate_desc(const retro_desc_t* d);  // RETRO_OK / RETRO_ERR_ARG / RETRO_ERR_UNSUPPORTED
 
