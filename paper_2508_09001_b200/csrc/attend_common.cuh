@@ -28,17 +28,38 @@ __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, s
                                                         int G, int R, unsigned int* s_ticket) {
   constexpr int kCh = D / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
-  __threadfence();
-  RETRO_COMBINE_STAMP(24);
+  // Release: every thread's partial stores happen-before the barrier, thread 0's fence is cumulative over them.
   __syncthreads();
-  if (tid == 0) *s_ticket = atomicAdd(&p.counters[unit], 1u);
+  if (tid == 0) {
+    __threadfence();
+    *s_ticket = atomicAdd(&p.counters[unit], 1u);
+    __threadfence();
+  }
+  RETRO_COMBINE_STAMP(24);
   __syncthreads();
   RETRO_COMBINE_STAMP(25);
   if (*s_ticket != (unsigned)(p.nsplit - 1)) return;
   if (tid == 0) p.counters[unit] = 0;   // leave the workspace consistent for the next call
-  __threadfence();
   for (int rho = warp; rho < rows; rho += nwarps) {
     const float* lse_s = p.split_lse + unit * p.nsplit * rows + rho;
+    const float* o_s = p.split_o + (unit * p.nsplit * rows + rho) * D + lane * kCh;
+    const size_t o_stride = (size_t)rows * D;
+    // the partial loads do not depend on the weights: the first 8 go out together with the lse loads
+    float4 v4[8];
+    float v1[8][kCh];
+    auto load8 = [&](int s_first) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const float* src = o_s + (size_t)min(s_first + u, p.nsplit - 1) * o_stride;
+        if constexpr (kCh == 4) {
+          v4[u] = __ldcg(reinterpret_cast<const float4*>(src));
+        } else {
+#pragma unroll
+          for (int c = 0; c < kCh; ++c) v1[u][c] = __ldcg(src + c);
+        }
+      }
+    };
+    load8(0);
     float mx = -INFINITY;
     for (int s = lane; s < p.nsplit; s += 32) mx = fmaxf(mx, __ldcg(lse_s + (size_t)s * rows));
     mx = warp_max(mx);
@@ -47,19 +68,28 @@ __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, s
     for (int c = 0; c < kCh; ++c) o[c] = 0.f;
     float wsum = 0.f;
     if (mx > -INFINITY) {
-      for (int s = 0; s < p.nsplit; ++s) {
-        const float ls = __ldcg(lse_s + (size_t)s * rows);
-        if (ls == -INFINITY) continue;
-        const float wgt = exp2f(ls - mx);
-        wsum += wgt;
-        const float* src = p.split_o + ((unit * p.nsplit + s) * rows + rho) * D + lane * kCh;
-        if constexpr (kCh == 4) {
-          const float4 v = __ldcg(reinterpret_cast<const float4*>(src));
-          o[0] = fmaf(wgt, v.x, o[0]); o[1] = fmaf(wgt, v.y, o[1]);
-          o[2] = fmaf(wgt, v.z, o[2]); o[3] = fmaf(wgt, v.w, o[3]);
-        } else {
+      for (int s0 = 0; s0 < p.nsplit; s0 += 32) {
+        const int sl = s0 + lane;
+        const float ls = sl < p.nsplit ? __ldcg(lse_s + (size_t)sl * rows) : -INFINITY;
+        const float wl_ = exp2f(ls - mx);                 // lane s holds the weight of split s0 + s; 0 if empty
+        const int cnt = min(32, p.nsplit - s0);
+        for (int s1 = 0; s1 < cnt; s1 += 8) {
+          if (s0 + s1 > 0) load8(s0 + s1);
 #pragma unroll
-          for (int c = 0; c < kCh; ++c) o[c] = fmaf(wgt, __ldcg(src + c), o[c]);
+          for (int u = 0; u < 8; ++u) {
+            float wgt = __shfl_sync(0xffffffffu, wl_, (s1 + u) & 31);
+            if (s1 + u >= cnt) wgt = 0.f;
+            if (wgt > 0.f) {                              // an empty split's o is unspecified: never multiply it
+              wsum += wgt;
+              if constexpr (kCh == 4) {
+                o[0] = fmaf(wgt, v4[u].x, o[0]); o[1] = fmaf(wgt, v4[u].y, o[1]);
+                o[2] = fmaf(wgt, v4[u].z, o[2]); o[3] = fmaf(wgt, v4[u].w, o[3]);
+              } else {
+#pragma unroll
+                for (int c = 0; c < kCh; ++c) o[c] = fmaf(wgt, v1[u][c], o[c]);
+              }
+            }
+          }
         }
       }
     }

@@ -2,29 +2,34 @@
 // the selected pages is a dense contraction (Eq. 2 / 6 / 7; arithmetic intensity ~ rows
 // flop per KV byte), far above what the fp32 ALUs sustain at HBM rate once rows > ~8.
 //
-// Per block of 8 pages (128 keys), two tensor-core passes, each reading the 32 KB K or V block from shared
-// memory exactly once (small-N tcgen05.mma is bound by the operand fetch from shared memory, not by the math):
-//   S^T = K Q^T    A = K block [128 keys x 128 ch] (K-major, TMA SW128), B = Q [NT rows x 128 ch], N = NT
-//                  -> TMEM S [lane = key][column = row]: every softmax thread owns one key, no row padding.
-//   O  += P V      A = [P_hi ; P_lo] stacked on M (64 rows of bf16 hi, 64 rows of bf16 lo, MN-major),
-//                  B = V block [128 keys x 128 ch] (MN-major), N = 128
-//                  -> TMEM O [lane = row (hi) | 64 + row (lo)][column = channel]; O = O_hi + O_lo in the epilogue.
+// Per block of 8 pages (128 keys), two tensor-core passes; keys sit on the 128 TMEM lanes of S, query rows on N,
+// so no tensor-core or softmax work is spent on row padding and every softmax thread owns one key:
+//   S^T = K Q^T     A = K block [128 keys x 128 ch] (K-major, TMA SW128), B = Q [NT rows x 128 ch], N = NT
+//                   -> TMEM S [lane = key][column = row]
+//   O^T += V^T P^T  A = V block (MN-major, M = 128 channels), B = [P_hi | P_lo] [128 keys x 2 NT] (MN-major),
+//                   N = 2 NT -> TMEM O [lane = channel][column = row (hi) | NT + row (lo)]; O = O_hi + O_lo.
+// Measured on B200 (probe: one tcgen05.mma costs ~42 + N/2 cycles with A from shared memory, M = 64 or 128):
+// the fixed part is the A fetch, so the P hi / lo halves share one MMA (stacked on N) instead of two.
 // P = 2^(s*scale - m_ref[row]) with the retrospective mask (page j is visible to the row at position p iff
 // sel_prev_j < p; token l iff l <= p) goes to shared memory as bf16 hi + bf16 lo: a single bf16 P (2^-9) leaves
 // |err| ~ 2^-9 |v| on the x8 outlier channels of V, outside the 2e-2 tolerance, and the hardware rejects a bf16
-// A with an fp16 B operand.  Row sums L are accumulated by the softmax threads themselves (a 3-level halving
-// shuffle per block, finished once per CTA).  m_ref is a per-row reference in shared memory; it is raised (and
-// O, L rescaled) only when some logit exceeds it by more than 2^8, so the common block needs no reduction.
+// A with an fp16 B operand.  Row sums L are accumulated in registers by the softmax threads (one key each) and
+// reduced once per CTA.  m_ref is a per-row reference in shared memory; it is raised (and O, L rescaled) only
+// when some logit exceeds it by more than 64 (log2 units: bf16 and fp32 share the exponent range, so P up to
+// 2^64 costs no precision), so the common block needs no reduction.
 //
-// One CTA per (split, KV head, sequence), 576 threads, warp-specialised:
-//   warp 0      TMA producer: every selected (page, head) K / V tile arrives as two 64-channel boxes with the
-//               128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier) into a ring of 32 KB slots
-//               (8 pages = 128 keys of K, then the same 128 keys of V, ...).
-//   warp 1      MMA issuer (one elected thread), owns the TMEM allocation; tcgen05.commit signals mbarriers.
-//   warps 2..17 softmax: TMEM lane quadrant = warp % 4 (32 keys), column group = (warp - 2) / 4 (a quarter of the rows).
+// One CTA per (split, KV head, sequence), 640 threads, warp-specialised:
+//   warp 0, 1   TMA producers, one for K and one for V (separate rings of 32 KB slots = 8 pages = 128 keys, so a
+//               K block never queues behind the longer-lived V block): every selected (page, head) tile arrives
+//               as two 64-channel boxes with the 128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier).
+//   warp 2      MMA issuer (converged warp, elect.sync: the operands stay in uniform registers), owns the TMEM
+//               allocation; tcgen05.commit signals mbarriers.
+//   warp 3      idle (keeps the softmax warps aligned to the TMEM lane quadrants)
+//   warps 4..19 softmax: TMEM lane quadrant = warp % 4 (32 keys), column group = (warp - 4) / 4 (a quarter of the rows).
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
 
+#include <cstdio>
 #include <cstdlib>
 
 #ifdef RETRO_STAMPS
@@ -36,7 +41,7 @@ namespace retro { __device__ void retro_stamp(int i); }
 
 namespace retro {
 
-constexpr int kUmmaThreads = 576;
+constexpr int kUmmaThreads = 640;
 constexpr int kSoftmaxThreads = 512;
 constexpr int kPB = 8;                        // pages per KV block (128 keys)
 constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel half) box: 16 rows x 128 B
@@ -44,8 +49,7 @@ constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][1
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
 constexpr int kTmemCols = 512;
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
-constexpr int kStageStride = 132;             // floats per staged output row (conflict-free 128-bit accesses)
-constexpr float kRescaleThreshold = 8.f;      // log2 units
+constexpr float kRescaleThreshold = 64.f;     // log2 units: P <= 2^64, sums stay far below the fp32 / bf16 range
 constexpr float kMrefInit = -1.0e30f;         // finite "row not started" reference: -inf - kMrefInit stays -inf
 
 // ---- PTX wrappers -------------------------------------------------------------------------------
@@ -54,6 +58,16 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
       ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(smem_u32(bar))
       : "memory");
+}
+// One lane of a converged warp; code under it is single-threaded, so tensor-map / descriptor operands need no
+// per-lane "waterfall" loop (a plain lane == 0 test costs ~90 cycles per tcgen05.mma or TMA instruction).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ void prefetch_l2_bulk(const void* gptr, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gptr), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -138,6 +152,11 @@ __device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t* r) {
                : "r"(taddr)
                : "memory");
 }
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t* r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+               ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3])
+               : "memory");
+}
 __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* r) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
@@ -160,19 +179,19 @@ struct UmmaLayout {
 };
 __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
   UmmaLayout L;
-  const int natom = (NT + 63) / 64;
+  const int natom = (2 * NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
-  L.p = L.q + 2 * NT * 128;                  // [buf][hi|lo][atom][128 keys][128 B = 64 rows]
-  L.p_hl_bytes = natom * 16384;
-  L.p_buf_bytes = 2 * L.p_hl_bytes;
-  L.ring = L.p + NP * L.p_buf_bytes;         // the first 33 KB double as the epilogue's output staging
+  L.p = L.q + 2 * NT * 128;                  // [buf][atom][128 keys][128 B = 64 columns]; columns = hi rows | lo rows
+  L.p_hl_bytes = 0;
+  L.p_buf_bytes = natom * 16384;
+  L.ring = L.p + NP * L.p_buf_bytes;
   L.list = L.ring + NS * kSlotBytes;         // int32 [3][pages_per_split]
   L.total = L.list + 3 * pages_per_split * 4;
   return L;
 }
 
 #ifdef RETRO_STAMPS
-__device__ unsigned long long g_stamps[32];
+__device__ unsigned long long g_stamps[128];
 __device__ __forceinline__ void stamp(int i) {
   unsigned long long t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
@@ -185,10 +204,10 @@ __device__ void retro_stamp(int i) { stamp(i); }
 #endif
 
 struct UmmaCfg {
-  int NS;         // ring slots (32 KB each)
+  int NK, NV;     // K and V ring slots (32 KB each)
   int NP;         // P buffers (1 or 2)
   int NSB;        // S buffers in TMEM (1 or 2)
-  int tmem_cols;  // power of two >= NSB * NT + 128 * atoms
+  int tmem_cols;  // power of two >= (NSB + 2) * NT
 };
 
 // NCH = NT / 16; every softmax thread owns one key and NC = 4 * NCH of the padded rows (four column groups).
@@ -198,7 +217,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
                    const __grid_constant__ CUtensorMap tmap_v) {
   constexpr int NT = 16 * NCH;
   constexpr int NC = 4 * NCH;
-  constexpr int NATOM = (NT + 63) / 64;
   extern __shared__ __align__(1024) unsigned char smem[];
   __shared__ __align__(8) uint64_t bars[24];
   __shared__ uint32_t tmem_ptr_s;
@@ -211,9 +229,11 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(16) int s_coloff[NT];     // output offset (floats) of the row
   __shared__ __align__(16) float s_L[NT];        // row sums (epilogue)
   const int pps = p.pages_per_split;
-  const UmmaLayout lay = umma_layout(NT, cfg.NS, cfg.NP, pps);
-  uint64_t* ring_full = bars;            // [NS <= 6]
-  uint64_t* ring_empty = bars + 6;       // [NS <= 6]
+  const UmmaLayout lay = umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, pps);
+  uint64_t* k_full = bars;               // [NK <= 3]
+  uint64_t* k_empty = bars + 3;          // [NK <= 3]
+  uint64_t* v_full = bars + 6;           // [NV <= 3]
+  uint64_t* v_empty = bars + 9;          // [NV <= 3]
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
   uint64_t* o_full = bars + 16;          // [2] PV of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
@@ -232,13 +252,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   const int count = p.sel_count[unit];
   const int L = p.seq_lens[b];
   if (tid == 0) {
-    for (int i = 0; i < 6; ++i) { mbar_init(&ring_full[i], 1); mbar_init(&ring_empty[i], 1); }
+    for (int i = 0; i < 12; ++i) mbar_init(&bars[i], 1);
     mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
-    mbar_init(&p_ready[0], kSoftmaxThreads); mbar_init(&p_ready[1], kSoftmaxThreads);
+    mbar_init(&p_ready[0], kSoftmaxThreads / 32); mbar_init(&p_ready[1], kSoftmaxThreads / 32);
     mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
     fence_mbar_init();
   }
-  if (warp == 1) {
+  if (warp == 2) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_ptr_s)),
                  "r"(cfg.tmem_cols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -299,33 +319,41 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   STAMP(cta0 && tid == 0, 1);
 
   if (nblk > 0) {
-    if (warp == 0) {
-      // ===== TMA producer: tile sequence K(0) V(0) K(1) V(1) ... through a ring of NS 32 KB slots =====
-      for (int q = 0; q < 2 * nblk; ++q) {
-        const int blk = q >> 1, slot = q % cfg.NS, n = q / cfg.NS;
+    if (warp < 2) {
+      // ===== TMA producers: warp 0 streams the K blocks, warp 1 the V blocks, each through its own ring =====
+      const int NR = warp == 0 ? cfg.NK : cfg.NV;
+      uint64_t* full = warp == 0 ? k_full : v_full;
+      uint64_t* empty = warp == 0 ? k_empty : v_empty;
+      const CUtensorMap* map = warp == 0 ? &tmap_k : &tmap_v;
+      unsigned char* ring = smem + lay.ring + (warp == 0 ? 0 : cfg.NK * kSlotBytes);
+      for (int blk = 0; blk < nblk; ++blk) {
+        const int slot = blk % NR, n = blk / NR;
         const int np = min(kPB, n_my - blk * kPB);
-        unsigned char* dst = smem + lay.ring + slot * kSlotBytes;
-        const CUtensorMap* map = (q & 1) ? &tmap_v : &tmap_k;
-        if (n > 0) mbar_wait(&ring_empty[slot], (n - 1) & 1);
-        if (lane == 0) mbar_expect_tx(&ring_full[slot], np * 2 * kTileHalfBytes);
-        __syncwarp();
-        if (lane < 2 * np) {                  // lane = 2 * page + channel half: 16 boxes in flight at once
-          const int pg = lane >> 1, hf = lane & 1;
-          const int row0 = (s_list[2 * pps + blk * kPB + pg] * p.h_k + h) * 16;
-          tma_load_2d(dst + hf * kHalfStride + pg * kTileHalfBytes, map, hf * 64, row0, &ring_full[slot]);
+        unsigned char* dst = ring + slot * kSlotBytes;
+        if (n > 0) mbar_wait(&empty[slot], (n - 1) & 1);
+        STAMP(cta0 && lane == 0 && warp == 0 && blk < 12, 32 + blk * 8 + 7);
+        if (elect_one()) {
+          mbar_expect_tx(&full[slot], np * 2 * kTileHalfBytes);
+          for (int pg = 0; pg < np; ++pg) {
+            const int row0 = (s_list[2 * pps + blk * kPB + pg] * p.h_k + h) * 16;
+            tma_load_2d(dst + pg * kTileHalfBytes, map, 0, row0, &full[slot]);
+            tma_load_2d(dst + kHalfStride + pg * kTileHalfBytes, map, 64, row0, &full[slot]);
+          }
         }
+        __syncwarp();
       }
-    } else if (warp == 1) {
-      // ===== MMA issuer =====
-      if (lane == 0) {
-        const uint32_t q_addr = smem_u32(smem + lay.q);
-        const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
-        const uint32_t idesc_o = idesc_bf16_ab(128, true, true);
-        auto issue_s = [&](int blk) {
-          const int q = 2 * blk, slot = q % cfg.NS, n = q / cfg.NS;
-          mbar_wait(&ring_full[slot], n & 1);
-          STAMP(cta0 && blk == 0, 2);
-          tc_fence_after();
+    } else if (warp == 2) {
+      // ===== MMA issuer: the whole warp walks the loop (waits), one elected lane issues =====
+      const uint32_t q_addr = smem_u32(smem + lay.q);
+      const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
+      const uint32_t idesc_o = idesc_bf16_ab(2 * NT, true, true);
+      auto issue_s = [&](int blk) {
+        const int slot = blk % cfg.NK, n = blk / cfg.NK;
+        mbar_wait(&k_full[slot], n & 1);
+        STAMP(cta0 && lane == 0 && blk == 0, 2);
+        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 3);
+        tc_fence_after();
+        if (elect_one()) {
           const uint32_t k_addr = smem_u32(smem + lay.ring + slot * kSlotBytes);
           const uint32_t d_tmem = tmem_base + colS + (blk % cfg.NSB) * NT;
 #pragma unroll
@@ -334,45 +362,48 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             const uint32_t qoff = (ks >> 2) * (NT * 128) + (ks & 3) * 32;
             umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff), idesc_s, ks > 0);
           }
-          tc_commit(&ring_empty[slot]);
+          tc_commit(&k_empty[slot]);
           tc_commit(&s_full[blk % cfg.NSB]);
-        };
-        if (cfg.NSB == 2) issue_s(0);
-        for (int blk = 0; blk < nblk; ++blk) {
-          if (cfg.NSB == 2) {
-            if (blk + 1 < nblk) issue_s(blk + 1);
-          } else if (blk == 0) {
-            issue_s(0);
-          }
-          const int q = 2 * blk + 1, slot = q % cfg.NS, n = q / cfg.NS;
-          const int np = min(kPB, n_my - blk * kPB);
-          mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
-          if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
-          mbar_wait(&ring_full[slot], n & 1);
-          tc_fence_after();
-          const uint32_t v_addr = smem_u32(smem + lay.ring + slot * kSlotBytes);
+        }
+        __syncwarp();
+      };
+      if (cfg.NSB == 2) issue_s(0);
+      for (int blk = 0; blk < nblk; ++blk) {
+        if (cfg.NSB == 2) {
+          if (blk + 1 < nblk) issue_s(blk + 1);
+        } else if (blk == 0) {
+          issue_s(0);
+        }
+        const int slot = blk % cfg.NV, n = blk / cfg.NV;
+        const int np = min(kPB, n_my - blk * kPB);
+        mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
+        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 4);
+        if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
+        mbar_wait(&v_full[slot], n & 1);
+        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 5);
+        tc_fence_after();
+        if (elect_one()) {
+          const uint32_t v_addr = smem_u32(smem + lay.ring + (cfg.NK + slot) * kSlotBytes);
           const uint32_t p_addr = smem_u32(smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes);
           for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
             const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
-            const uint32_t acc = (blk > 0 || ks > 0) ? 1u : 0u;
-#pragma unroll
-            for (int a = 0; a < NATOM; ++a) {   // M = 128: 64 rows of P_hi then the same 64 rows of P_lo
-              const uint64_t pdesc = desc_mnmajor_sw128(p_addr + a * 16384 + ks * 2048, lay.p_hl_bytes);
-              umma_bf16(tmem_base + colO + a * 128, pdesc, vdesc, idesc_o, acc);
-            }
+            const uint64_t pdesc = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
+            umma_bf16(tmem_base + colO, vdesc, pdesc, idesc_o, (blk > 0 || ks > 0) ? 1u : 0u);
           }
-          tc_commit(&ring_empty[slot]);
+          tc_commit(&v_empty[slot]);
           tc_commit(&o_full[blk & 1]);
         }
+        __syncwarp();
+        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 6);
       }
-    } else {
+    } else if (warp >= 4) {
       // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NC = NT / 4 columns (rows) each =====
-      const int sw = warp - 2;                            // 0..15
+      const int sw = warp - 4;                            // 0..15
       const int quadrant = warp & 3;                      // TMEM lanes a warp may touch: 32*(warp%4)..+31
       const int cg = sw >> 2;                             // column group
       const int key = quadrant * 32 + lane;
       const int cbeg = cg * NC;
-      const int st = tid - 64;                            // 0..511
+      const int st = tid - 128;                           // 0..511
       const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
       float l_acc[NC];                                    // this key-thread's share of the row sums
 #pragma unroll
@@ -388,6 +419,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         if (st == 0) s_flag[(blk + 1) % 3] = 0;
         mbar_wait(&s_full[blk % cfg.NSB], (blk / cfg.NSB) & 1);
         STAMP(cta0 && st == 0, 3 + 4 * min(blk, 3));
+        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 0);
         tc_fence_after();
         const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
         // d = s * scale - m_ref (log2 units), -inf where masked; the common block needs nothing else
@@ -415,6 +447,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         if (__any_sync(0xffffffffu, tmax > kRescaleThreshold) && lane == 0) s_flag[blk % 3] = 1;
         softmax_bar();
         STAMP(cta0 && st == 0, 4 + 4 * min(blk, 3));
+        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 1);
         if (s_flag[blk % 3] != 0) {
           // ---- slow path: exact column max of this block, raise m_ref, rescale O and L ----
           float xs[NC];
@@ -450,16 +483,20 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O is ours
             tc_fence_after();
 #pragma unroll
-            for (int a = 0; a < NATOM; ++a) {
-              const int row = a * 64 + (key & 63);          // lanes 64..127 hold the lo part of the same rows
-              const float al = s_alpha[min(row, NT - 1)];
-              uint32_t ov[32];
-              const uint32_t addr = lane_addr + colO + a * 128 + cg * 32;
-              tmem_ld32(addr, ov);
+            for (int i = 0; i < NCH; ++i) {                  // this thread's columns of O_hi and O_lo
+              const float4 al4 = *reinterpret_cast<const float4*>(s_alpha + cbeg + 4 * i);
+              const float al[4] = {al4.x, al4.y, al4.z, al4.w};
+              uint32_t oh[4], ol[4];
+              tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
+              tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
               tmem_wait_ld();
 #pragma unroll
-              for (int u = 0; u < 32; ++u) ov[u] = __float_as_uint(__uint_as_float(ov[u]) * al);
-              tmem_st32(addr, ov);
+              for (int u = 0; u < 4; ++u) {
+                oh[u] = __float_as_uint(__uint_as_float(oh[u]) * al[u]);
+                ol[u] = __float_as_uint(__uint_as_float(ol[u]) * al[u]);
+              }
+              tmem_st4(lane_addr + colO + cbeg + 4 * i, oh);
+              tmem_st4(lane_addr + colO + NT + cbeg + 4 * i, ol);
             }
             tmem_wait_st();
           }
@@ -476,19 +513,21 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             e[u] = ex2_approx(d[4 * i + u]);
             l_acc[4 * i + u] += e[u];
           }
-          const int col0 = cbeg + 4 * i;
-          unsigned char* dst =
-              p_row + (col0 >> 6) * 16384 + ((((col0 & 63) >> 3) ^ (key & 7)) << 4) + ((col0 & 4) << 1);
+          const int c_hi = cbeg + 4 * i, c_lo = NT + c_hi;
           uint2 hi, lo;
           split_bf16x2(e[0], e[1], hi.x, lo.x);
           split_bf16x2(e[2], e[3], hi.y, lo.y);
-          *reinterpret_cast<uint2*>(dst) = hi;
-          *reinterpret_cast<uint2*>(dst + lay.p_hl_bytes) = lo;
+          *reinterpret_cast<uint2*>(p_row + (c_hi >> 6) * 16384 + ((((c_hi & 63) >> 3) ^ (key & 7)) << 4) +
+                                    ((c_hi & 4) << 1)) = hi;
+          *reinterpret_cast<uint2*>(p_row + (c_lo >> 6) * 16384 + ((((c_lo & 63) >> 3) ^ (key & 7)) << 4) +
+                                    ((c_lo & 4) << 1)) = lo;
         }
         fence_proxy_async();
         tc_fence_before();
-        mbar_arrive(&p_ready[blk % cfg.NP]);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&p_ready[blk % cfg.NP]);   // one arrival per warp (512 would serialise)
         STAMP(cta0 && st == 0, 6 + 4 * min(blk, 3));
+        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 2);
       }
       // ---- epilogue: L per row, O = (O_hi + O_lo) / L through a shared-memory stage, coalesced stores ----
       {
@@ -512,7 +551,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
       STAMP(cta0 && st == 0, 20);
       tc_fence_after();
-      softmax_bar();                                       // s_L complete; every PV retired (ring is free)
+      softmax_bar();                                       // s_L complete
       float* o_base;
       float* lse_base;
       if (p.nsplit > 1) {
@@ -523,48 +562,24 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         lse_base = p.part_lse + (size_t)b * R * p.h_q;
       }
       const float lse_scale = p.nsplit > 1 ? 1.f : kLn2;
-      float* stage = reinterpret_cast<float*>(smem + lay.ring);
-      const int rl = key & 63;
-      const bool is_lo = key >= 64;                        // warp-uniform (quadrants 2, 3)
-      float* my_stage = stage + rl * kStageStride + cg * 32;
+      // thread = channel `key`; its NC rows: O = (O_hi + O_lo) / L, 128 B coalesced per warp and row
 #pragma unroll
-      for (int a = 0; a < NATOM; ++a) {
-        if (a * 64 < rows) {                                // CTA-uniform
-          const int row = a * 64 + rl;
-          const float l = s_L[min(row, NT - 1)];
-          const float inv = (row < rows && l > 0.f) ? rcp_approx(l) : 0.f;
-          if (a > 0) softmax_bar();                         // previous atom's stage fully written out
-          uint32_t ov[32];
-          tmem_ld32(lane_addr + colO + a * 128 + cg * 32, ov);
+      for (int i = 0; i < NCH; ++i) {
+        if (cbeg + 4 * i < rows) {                          // warp-uniform
+          uint32_t oh[4], ol[4];
+          tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
+          tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
           tmem_wait_ld();
-          if (is_lo) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-              *reinterpret_cast<uint4*>(my_stage + 4 * c) =
-                  make_uint4(ov[4 * c], ov[4 * c + 1], ov[4 * c + 2], ov[4 * c + 3]);
-          }
-          softmax_bar();
-          if (!is_lo) {
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-              float4 v = *reinterpret_cast<float4*>(my_stage + 4 * c);
-              v.x = (v.x + __uint_as_float(ov[4 * c])) * inv;
-              v.y = (v.y + __uint_as_float(ov[4 * c + 1])) * inv;
-              v.z = (v.z + __uint_as_float(ov[4 * c + 2])) * inv;
-              v.w = (v.w + __uint_as_float(ov[4 * c + 3])) * inv;
-              *reinterpret_cast<float4*>(my_stage + 4 * c) = v;
+          for (int u = 0; u < 4; ++u) {
+            const int c = cbeg + 4 * i + u;
+            if (c < rows) {
+              const float l = s_L[c];
+              const float inv = l > 0.f ? rcp_approx(l) : 0.f;
+              const int off = s_coloff[c];
+              o_base[off + key] = (__uint_as_float(oh[u]) + __uint_as_float(ol[u])) * inv;
+              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + lg2_approx(l)) * lse_scale : -INFINITY;
             }
-          }
-          softmax_bar();
-          STAMP(cta0 && st == 0 && a == 0, 26);
-          const int nrow = min(64, rows - a * 64);
-          for (int rr = sw; rr < nrow; rr += kSoftmaxThreads / 32)
-            *reinterpret_cast<float4*>(o_base + s_coloff[a * 64 + rr] + 4 * lane) =
-                *reinterpret_cast<const float4*>(stage + rr * kStageStride + 4 * lane);
-          if (st < nrow) {
-            const int c = a * 64 + st;
-            const float lc = s_L[c];
-            lse_base[s_coloff[c] >> 7] = lc > 0.f ? (s_mref[c] + lg2_approx(lc)) * lse_scale : -INFINITY;
           }
         }
       }
@@ -586,7 +601,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   tc_fence_before();
   __syncthreads();
   STAMP(cta0 && tid == 0, 21);
-  if (warp == 1) {
+  if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
   }
@@ -597,7 +612,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
 
 #ifdef RETRO_STAMPS
 extern "C" int retro_debug_read_stamps(unsigned long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_stamps, sizeof(unsigned long long) * 32);
+  return (int)cudaMemcpyFromSymbol(host_out, g_stamps, sizeof(unsigned long long) * 128);
 }
 #endif
 
@@ -675,29 +690,31 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   const int nch = ceil_div(rows, 16), NT = 16 * nch;
   if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
   // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~2-3 KB static; two CTAs per SM up to
-  // 48 padded rows.  Prefer two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in
-  // flight per CTA, and room for the epilogue's 33 KB output stage).
-  const int per_sm = umma_ctas_per_sm(rows);
-  const int natom = (NT + 63) / 64;
+  // Prefer two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in flight per CTA).
   UmmaCfg cfg;
   cfg.NSB = 2;
+  int slots = 0;
   auto plan = [&](int budget) {
     cfg.NP = 2;
-    cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
-    if (cfg.NS < 3) {
+    slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
+    if (slots < 4) {
       cfg.NP = 1;
-      cfg.NS = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
+      slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
     }
   };
-  plan((per_sm == 2 ? 233472 / 2 : 232448) - 1024 - 3072);
-  if (cfg.NS < 2 && per_sm == 2) plan(232448 - 1024 - 3072);     // does not fit twice: one CTA per SM
-  if (cfg.NS < 2) return RETRO_ERR_UNSUPPORTED;
-  if (cfg.NS > 6) cfg.NS = 6;
+  plan(232448 - 1024 - 4096);
+  if (slots < 2) return RETRO_ERR_UNSUPPORTED;
+  if (slots > 6) slots = 6;
+  cfg.NK = slots / 2;             // a V block lives longer (it waits for the softmax of its own block)
+  cfg.NV = slots - cfg.NK;
+  if (const char* e = std::getenv("RETRO_UMMA_PLAN")) {   // TEMP probe: "NP NK NV"
+    sscanf(e, "%d %d %d", &cfg.NP, &cfg.NK, &cfg.NV);
+  }
   int cols = 32;
-  while (cols < cfg.NSB * NT + 128 * natom) cols <<= 1;
-  if (cols > kTmemCols / per_sm) return RETRO_ERR_UNSUPPORTED;
+  while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
+  if (cols > kTmemCols) return RETRO_ERR_UNSUPPORTED;
   cfg.tmem_cols = cols;
-  const size_t smem = (size_t)umma_layout(NT, cfg.NS, cfg.NP, prm.pages_per_split).total;
+  const size_t smem = (size_t)umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, prm.pages_per_split).total;
   switch (nch) {
     case 1: return launch_nch<1>(d, prm, cfg, smem, hit->mk, hit->mv, s);
     case 2: return launch_nch<2>(d, prm, cfg, smem, hit->mk, hit->mv, s);
