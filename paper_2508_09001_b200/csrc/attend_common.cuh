@@ -28,13 +28,9 @@ __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, s
                                                         int G, int R, unsigned int* s_ticket) {
   constexpr int kCh = D / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
-  // Release: every thread's partial stores happen-before the barrier, thread 0's fence is cumulative over them.
+  // Release: every thread's partial stores happen-before the barrier; thread 0's acq_rel ticket is cumulative.
   __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    *s_ticket = atomicAdd(&p.counters[unit], 1u);
-    __threadfence();
-  }
+  if (tid == 0) *s_ticket = ticket_acq_rel(&p.counters[unit]);
   RETRO_COMBINE_STAMP(24);
   __syncthreads();
   RETRO_COMBINE_STAMP(25);

@@ -12,7 +12,7 @@ namespace retro {
 constexpr int kWarp = 32;
 constexpr int kMaxWindow = 32;
 constexpr int kMaxGroup = 8;
-constexpr int kMaxPagesPerSeq = 24576;
+constexpr int kMaxPagesPerSeq = 16384;   // top-k: 256 threads x 64-bit ownership masks; 128 KB of keys
 
 // ---- error plumbing ---------------------------------------------------------------------------
 void set_cuda_error(cudaError_t e);
@@ -129,6 +129,15 @@ __device__ __forceinline__ uint4 ldg_stream(const void* p) {
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
                : "l"(p));
   return r;
+}
+
+// Arrival ticket with release + acquire in one L2 operation.  Used as  bar.sync ; thread 0: ticket ; bar.sync :
+// the CTA's earlier writes are released (cumulativity through the barrier), the last arriver's later reads of
+// other CTAs' data (ld.cg) are acquired.
+__device__ __forceinline__ unsigned int ticket_acq_rel(unsigned int* p) {
+  unsigned int old;
+  asm volatile("atom.add.acq_rel.gpu.global.u32 %0, [%1], 1;" : "=r"(old) : "l"(p) : "memory");
+  return old;
 }
 
 __device__ __forceinline__ float warp_max(float v) {

@@ -7,7 +7,8 @@
 // coalesced 128-bit load per lane per page.  Accumulation is fp64 (products of bf16/fp32 inputs are exact in
 // fp64), so ranking ties against the fp64 oracle only arise within ~1e-12 relative.
 //
-// Top-k: one CTA per (b, KV head).  Order-preserving 64-bit keys of the fp64 scores live in shared memory;
+// Score and top-k run in ONE kernel: every CTA scores 64 pages of one (b, KV head) unit; the last CTA of the unit
+// to finish (arrival counter in the workspace) selects.  Order-preserving 64-bit keys of the fp64 scores live in shared memory;
 // a range-adaptive radix select (2048 buckets over [min,max] of the live range, 11 bits per pass, early exit
 // when the threshold bucket is taken whole) finds the k-th key, then an in-order two-scan compaction emits
 // ascending page indices with ties resolved to the lower index, and the same pass does Alg. 2's
@@ -15,6 +16,18 @@
 #include "common.cuh"
 
 namespace retro {
+
+#ifdef RETRO_STAMPS
+__device__ unsigned long long g_sel_stamps[32];
+__device__ __forceinline__ void sel_stamp(int i) {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
+  g_sel_stamps[i] = t;
+}
+#define SSTAMP(cond, i) do { if (cond) sel_stamp(i); } while (0)
+#else
+#define SSTAMP(cond, i) do { } while (0)
+#endif
 
 constexpr int kScoreWarps = 8;
 constexpr int kPagesPerWarp = 8;
@@ -37,96 +50,9 @@ template <> struct Rec<float> {
 
 // record = [Kmax (D) ; Kmin (D)] = 2*D*sizeof(T) = 512 B: lane l holds elements [l*kVals, (l+1)*kVals) of the
 // concatenated vector, i.e. lanes 0..15 see Kmax channels, lanes 16..31 see Kmin channels.
-template <typename T, int D>
-__global__ void __launch_bounds__(kScoreWarps * 32) page_score_kernel(
-    const T* __restrict__ q_cur, const T* __restrict__ bounds, const int32_t* __restrict__ seq_lens,
-    double* __restrict__ scores, double* __restrict__ scores_out, int h_q, int h_k, int max_pages, int P,
-    int group_reduce) {
-  static_assert(2 * D * sizeof(T) == 512, "digest record must be 512 bytes");
-  constexpr int kVals = Rec<T>::kVals;
-  __shared__ double s_q[kMaxGroup][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
-  const int b = blockIdx.z, h = blockIdx.y;
-  const int G = h_q / h_k;
-  const int n_pages = (seq_lens[b] + P - 1) / P;
-  const int page0 = blockIdx.x * kPagesPerCta;
-  const size_t row = ((size_t)b * h_k + h) * max_pages;
-  if (page0 >= n_pages) {
-    if (scores_out != nullptr)
-      for (int j = page0 + threadIdx.x; j < min(page0 + kPagesPerCta, max_pages); j += blockDim.x)
-        scores_out[row + j] = -INFINITY;
-    return;
-  }
-  // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
-  for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) {
-    const int c = i % D;
-    const bool neg = i >= D;
-    double acc = 0.0;
-    for (int g = 0; g < G; ++g) {
-      const double qv = (double)Elem<T>::to_f32(q_cur[((size_t)b * h_q + h * G + g) * D + c]);
-      const double part = neg ? fmin(qv, 0.0) : fmax(qv, 0.0);
-      if (group_reduce == RETRO_GROUP_SUM) acc += part; else s_q[g][i] = part;
-    }
-    if (group_reduce == RETRO_GROUP_SUM) s_q[0][i] = acc;
-  }
-  __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int jbase = page0 + warp * kPagesPerWarp;
-  const uint4* rec = reinterpret_cast<const uint4*>(bounds + (row + jbase) * 2 * D) + lane;
-  uint4 raw[kPagesPerWarp];
-#pragma unroll
-  for (int i = 0; i < kPagesPerWarp; ++i)
-    if (jbase + i < n_pages) raw[i] = ldg_stream(rec + i * 32);
-  double acc[kPagesPerWarp];
-  if (group_reduce == RETRO_GROUP_SUM) {
-    double qreg[kVals];
-#pragma unroll
-    for (int c = 0; c < kVals; ++c) qreg[c] = s_q[0][lane * kVals + c];
-#pragma unroll
-    for (int i = 0; i < kPagesPerWarp; ++i) {
-      acc[i] = 0.0;
-      if (jbase + i < n_pages) {
-        float f[kVals];
-        Rec<T>::unpack(raw[i], f);
-#pragma unroll
-        for (int c = 0; c < kVals; ++c) acc[i] = fma(qreg[c], (double)f[c], acc[i]);
-      }
-    }
-#pragma unroll
-    for (int i = 0; i < kPagesPerWarp; ++i) acc[i] = warp_sum(acc[i]);
-  } else {
-#pragma unroll
-    for (int i = 0; i < kPagesPerWarp; ++i) {
-      acc[i] = -INFINITY;
-      if (jbase + i < n_pages) {
-        float f[kVals];
-        Rec<T>::unpack(raw[i], f);
-        for (int g = 0; g < G; ++g) {
-          double a = 0.0;
-#pragma unroll
-          for (int c = 0; c < kVals; ++c) a = fma(s_q[g][lane * kVals + c], (double)f[c], a);
-          a = warp_sum(a);
-          acc[i] = fmax(acc[i], a);
-        }
-      }
-    }
-  }
-  if (lane == 0) {
-#pragma unroll
-    for (int i = 0; i < kPagesPerWarp; ++i) {
-      const int j = jbase + i;
-      if (j < max_pages) {
-        const double v = j < n_pages ? acc[i] : -INFINITY;
-        if (j < n_pages) scores[row + j] = v;
-        if (scores_out != nullptr) scores_out[row + j] = v;
-      }
-    }
-  }
-}
-
 // ------------------------------------------------------------------------------------------------
 // top-k + mask
 // ------------------------------------------------------------------------------------------------
-constexpr int kTopkThreads = 1024;
 constexpr int kBuckets = 2048;
 
 __device__ __forceinline__ uint64_t order_key(double s) {
@@ -134,7 +60,9 @@ __device__ __forceinline__ uint64_t order_key(double s) {
   return (u >> 63) ? ~u : (u | 0x8000000000000000ull);   // larger score <=> larger key
 }
 
-// exclusive block scan of one int per thread (1024 threads); returns exclusive prefix, *total = block sum
+// exclusive block scan of one int per thread (NT threads, NT / 32 <= 32 warps); returns the exclusive prefix,
+// *total = block sum
+template <int NT>
 __device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int* total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   int inc = v;
@@ -147,7 +75,7 @@ __device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int*
   if (lane == 31) s_warp[warp] = inc;
   __syncthreads();
   if (warp == 0) {
-    int w = s_warp[lane];
+    int w = lane < NT / 32 ? s_warp[lane] : 0;
     int winc = w;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -162,19 +90,20 @@ __device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int*
   return s_warp[warp] + inc - v;
 }
 
-__global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
-    const double* __restrict__ scores, const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ budget_pages,
-    int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages, int32_t* __restrict__ sel_prev,
-    int32_t* __restrict__ sel_count, int h_k, int max_pages, int k_max, int P, int force_last) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  uint64_t* keys = reinterpret_cast<uint64_t*>(smem_raw);   // [max_pages]
+// Executed by all NT threads of one CTA for unit (b, h); scores are read through L2 (written by other CTAs).
+template <int NT>
+__device__ __forceinline__ void topk_mask_block(
+    uint64_t* keys /*shared [max_pages]*/, const double* scores, const int32_t* __restrict__ seq_lens,
+    const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
+    int32_t* __restrict__ sel_prev, int32_t* __restrict__ sel_count, int b, int h, int h_k, int max_pages, int k_max,
+    int P, int force_last) {
+  constexpr int kTopkThreads = NT;
   __shared__ int s_hist[kBuckets];
   __shared__ int s_warp[33];
   __shared__ uint64_t s_red[2][32];
   __shared__ uint64_t s_lo, s_width;
   __shared__ int s_need, s_done;
 
-  const int b = blockIdx.y, h = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int L = seq_lens[b];
   const int t = L - 1;
@@ -198,7 +127,7 @@ __global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
   if (!take_all && k_sel > 0) {
     uint64_t kmin = ~0ull, kmax = 0ull;
     for (int i = tid; i < m; i += kTopkThreads) {
-      const uint64_t key = order_key(scores[row * max_pages + i]);
+      const uint64_t key = order_key(__ldcg(scores + row * max_pages + i));
       keys[i] = key;
       kmin = key < kmin ? key : kmin;
       kmax = key > kmax ? key : kmax;
@@ -212,7 +141,8 @@ __global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
     if (lane == 0) { s_red[0][warp] = kmin; s_red[1][warp] = kmax; }
     __syncthreads();
     if (warp == 0) {
-      kmin = s_red[0][lane]; kmax = s_red[1][lane];
+      kmin = lane < NT / 32 ? s_red[0][lane] : ~0ull;
+      kmax = lane < NT / 32 ? s_red[1][lane] : 0ull;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
         const uint64_t a = __shfl_xor_sync(0xffffffffu, kmin, o), c = __shfl_xor_sync(0xffffffffu, kmax, o);
@@ -222,6 +152,7 @@ __global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
       if (lane == 0) { s_lo = kmin; s_width = kmax - kmin; s_need = k_sel; s_done = 0; }
     }
     __syncthreads();
+    SSTAMP(b == 0 && h == 0 && tid == 0, 4);
     // range-adaptive radix select: live range [lo, lo + range], `need` keys still to take from it
     for (int pass = 0; pass < 8; ++pass) {
       const uint64_t lo = s_lo, range = s_width;
@@ -235,14 +166,20 @@ __global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
         if (off <= range) atomicAdd(&s_hist[(int)(off >> shift)], 1);
       }
       __syncthreads();
-      // thread i owns buckets (2047-2i) and (2046-2i): scanning threads in order walks buckets downward
-      const int b_hi = kBuckets - 1 - 2 * tid, b_lo = b_hi - 1;
-      const int c_hi = s_hist[b_hi], c_lo = s_hist[b_lo];
+      // thread i owns kBuckets / NT consecutive buckets, highest first: scanning threads in order walks buckets
+      // downward
+      constexpr int kPer = kBuckets / NT;
+      int cbk[kPer], csum = 0;
+#pragma unroll
+      for (int u = 0; u < kPer; ++u) { cbk[u] = s_hist[kBuckets - 1 - (tid * kPer + u)]; csum += cbk[u]; }
       int total;
-      const int before = block_excl_scan(c_hi + c_lo, s_warp, &total);   // keys in strictly higher buckets
+      int run = block_excl_scan<NT>(csum, s_warp, &total);   // keys in strictly higher buckets
       int hit = -1, above = 0, cnt = 0;
-      if (before < need && need <= before + c_hi) { hit = b_hi; above = before; cnt = c_hi; }
-      else if (before + c_hi < need && need <= before + c_hi + c_lo) { hit = b_lo; above = before + c_hi; cnt = c_lo; }
+#pragma unroll
+      for (int u = 0; u < kPer; ++u) {
+        if (run < need && need <= run + cbk[u]) { hit = kBuckets - 1 - (tid * kPer + u); above = run; cnt = cbk[u]; }
+        run += cbk[u];
+      }
       if (hit >= 0) {
         const uint64_t new_lo = lo + ((uint64_t)hit << shift);
         const uint64_t width_m1 = shift == 0 ? 0 : ((1ull << shift) - 1);
@@ -260,81 +197,262 @@ __global__ void __launch_bounds__(kTopkThreads) topk_mask_kernel(
     need_in_band = s_need;
   }
 
+  SSTAMP(b == 0 && h == 0 && tid == 0, 5);
   // in-order compaction: thread owns a contiguous chunk of candidate indices
   const int per = (m + kTopkThreads - 1) / kTopkThreads;
   const int i0 = min(tid * per, m), i1 = min(i0 + per, m);
-  int band_cnt = 0;
-  if (!take_all && k_sel > 0)
-    for (int i = i0; i < i1; ++i) {
-      const uint64_t off = keys[i] - thr_lo;
-      band_cnt += (off <= thr_hi_excl_width) ? 1 : 0;
-    }
-  int tot_band;
-  int band_rank = block_excl_scan(band_cnt, s_warp, &tot_band);
-  int sel_cnt = 0;
-  uint32_t mybits_lo = 0;   // chunk sizes are tiny (<= 24): one bit per element
+  // one packed scan: low 16 bits = candidates above the band (always taken), high bits = candidates inside it
+  // (the first need_in_band of them, in index order, are taken); counts are <= kMaxPagesPerSeq < 2^15
+  int above_cnt = 0, band_cnt = 0;
+  uint64_t above_bits = 0, band_bits = 0;   // one bit per owned candidate: chunks are <= kMaxPagesPerSeq / NT = 64
   if (k_sel > 0)
     for (int i = i0; i < i1; ++i) {
-      bool take;
-      if (take_all) take = true;
-      else {
-        const uint64_t key = keys[i];
-        const uint64_t off = key - thr_lo;
-        if (off <= thr_hi_excl_width) { take = band_rank < need_in_band; ++band_rank; }
-        else take = key > thr_lo;   // above the band (off wrapped => key < thr_lo => not taken)
-      }
-      if (take) { mybits_lo |= 1u << (i - i0); ++sel_cnt; }
+      if (take_all) { above_bits |= 1ull << (i - i0); ++above_cnt; continue; }
+      const uint64_t key = keys[i];
+      const uint64_t off = key - thr_lo;
+      if (off <= thr_hi_excl_width) { band_bits |= 1ull << (i - i0); ++band_cnt; }
+      else if (key > thr_lo) { above_bits |= 1ull << (i - i0); ++above_cnt; }   // off wrapped <=> key < thr_lo
     }
-  int tot_sel;
-  int pos = block_excl_scan(sel_cnt, s_warp, &tot_sel);
-  for (int i = i0; i < i1; ++i)
-    if (mybits_lo & (1u << (i - i0))) {
-      if (pos < k_max) {
-        out_pages[pos] = i;
-        int prev = -1;
-        if (A != nullptr) { prev = A[i]; A[i] = t; }
-        out_prev[pos] = prev;
-      }
-      ++pos;
+  int tot_packed;
+  const int before = block_excl_scan<NT>(above_cnt | (band_cnt << 16), s_warp, &tot_packed);   // (ends all reads of keys[])
+  int above_rank = before & 0xffff, band_rank = before >> 16;
+  const int tot_sel = (tot_packed & 0xffff) + min(tot_packed >> 16, need_in_band);
+  int32_t* sel_s = reinterpret_cast<int32_t*>(keys);           // selected pages, ascending; reuses the key storage
+  for (int i = i0; i < i1; ++i) {
+    const uint64_t bit = 1ull << (i - i0);
+    bool take = false;
+    if (above_bits & bit) { take = true; }
+    else if (band_bits & bit) { take = band_rank < need_in_band; }
+    if (take) {
+      const int pos = above_rank + min(band_rank, need_in_band);
+      if (pos < k_max) sel_s[pos] = i;
     }
-  int count = min(tot_sel, k_max);
-  if (forced && tid == 0 && count < k_max) {
-    const int p = n_pages - 1;
-    out_pages[count] = p;
-    int prev = -1;
-    if (A != nullptr) { prev = A[p]; A[p] = t; }
-    out_prev[count] = prev;
+    if (above_bits & bit) ++above_rank;
+    if (band_bits & bit) ++band_rank;
   }
+  int count = min(tot_sel, k_max);
+  if (forced && tid == 0 && count < k_max) sel_s[count] = n_pages - 1;
   if (forced) count = min(count + 1, k_max);
+  __syncthreads();
+  SSTAMP(b == 0 && h == 0 && tid == 0, 6);
+  // Alg. 2: M.append(A[p]); A[p] <- t.  One selected page per thread, so the A gathers overlap.
+  for (int i = tid; i < count; i += kTopkThreads) {
+    const int j = sel_s[i];
+    int prev = -1;
+    if (A != nullptr) { prev = A[j]; A[j] = t; }
+    out_pages[i] = j;
+    out_prev[i] = prev;
+  }
   for (int i = count + tid; i < k_max; i += kTopkThreads) { out_pages[i] = -1; out_prev[i] = -1; }
   if (tid == 0) sel_count[row] = count;
 }
+
+template <typename T, int D>
+__global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
+    const T* __restrict__ q_cur, const T* __restrict__ bounds, const int32_t* __restrict__ seq_lens,
+    const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
+    int32_t* __restrict__ sel_prev, int32_t* __restrict__ sel_count, double* scores, double* __restrict__ scores_out,
+    unsigned int* counters, int h_q, int h_k, int max_pages, int k_max, int P, int group_reduce, int force_last,
+    int pages_per_cta /*multiple of kPagesPerCta*/) {
+  static_assert(2 * D * sizeof(T) == 512, "digest record must be 512 bytes");
+  constexpr int kVals = Rec<T>::kVals;
+  extern __shared__ __align__(16) unsigned char smem_raw[];   // top-k keys (only the unit's last CTA uses them)
+  [[maybe_unused]] const bool u0 = blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0;
+  SSTAMP(u0 && blockIdx.x == 0, 0);
+  unsigned long long t_begin = 0;
+#ifdef RETRO_STAMPS
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_begin) :: "memory");
+#endif
+  __shared__ double s_q[kMaxGroup][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
+  __shared__ unsigned int s_ticket;
+  const int b = blockIdx.z, h = blockIdx.y;
+  const int G = h_q / h_k;
+  const int n_pages = (seq_lens[b] + P - 1) / P;
+  const int cta_page0 = blockIdx.x * pages_per_cta;
+  const size_t row = ((size_t)b * h_k + h) * max_pages;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (scores_out != nullptr)   // test output: pages past the end read -inf
+    for (int j = max(cta_page0, n_pages) + threadIdx.x; j < min(cta_page0 + pages_per_cta, max_pages); j += blockDim.x)
+      scores_out[row + j] = -INFINITY;
+  if (cta_page0 < n_pages) {
+  // the digest stream does not depend on q: start the first batch before q is staged; afterwards one batch
+  // of 8 records per lane stays in flight while the previous one is reduced
+  const int page_end = min(cta_page0 + pages_per_cta, n_pages);
+  auto load = [&](uint4 (&r)[kPagesPerWarp], int page0) {
+    const int jbase = page0 + warp * kPagesPerWarp;
+    const uint4* rec = reinterpret_cast<const uint4*>(bounds + (row + jbase) * 2 * D) + lane;
+#pragma unroll
+    for (int i = 0; i < kPagesPerWarp; ++i)
+      if (jbase + i < n_pages) r[i] = ldg_stream(rec + i * 32);
+  };
+  uint4 raw_a[kPagesPerWarp], raw_b[kPagesPerWarp];
+  load(raw_a, cta_page0);
+  // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
+  for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) {
+    const int c = i % D;
+    const bool neg = i >= D;
+    double acc = 0.0;
+    for (int g = 0; g < G; ++g) {
+      const double qv = (double)Elem<T>::to_f32(q_cur[((size_t)b * h_q + h * G + g) * D + c]);
+      const double part = neg ? fmin(qv, 0.0) : fmax(qv, 0.0);
+      if (group_reduce == RETRO_GROUP_SUM) acc += part; else s_q[g][i] = part;
+    }
+    if (group_reduce == RETRO_GROUP_SUM) s_q[0][i] = acc;
+  }
+  __syncthreads();
+  double qreg[kVals];
+#pragma unroll
+  for (int c = 0; c < kVals; ++c) qreg[c] = s_q[0][lane * kVals + c];
+  auto reduce_store = [&](const uint4 (&r)[kPagesPerWarp], int page0) {
+    const int jbase = page0 + warp * kPagesPerWarp;
+    double acc[kPagesPerWarp];
+    if (group_reduce == RETRO_GROUP_SUM) {
+#pragma unroll
+      for (int i = 0; i < kPagesPerWarp; ++i) {
+        acc[i] = 0.0;
+        if (jbase + i < n_pages) {
+          float f[kVals];
+          Rec<T>::unpack(r[i], f);
+#pragma unroll
+          for (int c = 0; c < kVals; ++c) acc[i] = fma(qreg[c], (double)f[c], acc[i]);
+        }
+      }
+      // 8 sums over 32 lanes: three halving levels (4 + 2 + 1 exchanges) then two butterfly levels; the lanes
+      // with (lane & 3) == 0 end up with page jbase + (lane >> 2)
+      static_assert(kPagesPerWarp == 8, "halving reduction is written for 8 pages per warp");
+      {
+        const bool up = lane & 16;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const double send = up ? acc[i] : acc[i + 4], keep = up ? acc[i + 4] : acc[i];
+          acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+        }
+      }
+      {
+        const bool up = lane & 8;
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const double send = up ? acc[i] : acc[i + 2], keep = up ? acc[i + 2] : acc[i];
+          acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+      }
+      double v;
+      {
+        const bool up = lane & 4;
+        const double send = up ? acc[0] : acc[1], keep = up ? acc[1] : acc[0];
+        v = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+      }
+      v += __shfl_xor_sync(0xffffffffu, v, 2);
+      v += __shfl_xor_sync(0xffffffffu, v, 1);
+      const int j = jbase + (lane >> 2);
+      if ((lane & 3) == 0 && j < n_pages) {
+        scores[row + j] = v;
+        if (scores_out != nullptr) scores_out[row + j] = v;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < kPagesPerWarp; ++i) {
+        acc[i] = -INFINITY;
+        if (jbase + i < n_pages) {
+          float f[kVals];
+          Rec<T>::unpack(r[i], f);
+          for (int g = 0; g < G; ++g) {
+            double a = 0.0;
+#pragma unroll
+            for (int c = 0; c < kVals; ++c) a = fma(s_q[g][lane * kVals + c], (double)f[c], a);
+            a = warp_sum(a);
+            acc[i] = fmax(acc[i], a);
+          }
+        }
+      }
+      if (lane == 0) {
+#pragma unroll
+        for (int i = 0; i < kPagesPerWarp; ++i) {
+          const int j = jbase + i;
+          if (j < n_pages) {
+            scores[row + j] = acc[i];
+            if (scores_out != nullptr) scores_out[row + j] = acc[i];
+          }
+        }
+      }
+    }
+  };
+  int page0 = cta_page0;
+  while (true) {
+    if (page0 + kPagesPerCta < page_end) load(raw_b, page0 + kPagesPerCta);
+    reduce_store(raw_a, page0);
+    page0 += kPagesPerCta;
+    if (page0 >= page_end) break;
+    if (page0 + kPagesPerCta < page_end) load(raw_a, page0 + kPagesPerCta);
+    reduce_store(raw_b, page0);
+    page0 += kPagesPerCta;
+    if (page0 >= page_end) break;
+  }
+  }   // cta_page0 < n_pages
+  // ---- the last CTA of the unit to get here selects (release: barrier, then one cumulative fence) ----
+  const size_t unit = (size_t)b * h_k + h;
+  SSTAMP(u0 && blockIdx.x == 0, 1);
+  __syncthreads();
+  if (threadIdx.x == 0) s_ticket = ticket_acq_rel(&counters[unit]);
+  __syncthreads();
+  if (s_ticket != gridDim.x - 1) return;
+#ifdef RETRO_STAMPS
+  if (u0) g_sel_stamps[2] = t_begin;
+#endif
+  SSTAMP(u0, 3);
+  if (threadIdx.x == 0) counters[unit] = 0;   // leave the workspace consistent for the next call
+  topk_mask_block<kScoreWarps * 32>(reinterpret_cast<uint64_t*>(smem_raw), scores, seq_lens, budget_pages,
+                                    last_loaded, sel_pages, sel_prev, sel_count, b, h, h_k, max_pages, k_max, P,
+                                    force_last);
+  SSTAMP(u0, 9);
+}
+
+#ifdef RETRO_STAMPS
+extern "C" int retro_debug_read_sel_stamps(unsigned long long* host_out) {
+  return (int)cudaMemcpyFromSymbol(host_out, g_sel_stamps, sizeof(unsigned long long) * 32);
+}
+#endif
 
 int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
                         const int32_t* seq_lens, const int32_t* budget_pages, int32_t* last_loaded,
                         int32_t* sel_pages, int32_t* sel_prev, int32_t* sel_count, double* scores_out,
                         void* workspace, cudaStream_t s) {
-  double* scores = reinterpret_cast<double*>(static_cast<char*>(workspace) + wl.scores_off);
-  dim3 grid(ceil_div(d->max_pages_per_seq, kPagesPerCta), d->num_kv_heads, d->batch);
-  if (d->dtype == RETRO_BF16) {
-    page_score_kernel<__nv_bfloat16, 128><<<grid, kScoreWarps * 32, 0, s>>>(
-        (const __nv_bfloat16*)q_cur, (const __nv_bfloat16*)bounds, seq_lens, scores, scores_out, d->num_q_heads,
-        d->num_kv_heads, d->max_pages_per_seq, d->page_size, d->group_reduce);
-  } else {
-    page_score_kernel<float, 64><<<grid, kScoreWarps * 32, 0, s>>>(
-        (const float*)q_cur, (const float*)bounds, seq_lens, scores, scores_out, d->num_q_heads, d->num_kv_heads,
-        d->max_pages_per_seq, d->page_size, d->group_reduce);
-  }
-  RETRO_LAUNCH_CHECK();
+  char* ws = static_cast<char*>(workspace);
+  double* scores = reinterpret_cast<double*>(ws + wl.scores_off);
+  unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;
+  // about three resident CTAs per SM in total, each streaming whole batches of 64 pages: the per-CTA costs (q
+  // staging, arrival ticket) amortise over several batches when there are many units
+  const int units = d->batch * d->num_kv_heads;
+  int nchunk = (3 * 148) / units;
+  if (nchunk < 1) nchunk = 1;
+  const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerCta);
+  if (nchunk > max_chunks) nchunk = max_chunks;
+  const int pages_per_cta = ceil_div(ceil_div(d->max_pages_per_seq, nchunk), kPagesPerCta) * kPagesPerCta;
+  dim3 grid(ceil_div(d->max_pages_per_seq, pages_per_cta), d->num_kv_heads, d->batch);
   const size_t smem = (size_t)d->max_pages_per_seq * sizeof(uint64_t);
-  static bool attr_set = false;
-  if (!attr_set) {
-    RETRO_CUDA_TRY(cudaFuncSetAttribute(topk_mask_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    attr_set = true;
+  if (d->dtype == RETRO_BF16) {
+    auto kern = select_pages_kernel<__nv_bfloat16, 128>;
+    static size_t allowed = 48 * 1024;
+    if (smem > allowed) {
+      RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      allowed = smem;
+    }
+    kern<<<grid, kScoreWarps * 32, smem, s>>>(
+        (const __nv_bfloat16*)q_cur, (const __nv_bfloat16*)bounds, seq_lens, budget_pages, last_loaded, sel_pages,
+        sel_prev, sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
+        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta);
+  } else {
+    auto kern = select_pages_kernel<float, 64>;
+    static size_t allowed = 48 * 1024;
+    if (smem > allowed) {
+      RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      allowed = smem;
+    }
+    kern<<<grid, kScoreWarps * 32, smem, s>>>(
+        (const float*)q_cur, (const float*)bounds, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev,
+        sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
+        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta);
   }
-  topk_mask_kernel<<<dim3(d->num_kv_heads, d->batch), kTopkThreads, smem, s>>>(
-      scores, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev, sel_count, d->num_kv_heads,
-      d->max_pages_per_seq, d->max_sel_pages, d->page_size, d->force_last_page);
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }
