@@ -88,6 +88,8 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
 
   const int split = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  pdl_wait();
+  pdl_trigger();
   const int L = p.seq_lens[b];
   const int t = L - 1;
   const size_t unit = (size_t)b * p.h_k + h;
@@ -244,7 +246,7 @@ static int launch_simt(const retro_desc_t* d, const AttendParams& prm, cudaStrea
     RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     smem_allowed = smem;
   }
-  kern<<<dim3(prm.nsplit, d->num_kv_heads, d->batch), kAttWarps * 32, smem, s>>>(prm);
+  RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit, d->num_kv_heads, d->batch), dim3(kAttWarps * 32), smem, s, prm));
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }

@@ -247,10 +247,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
   const size_t unit = (size_t)b * p.h_k + h;
 
-  // ---- prologue.  Global loads that depend on nothing are issued first (count, length, the list entries of
-  // this split, Q); only block_table[j] is a second round trip.
-  const int count = p.sel_count[unit];
-  const int L = p.seq_lens[b];
+  // ---- prologue.  Barriers and TMEM do not depend on the previous kernel: set them up before waiting for it.
   if (tid == 0) {
     for (int i = 0; i < 12; ++i) mbar_init(&bars[i], 1);
     mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
@@ -263,6 +260,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
                  "r"(cfg.tmem_cols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
+  pdl_wait();
+  pdl_trigger();
+  // Global loads that depend on nothing are issued first (count, length, the list entries of this split, Q);
+  // only block_table[j] is a second round trip.
+  const int count = p.sel_count[unit];
+  const int L = p.seq_lens[b];
   for (int i = tid; i < pps; i += kUmmaThreads) {
     const int idx = split * pps + i;
     int j = 0, prev = 0;
@@ -659,7 +662,8 @@ static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const Umma
                                         cudaSharedmemCarveoutMaxShared));
     smem_allowed = smem;
   }
-  kern<<<dim3(prm.nsplit, d->num_kv_heads, d->batch), kUmmaThreads, smem, s>>>(prm, cfg, mk, mv);
+  RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit, d->num_kv_heads, d->batch), dim3(kUmmaThreads), smem, s, prm, cfg, mk,
+                               mv));
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }

@@ -64,6 +64,8 @@ __global__ void __launch_bounds__(128) page_bounds_kernel(const T* __restrict__ 
   const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   const int total = B * h_k * max_touched;
+  pdl_wait();
+  pdl_trigger();
   if (warp >= total) return;
   const int jj = warp % max_touched;
   const int h = (warp / max_touched) % h_k;
@@ -115,15 +117,14 @@ int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const 
   const int block = 128;
   const unsigned grid = (unsigned)((warps * 32 + block - 1) / block);
   if (d->dtype == RETRO_BF16) {
-    page_bounds_kernel<__nv_bfloat16, 128, 16><<<grid, block, 0, s>>>(
+    RETRO_CUDA_TRY(launch_kernel(page_bounds_kernel<__nv_bfloat16, 128, 16>, dim3(grid), dim3(block), 0, s,
         (const __nv_bfloat16*)k_pages, block_table, seq_lens, pos_begin, (__nv_bfloat16*)bounds, d->batch,
-        d->num_kv_heads, d->max_pages_per_seq, max_touched);
+        d->num_kv_heads, d->max_pages_per_seq, max_touched));
   } else {
-    page_bounds_kernel<float, 64, 16><<<grid, block, 0, s>>>((const float*)k_pages, block_table, seq_lens, pos_begin,
-                                                             (float*)bounds, d->batch, d->num_kv_heads,
-                                                             d->max_pages_per_seq, max_touched);
+    RETRO_CUDA_TRY(launch_kernel(page_bounds_kernel<float, 64, 16>, dim3(grid), dim3(block), 0, s, (const float*)k_pages,
+                                 block_table, seq_lens, pos_begin, (float*)bounds, d->batch, d->num_kv_heads,
+                                 d->max_pages_per_seq, max_touched));
   }
-  RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }
 
@@ -133,6 +134,8 @@ __global__ void append_kv_kernel(const T* __restrict__ k_new, const T* __restric
                                  const int32_t* __restrict__ block_table, const int32_t* __restrict__ seq_lens,
                                  T* __restrict__ k_pages, T* __restrict__ v_pages, int B, int h_k, int max_pages) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // one 16 B chunk each: [B][h_k][2][16]
+  pdl_wait();
+  pdl_trigger();
   if (idx >= B * h_k * 32) return;
   const int col = idx & 15, kv = (idx >> 4) & 1, h = (idx >> 5) % h_k, b = idx / (32 * h_k);
   const int pos = seq_lens[b] - 1;
@@ -148,15 +151,14 @@ int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new
   const int n = d->batch * d->num_kv_heads * 32;
   const int block = 128, grid = ceil_div(n, block);
   if (d->dtype == RETRO_BF16) {
-    append_kv_kernel<__nv_bfloat16, 128, 16><<<grid, block, 0, s>>>(
+    RETRO_CUDA_TRY(launch_kernel(append_kv_kernel<__nv_bfloat16, 128, 16>, dim3(grid), dim3(block), 0, s,
         (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new, block_table, seq_lens, (__nv_bfloat16*)k_pages,
-        (__nv_bfloat16*)v_pages, d->batch, d->num_kv_heads, d->max_pages_per_seq);
+        (__nv_bfloat16*)v_pages, d->batch, d->num_kv_heads, d->max_pages_per_seq));
   } else {
-    append_kv_kernel<float, 64, 16><<<grid, block, 0, s>>>((const float*)k_new, (const float*)v_new, block_table,
-                                                           seq_lens, (float*)k_pages, (float*)v_pages, d->batch,
-                                                           d->num_kv_heads, d->max_pages_per_seq);
+    RETRO_CUDA_TRY(launch_kernel(append_kv_kernel<float, 64, 16>, dim3(grid), dim3(block), 0, s, (const float*)k_new,
+                                 (const float*)v_new, block_table, seq_lens, (float*)k_pages, (float*)v_pages,
+                                 d->batch, d->num_kv_heads, d->max_pages_per_seq));
   }
-  RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }
 
@@ -167,6 +169,8 @@ __global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __res
                                                                int32_t* q_pos, uint4* q_cur_out, int B, int h_q,
                                                                int rows) {
   __shared__ int s_pos[64];
+  pdl_wait();
+  pdl_trigger();
   const int row_chunks = h_q * 16;   // uint4 per [h_q][d] block (a q row is 256 B)
   size_t src_off = 0;
   if (step_counter != nullptr) src_off = (size_t)(*step_counter % pool_steps) * B * row_chunks;
@@ -194,10 +198,9 @@ __global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __res
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
                           int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s) {
   if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
-  window_advance_kernel<<<1, 1024, 0, s>>>((const uint4*)q_new_or_pool, step_counter, pool_steps, seq_lens,
-                                           (uint4*)q_win, q_pos, (uint4*)q_cur_out, d->batch, d->num_q_heads,
-                                           d->window + 1);
-  RETRO_LAUNCH_CHECK();
+  RETRO_CUDA_TRY(launch_kernel(window_advance_kernel, dim3(1), dim3(1024), 0, s, (const uint4*)q_new_or_pool,
+                               step_counter, pool_steps, seq_lens, (uint4*)q_win, q_pos, (uint4*)q_cur_out, d->batch,
+                               d->num_q_heads, d->window + 1));
   return RETRO_OK;
 }
 

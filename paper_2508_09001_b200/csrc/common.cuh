@@ -68,6 +68,33 @@ int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int3
                           int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s);
 
 #ifdef __CUDACC__
+// ---- programmatic dependent launch ---------------------------------------------------------------
+// Every libretro kernel is launched with the programmatic-stream-serialization attribute, waits for the
+// COMPLETION of its predecessor (pdl_wait) before it touches global memory and then lets its own dependent
+// start launching (pdl_trigger).  The next kernel's launch latency, CTA scheduling and shared-memory / TMEM
+// set-up overlap the current kernel (also inside a captured CUDA graph); the data dependence is unchanged and at
+// most two kernels are resident at a time (triggering before the wait let the whole chain pile up on the SMs).
+// RETRO_PDL=0 turns the attribute off (griddepcontrol.* are then no-ops).
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+inline bool pdl_enabled() {
+  static const bool on = [] { const char* e = getenv("RETRO_PDL"); return e == nullptr || e[0] != '0'; }();
+  return on;
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                 Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ---- device helpers ---------------------------------------------------------------------------
 template <typename T> struct Elem;
 template <> struct Elem<float> {

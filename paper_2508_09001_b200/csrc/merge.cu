@@ -31,6 +31,8 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
                                                           float* cache_lse, int32_t* cache_pos, T* __restrict__ out,
                                                           float* __restrict__ out_lse, int h_q, int D, int w) {
   const int b = blockIdx.y, x = blockIdx.x;
+  pdl_wait();
+  pdl_trigger();
   const int R = w + 1;
   const int t = seq_lens[b] - 1;
   const int vec_per_row = D / 4;
@@ -146,13 +148,13 @@ int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const 
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s) {
   dim3 grid(d->window + 1, d->batch);
   if (d->dtype == RETRO_BF16)
-    merge_cache_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>(part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse,
-                                                          cache_pos, (__nv_bfloat16*)out, out_lse, d->num_q_heads,
-                                                          d->head_dim, d->window);
+    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<__nv_bfloat16>, grid, dim3(256), 0, s, part_o, part_lse, q_pos,
+                                 seq_lens, cache_o, cache_lse, cache_pos, (__nv_bfloat16*)out, out_lse,
+                                 d->num_q_heads, d->head_dim, d->window));
   else
-    merge_cache_kernel<float><<<grid, 256, 0, s>>>(part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse, cache_pos,
-                                                   (float*)out, out_lse, d->num_q_heads, d->head_dim, d->window);
-  RETRO_LAUNCH_CHECK();
+    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<float>, grid, dim3(256), 0, s, part_o, part_lse, q_pos, seq_lens,
+                                 cache_o, cache_lse, cache_pos, (float*)out, out_lse, d->num_q_heads, d->head_dim,
+                                 d->window));
   return RETRO_OK;
 }
 

@@ -265,6 +265,8 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
 #endif
   __shared__ double s_q[kMaxGroup][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
   __shared__ unsigned int s_ticket;
+  pdl_wait();
+  pdl_trigger();
   const int b = blockIdx.z, h = blockIdx.y;
   const int G = h_q / h_k;
   const int n_pages = (seq_lens[b] + P - 1) / P;
@@ -420,10 +422,11 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   char* ws = static_cast<char*>(workspace);
   double* scores = reinterpret_cast<double*>(ws + wl.scores_off);
   unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;
-  // about three resident CTAs per SM in total, each streaming whole batches of 64 pages: the per-CTA costs (q
-  // staging, arrival ticket) amortise over several batches when there are many units
+  // at most ONE wave of CTAs (two are resident per SM: 128 registers x 256 threads), each streaming whole batches
+  // of 64 pages: the per-CTA costs (q staging, arrival ticket) amortise over several batches when there are many
+  // units, and no unit waits for a second wave before its last CTA can select
   const int units = d->batch * d->num_kv_heads;
-  int nchunk = (3 * 148) / units;
+  int nchunk = (2 * 148) / units;
   if (nchunk < 1) nchunk = 1;
   const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerCta);
   if (nchunk > max_chunks) nchunk = max_chunks;
@@ -437,10 +440,10 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
       RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       allowed = smem;
     }
-    kern<<<grid, kScoreWarps * 32, smem, s>>>(
+    RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s,
         (const __nv_bfloat16*)q_cur, (const __nv_bfloat16*)bounds, seq_lens, budget_pages, last_loaded, sel_pages,
         sel_prev, sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
-        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta);
+        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
   } else {
     auto kern = select_pages_kernel<float, 64>;
     static size_t allowed = 48 * 1024;
@@ -448,12 +451,11 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
       RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       allowed = smem;
     }
-    kern<<<grid, kScoreWarps * 32, smem, s>>>(
+    RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s,
         (const float*)q_cur, (const float*)bounds, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev,
         sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
-        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta);
+        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
   }
-  RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }
 
