@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
   const int t = seq_lens[b] - 1;
   const int vec_per_row = D / 4;
   const int n_vec = h_q * vec_per_row;
-  __shared__ int s_past_row, s_cur_row, s_cached;
+  __shared__ int s_past_row, s_cur_row, s_cached, s_ppast;
 
   if (x == w) {   // empty rows -> zeros / -inf
     for (int r = 0; r < R; ++r) {
@@ -63,83 +63,91 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
     return;
   }
 
-  // slot x: the past position p in [t-w, t-1] with p mod w == x, and (if x == t mod w) the current row
+  // slot x: the past position p in [t-w, t-1] with p mod w == x, and (if x == t mod w) the current row.
+  // A slot has exactly one writer per step: if the current row lands here, the past row of this slot is the
+  // evicted one (position t-w).  Latency-bound, so: one round trip for the roles, one for ALL the operands
+  // (issued unconditionally where the address is valid), then the stores.
   const int slot = x;
-  if (threadIdx.x == 0) {
-    int past = -1, cur = -1;
-    for (int r = 0; r < R; ++r) {
-      const int p = q_pos[b * R + r];
-      if (p < 0 || p > t || p < t - w) continue;
-      if (p == t) { if (t % w == slot) cur = r; }
-      else if (p % w == slot) past = r;
+  if (threadIdx.x == 0) { s_past_row = -1; s_cur_row = -1; s_cached = 0; s_ppast = -1; }
+  __syncthreads();
+  if (threadIdx.x < R) {
+    const int r = threadIdx.x;
+    const int p = q_pos[b * R + r];
+    if (p >= 0 && p <= t && p >= t - w) {
+      if (p == t) { if (t % w == slot) s_cur_row = r; }
+      else if (p % w == slot) { s_past_row = r; s_ppast = p; s_cached = (cache_pos[b * w + slot] == p) ? 1 : 0; }
     }
-    s_past_row = past;
-    s_cur_row = cur;
-    s_cached = (past >= 0 && cache_pos[b * w + slot] == q_pos[b * R + past]) ? 1 : 0;
   }
   __syncthreads();
   const int past = s_past_row, cur = s_cur_row;
   const bool cached = s_cached != 0;
-  const int p_past = past >= 0 ? q_pos[b * R + past] : -1;
+  const int p_past = s_ppast;
   const bool evict = past >= 0 && p_past == t - w;   // popped after its last merge
   float* c_o = cache_o + ((size_t)b * w + slot) * h_q * D;
   float* c_l = cache_lse + ((size_t)b * w + slot) * h_q;
-
-  if (past >= 0) {
-    const float* po = part_o + ((size_t)b * R + past) * h_q * D;
-    const float* pl = part_lse + ((size_t)b * R + past) * h_q;
-    T* oo = out + ((size_t)b * R + past) * h_q * D;
-    for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
+  const float* po = part_o + ((size_t)b * R + (past >= 0 ? past : 0)) * h_q * D;
+  const float* pl = part_lse + ((size_t)b * R + (past >= 0 ? past : 0)) * h_q;
+  const float* qo = part_o + ((size_t)b * R + (cur >= 0 ? cur : 0)) * h_q * D;
+  const float* ql = part_lse + ((size_t)b * R + (cur >= 0 ? cur : 0)) * h_q;
+  for (int i0 = 0; i0 < n_vec; i0 += 4 * blockDim.x) {
+    float4 vp[4], vc[4], vq[4];
+    float lp[4], lc[4], lq[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {             // every load of the pass is in flight before the first use
+      const int i = i0 + u * blockDim.x + threadIdx.x;
+      if (i < n_vec) {
+        const int hh = i / vec_per_row;
+        if (past >= 0) { vp[u] = *reinterpret_cast<const float4*>(po + (size_t)i * 4); lp[u] = pl[hh]; }
+        if (past >= 0 && cached) { vc[u] = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4); lc[u] = c_l[hh]; }
+        if (cur >= 0) { vq[u] = *reinterpret_cast<const float4*>(qo + (size_t)i * 4); lq[u] = ql[hh]; }
+      }
+    }
+    if (!cached) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) lc[u] = -INFINITY;
+    }
+    __syncthreads();   // c_l / c_o of this pass are in registers before anybody rewrites them
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * blockDim.x + threadIdx.x;
+      if (i >= n_vec) continue;
       const int hh = i / vec_per_row;
-      const float lp = pl[hh];
-      const float lc = cached ? c_l[hh] : -INFINITY;
-      float4 vp = *reinterpret_cast<const float4*>(po + (size_t)i * 4);
-      float4 res;
-      if (lc == -INFINITY) res = vp;
-      else if (lp == -INFINITY) res = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4);
-      else {
-        const float4 vc = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4);
-        const float mx = fmaxf(lc, lp);
-        const float wc = __expf(lc - mx), wp = __expf(lp - mx);
-        const float inv = 1.f / (wc + wp);
-        res.x = (wc * vc.x + wp * vp.x) * inv; res.y = (wc * vc.y + wp * vp.y) * inv;
-        res.z = (wc * vc.z + wp * vp.z) * inv; res.w = (wc * vc.w + wp * vp.w) * inv;
+      const bool head_lane = (i % vec_per_row) == 0;
+      if (past >= 0) {
+        T* oo = out + ((size_t)b * R + past) * h_q * D;
+        float4 res;
+        float lse;
+        if (lc[u] == -INFINITY) { res = vp[u]; lse = lp[u]; }
+        else if (lp[u] == -INFINITY) { res = vc[u]; lse = lc[u]; }
+        else {
+          const float mx = fmaxf(lc[u], lp[u]);
+          const float wc = __expf(lc[u] - mx), wp = __expf(lp[u] - mx);
+          const float inv = 1.f / (wc + wp);
+          res.x = (wc * vc[u].x + wp * vp[u].x) * inv; res.y = (wc * vc[u].y + wp * vp[u].y) * inv;
+          res.z = (wc * vc[u].z + wp * vp[u].z) * inv; res.w = (wc * vc[u].w + wp * vp[u].w) * inv;
+          lse = mx + __logf(wc + wp);
+        }
+        OutVec<T>::store(oo + (size_t)i * 4, res);
+        if (!evict) *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = res;
+        if (head_lane) {
+          if (out_lse != nullptr) out_lse[((size_t)b * R + past) * h_q + hh] = lse;
+          if (!evict) c_l[hh] = lse;
+        }
       }
-      OutVec<T>::store(oo + (size_t)i * 4, res);
-      if (!evict) *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = res;
-    }
-    __syncthreads();   // every thread has read c_l before it is rewritten
-    for (int hh = threadIdx.x; hh < h_q; hh += blockDim.x) {
-      const float lp = pl[hh];
-      const float lc = cached ? c_l[hh] : -INFINITY;
-      float lse;
-      if (lc == -INFINITY) lse = lp;
-      else if (lp == -INFINITY) lse = lc;
-      else {
-        const float mx = fmaxf(lc, lp);
-        lse = mx + __logf(__expf(lc - mx) + __expf(lp - mx));
+      if (cur >= 0) {   // push O_org of the current query (the popped row is already in registers)
+        T* oo = out + ((size_t)b * R + cur) * h_q * D;
+        OutVec<T>::store(oo + (size_t)i * 4, vq[u]);
+        *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = vq[u];
+        if (head_lane) {
+          if (out_lse != nullptr) out_lse[((size_t)b * R + cur) * h_q + hh] = lq[u];
+          c_l[hh] = lq[u];
+        }
       }
-      if (out_lse != nullptr) out_lse[((size_t)b * R + past) * h_q + hh] = lse;
-      if (!evict) c_l[hh] = lse;
     }
-    if (!evict && threadIdx.x == 0) cache_pos[b * w + slot] = p_past;
   }
-  if (cur >= 0) {   // push O_org of the current query (after the popped row was read above)
-    __syncthreads();
-    const float* po = part_o + ((size_t)b * R + cur) * h_q * D;
-    const float* pl = part_lse + ((size_t)b * R + cur) * h_q;
-    T* oo = out + ((size_t)b * R + cur) * h_q * D;
-    for (int i = threadIdx.x; i < n_vec; i += blockDim.x) {
-      const float4 v = *reinterpret_cast<const float4*>(po + (size_t)i * 4);
-      OutVec<T>::store(oo + (size_t)i * 4, v);
-      *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = v;
-    }
-    for (int hh = threadIdx.x; hh < h_q; hh += blockDim.x) {
-      const float l = pl[hh];
-      if (out_lse != nullptr) out_lse[((size_t)b * R + cur) * h_q + hh] = l;
-      c_l[hh] = l;
-    }
-    if (threadIdx.x == 0) cache_pos[b * w + slot] = t;
+  if (threadIdx.x == 0) {
+    if (cur >= 0) cache_pos[b * w + slot] = t;
+    else if (past >= 0 && !evict) cache_pos[b * w + slot] = p_past;
   }
 }
 
