@@ -49,12 +49,19 @@ def measured_hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+C5_POINT = {"window": 8, "budget": 4096}     # the C5 sweep point `--workload c5` runs (see --window / --budget)
+
+
 def workload_cfg(name: str, n_steps: int, window=None):
     from paper_2508_09001_b200 import workload as wl
     if name == "c2":
         cfg = wl.c2(n_steps=n_steps)
+    elif name == "c3":
+        cfg = wl.c3(n_steps=n_steps)
+    elif name == "c4":
+        cfg = wl.c4(n_steps=n_steps)
     elif name == "c5":
-        cfg = wl.c5(8, 4096, n_steps=n_steps)
+        cfg = wl.c5(C5_POINT["window"], C5_POINT["budget"], n_steps=n_steps)
     elif name == "c1":
         cfg = wl.c1()
     else:
@@ -221,7 +228,15 @@ def main():
     ap.add_argument("--layers", type=int, default=32)
     ap.add_argument("--no-extras", action="store_true", help="skip w=0 overhead run, stage timing, e2e, cpu baseline")
     ap.add_argument("--oracle-steps", type=int, default=8)
+    ap.add_argument("--window", type=int, default=None, help="C5 sweep: retro window w (past queries)")
+    ap.add_argument("--budget", type=int, default=None, help="C5 sweep: budget in tokens")
+    ap.add_argument("--no-w0", action="store_true", help="skip the w=0 overhead run (sweeps measure w=0 themselves)")
+    ap.add_argument("--lite", action="store_true", help="sweep point: stage timing only (no e2e, cpu baseline, w=0 run)")
     args = ap.parse_args()
+    if args.window is not None:
+        C5_POINT["window"] = args.window
+    if args.budget is not None:
+        C5_POINT["budget"] = args.budget
     if args.impl == "reference":
         return run_reference(args)
 
@@ -299,6 +314,11 @@ def main():
                             "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS}
         line["attend_arith_intensity_flop_per_byte"] = hs.attend_flops(cfg, seq_now) / bytes_model["kv"]
 
+        if args.lite:
+            line["e2e"] = None
+            if ri.rank == 0:
+                print(json.dumps(line))
+            return 0
         # ---- end to end through the C ABI with HOST buffers (H2D of the step's inputs, D2H of its result) ----
         e2e_steps = min(steps, 32)
         e2e = run_e2e(stack, cfg, e2e_steps, dev)
@@ -321,7 +341,7 @@ def main():
         stack_inputs_free(stack)
         del stack
         torch.cuda.empty_cache()
-        if cfg.window > 0:
+        if cfg.window > 0 and not args.no_w0:
             cfg0 = workload_cfg(args.workload, n_steps=warmup + steps + 80, window=0)
             stack0, graph0, ms0 = run_stack(cfg0, L, steps, warmup, seed_off, barrier)
             ms0 = hs.max_over_ranks(ms0, dev)

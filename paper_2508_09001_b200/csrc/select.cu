@@ -32,19 +32,22 @@ __device__ __forceinline__ void sel_stamp(int i) {
 constexpr int kScoreWarps = 8;
 constexpr int kPagesPerWarp = 8;
 constexpr int kPagesPerCta = kScoreWarps * kPagesPerWarp;
+constexpr int kStages = 3;                       // digest batches in flight per CTA
+constexpr int kStageBytes = kPagesPerCta * 512;  // 32 KB
 
-template <typename T> struct Rec;   // how a lane turns its 16 B of a digest record into floats
+template <typename T> struct Rec;   // how a lane turns its 16 B of a digest record into fp64 values
 template <> struct Rec<__nv_bfloat16> {
   static constexpr int kVals = 8;
-  __device__ static __forceinline__ void unpack(uint4 v, float* f) {
-    f[0] = bf16_lo(v.x); f[1] = bf16_hi(v.x); f[2] = bf16_lo(v.y); f[3] = bf16_hi(v.y);
-    f[4] = bf16_lo(v.z); f[5] = bf16_hi(v.z); f[6] = bf16_lo(v.w); f[7] = bf16_hi(v.w);
+  __device__ static __forceinline__ void unpack(uint4 v, double* f) {
+    f[0] = (double)bf16_lo(v.x); f[1] = (double)bf16_hi(v.x); f[2] = (double)bf16_lo(v.y); f[3] = (double)bf16_hi(v.y);
+    f[4] = (double)bf16_lo(v.z); f[5] = (double)bf16_hi(v.z); f[6] = (double)bf16_lo(v.w); f[7] = (double)bf16_hi(v.w);
   }
 };
 template <> struct Rec<float> {
   static constexpr int kVals = 4;
-  __device__ static __forceinline__ void unpack(uint4 v, float* f) {
-    f[0] = __uint_as_float(v.x); f[1] = __uint_as_float(v.y); f[2] = __uint_as_float(v.z); f[3] = __uint_as_float(v.w);
+  __device__ static __forceinline__ void unpack(uint4 v, double* f) {
+    f[0] = (double)__uint_as_float(v.x); f[1] = (double)__uint_as_float(v.y);
+    f[2] = (double)__uint_as_float(v.z); f[3] = (double)__uint_as_float(v.w);
   }
 };
 
@@ -247,7 +250,7 @@ __device__ __forceinline__ void topk_mask_block(
   if (tid == 0) sel_count[row] = count;
 }
 
-template <typename T, int D>
+template <typename T, int D, bool kGroupMax>
 __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
     const T* __restrict__ q_cur, const T* __restrict__ bounds, const int32_t* __restrict__ seq_lens,
     const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
@@ -256,14 +259,16 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
     int pages_per_cta /*multiple of kPagesPerCta*/) {
   static_assert(2 * D * sizeof(T) == 512, "digest record must be 512 bytes");
   constexpr int kVals = Rec<T>::kVals;
-  extern __shared__ __align__(16) unsigned char smem_raw[];   // top-k keys (only the unit's last CTA uses them)
+  // digest ring [kStages][64 records x 512 B]; the unit's last CTA reuses it for the top-k keys
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  __shared__ __align__(8) uint64_t s_full[kStages];
   [[maybe_unused]] const bool u0 = blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0;
   SSTAMP(u0 && blockIdx.x == 0, 0);
   unsigned long long t_begin = 0;
 #ifdef RETRO_STAMPS
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_begin) :: "memory");
 #endif
-  __shared__ double s_q[kMaxGroup][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
+  __shared__ double s_q[kGroupMax ? kMaxGroup : 1][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
   __shared__ unsigned int s_ticket;
   pdl_wait();
   pdl_trigger();
@@ -279,16 +284,23 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
   if (cta_page0 < n_pages) {
   // the digest stream does not depend on q: start the first batch before q is staged; afterwards one batch
   // of 8 records per lane stays in flight while the previous one is reduced
+  // The digest records of consecutive pages are contiguous: one bulk copy (TMA unit, cp.async.bulk + mbarrier)
+  // brings a whole batch of 64 records (32 KB) into the shared-memory ring, kStages batches in flight per CTA,
+  // so the bytes in flight are bounded by shared memory, not by registers.
   const int page_end = min(cta_page0 + pages_per_cta, n_pages);
-  auto load = [&](uint4 (&r)[kPagesPerWarp], int page0) {
-    const int jbase = page0 + warp * kPagesPerWarp;
-    const uint4* rec = reinterpret_cast<const uint4*>(bounds + (row + jbase) * 2 * D) + lane;
-#pragma unroll
-    for (int i = 0; i < kPagesPerWarp; ++i)
-      if (jbase + i < n_pages) r[i] = ldg_stream(rec + i * 32);
+  const int nbatch = (page_end - cta_page0 + kPagesPerCta - 1) / kPagesPerCta;
+  auto issue_batch = [&](int it) {   // thread 0
+    const int p0 = cta_page0 + it * kPagesPerCta;
+    const uint32_t bytes = (uint32_t)min(kPagesPerCta, page_end - p0) * (2 * D * sizeof(T));
+    const int st = it % kStages;
+    mbar_expect_tx(&s_full[st], bytes);
+    bulk_g2s(smem_raw + (size_t)st * kStageBytes, bounds + (row + p0) * 2 * D, bytes, &s_full[st]);
   };
-  uint4 raw_a[kPagesPerWarp], raw_b[kPagesPerWarp];
-  load(raw_a, cta_page0);
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < kStages; ++i) mbar_init(&s_full[i], 1);
+    fence_mbar_init();
+    for (int it = 0; it < min(kStages, nbatch); ++it) issue_batch(it);
+  }
   // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
   for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) {
     const int c = i % D;
@@ -297,27 +309,26 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
     for (int g = 0; g < G; ++g) {
       const double qv = (double)Elem<T>::to_f32(q_cur[((size_t)b * h_q + h * G + g) * D + c]);
       const double part = neg ? fmin(qv, 0.0) : fmax(qv, 0.0);
-      if (group_reduce == RETRO_GROUP_SUM) acc += part; else s_q[g][i] = part;
+      if (!kGroupMax) acc += part; else s_q[g][i] = part;
     }
-    if (group_reduce == RETRO_GROUP_SUM) s_q[0][i] = acc;
+    if (!kGroupMax) s_q[0][i] = acc;
   }
   __syncthreads();
   double qreg[kVals];
 #pragma unroll
   for (int c = 0; c < kVals; ++c) qreg[c] = s_q[0][lane * kVals + c];
-  auto reduce_store = [&](const uint4 (&r)[kPagesPerWarp], int page0) {
+  auto reduce_store = [&](const unsigned char* stage, int page0) {
     const int jbase = page0 + warp * kPagesPerWarp;
+    const uint4* rec = reinterpret_cast<const uint4*>(stage) + warp * kPagesPerWarp * 32 + lane;
     double acc[kPagesPerWarp];
-    if (group_reduce == RETRO_GROUP_SUM) {
+    if constexpr (!kGroupMax) {
 #pragma unroll
-      for (int i = 0; i < kPagesPerWarp; ++i) {
+      for (int i = 0; i < kPagesPerWarp; ++i) {   // records past the last page hold stale bytes: their sums are
+        double f[kVals];                            // computed branch-free and never stored
+        Rec<T>::unpack(rec[i * 32], f);
         acc[i] = 0.0;
-        if (jbase + i < n_pages) {
-          float f[kVals];
-          Rec<T>::unpack(r[i], f);
 #pragma unroll
-          for (int c = 0; c < kVals; ++c) acc[i] = fma(qreg[c], (double)f[c], acc[i]);
-        }
+        for (int c = 0; c < kVals; ++c) acc[i] = fma(qreg[c], f[c], acc[i]);
       }
       // 8 sums over 32 lanes: three halving levels (4 + 2 + 1 exchanges) then two butterfly levels; the lanes
       // with (lane & 3) == 0 end up with page jbase + (lane >> 2)
@@ -356,12 +367,12 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
       for (int i = 0; i < kPagesPerWarp; ++i) {
         acc[i] = -INFINITY;
         if (jbase + i < n_pages) {
-          float f[kVals];
-          Rec<T>::unpack(r[i], f);
+          double f[kVals];
+          Rec<T>::unpack(rec[i * 32], f);
           for (int g = 0; g < G; ++g) {
             double a = 0.0;
 #pragma unroll
-            for (int c = 0; c < kVals; ++c) a = fma(s_q[g][lane * kVals + c], (double)f[c], a);
+            for (int c = 0; c < kVals; ++c) a = fma(s_q[g][lane * kVals + c], f[c], a);
             a = warp_sum(a);
             acc[i] = fmax(acc[i], a);
           }
@@ -379,16 +390,12 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
       }
     }
   };
-  int page0 = cta_page0;
-  while (true) {
-    if (page0 + kPagesPerCta < page_end) load(raw_b, page0 + kPagesPerCta);
-    reduce_store(raw_a, page0);
-    page0 += kPagesPerCta;
-    if (page0 >= page_end) break;
-    if (page0 + kPagesPerCta < page_end) load(raw_a, page0 + kPagesPerCta);
-    reduce_store(raw_b, page0);
-    page0 += kPagesPerCta;
-    if (page0 >= page_end) break;
+  for (int it = 0; it < nbatch; ++it) {
+    const int st = it % kStages;
+    mbar_wait(&s_full[st], (it / kStages) & 1);
+    reduce_store(smem_raw + (size_t)st * kStageBytes, cta_page0 + it * kPagesPerCta);
+    __syncthreads();                                   // every warp is done with the stage: refill it
+    if (threadIdx.x == 0 && it + kStages < nbatch) issue_batch(it + kStages);
   }
   }   // cta_page0 < n_pages
   // ---- the last CTA of the unit to get here selects (release: barrier, then one cumulative fence) ----
@@ -432,31 +439,38 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   if (nchunk > max_chunks) nchunk = max_chunks;
   const int pages_per_cta = ceil_div(ceil_div(d->max_pages_per_seq, nchunk), kPagesPerCta) * kPagesPerCta;
   dim3 grid(ceil_div(d->max_pages_per_seq, pages_per_cta), d->num_kv_heads, d->batch);
-  const size_t smem = (size_t)d->max_pages_per_seq * sizeof(uint64_t);
+  const size_t keys_bytes = (size_t)d->max_pages_per_seq * sizeof(uint64_t);
+  const size_t smem = keys_bytes > (size_t)kStages * kStageBytes ? keys_bytes : (size_t)kStages * kStageBytes;
+  auto launch = [&](auto kern, auto* qp, auto* bp) -> int {
+    // raise the dynamic shared-memory limit once per kernel instantiation (not a stream operation)
+    static const void* raised[8];
+    static size_t raised_to[8];
+    int slot = -1;
+    for (int i = 0; i < 8 && slot < 0; ++i)
+      if (raised[i] == (const void*)kern || raised[i] == nullptr) slot = i;
+    if (slot < 0) slot = 0;
+    if (raised[slot] != (const void*)kern || raised_to[slot] < smem) {
+      RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      raised[slot] = (const void*)kern;
+      raised_to[slot] = smem;
+    }
+    RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s, qp, bp, seq_lens, budget_pages,
+                                 last_loaded, sel_pages, sel_prev, sel_count, scores, scores_out, counters,
+                                 d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq, d->max_sel_pages,
+                                 d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
+    return RETRO_OK;
+  };
+  const bool gmax = d->group_reduce == RETRO_GROUP_MAX;
   if (d->dtype == RETRO_BF16) {
-    auto kern = select_pages_kernel<__nv_bfloat16, 128>;
-    static size_t allowed = 48 * 1024;
-    if (smem > allowed) {
-      RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      allowed = smem;
-    }
-    RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s,
-        (const __nv_bfloat16*)q_cur, (const __nv_bfloat16*)bounds, seq_lens, budget_pages, last_loaded, sel_pages,
-        sel_prev, sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
-        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
-  } else {
-    auto kern = select_pages_kernel<float, 64>;
-    static size_t allowed = 48 * 1024;
-    if (smem > allowed) {
-      RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      allowed = smem;
-    }
-    RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s,
-        (const float*)q_cur, (const float*)bounds, seq_lens, budget_pages, last_loaded, sel_pages, sel_prev,
-        sel_count, scores, scores_out, counters, d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq,
-        d->max_sel_pages, d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
+    const auto* qp = (const __nv_bfloat16*)q_cur;
+    const auto* bp = (const __nv_bfloat16*)bounds;
+    return gmax ? launch(select_pages_kernel<__nv_bfloat16, 128, true>, qp, bp)
+                : launch(select_pages_kernel<__nv_bfloat16, 128, false>, qp, bp);
   }
-  return RETRO_OK;
+  const auto* qp = (const float*)q_cur;
+  const auto* bp = (const float*)bounds;
+  return gmax ? launch(select_pages_kernel<float, 64, true>, qp, bp)
+              : launch(select_pages_kernel<float, 64, false>, qp, bp);
 }
 
 }  // namespace retro
