@@ -32,7 +32,7 @@ __device__ __forceinline__ void sel_stamp(int i) {
 constexpr int kScoreWarps = 8;
 constexpr int kPagesPerWarp = 8;
 constexpr int kPagesPerCta = kScoreWarps * kPagesPerWarp;
-constexpr int kStages = 3;                       // digest batches in flight per CTA
+constexpr int kStages = 2;                       // digest batches in flight per CTA
 constexpr int kStageBytes = kPagesPerCta * 512;  // 32 KB
 
 template <typename T> struct Rec;   // how a lane turns its 16 B of a digest record into fp64 values
@@ -251,7 +251,7 @@ __device__ __forceinline__ void topk_mask_block(
 }
 
 template <typename T, int D, bool kGroupMax>
-__global__ void __launch_bounds__(kScoreWarps * 32, 2) select_pages_kernel(
+__global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     const T* __restrict__ q_cur, const T* __restrict__ bounds, const int32_t* __restrict__ seq_lens,
     const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
     int32_t* __restrict__ sel_prev, int32_t* __restrict__ sel_count, double* scores, double* __restrict__ scores_out,
@@ -433,7 +433,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   // of 64 pages: the per-CTA costs (q staging, arrival ticket) amortise over several batches when there are many
   // units, and no unit waits for a second wave before its last CTA can select
   const int units = d->batch * d->num_kv_heads;
-  int nchunk = (2 * 148) / units;
+  int nchunk = (3 * 148) / units;
   if (nchunk < 1) nchunk = 1;
   const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerCta);
   if (nchunk > max_chunks) nchunk = max_chunks;
