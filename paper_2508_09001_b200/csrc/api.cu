@@ -32,10 +32,13 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   const int units = d->batch * d->num_kv_heads;
   wl.rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
   // split-KV.  Scalar path: units * nsplit covers the 148 SMs about twice, at least 2 pages per split.  The
-  // tensor-core path (bf16, rows <= 128) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per
-  // split: its splits are whole blocks and the grid is at most ONE wave of resident CTAs (148 x CTAs per SM).
-  const bool umma = d->dtype == RETRO_BF16 && wl.rows <= 128;
-  int nsplit = umma ? (148 * umma_ctas_per_sm(wl.rows)) / units : ceil_div(2 * 148, units);
+  // tensor-core path (bf16) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per split: its
+  // splits are whole blocks and the grid (units x row groups x splits) is at most ONE wave of resident CTAs
+  // (one CTA per SM).  More than 128 query rows are handled as ceil(rows / 128) balanced row groups.
+  const bool umma = d->dtype == RETRO_BF16;
+  wl.nrg = umma ? ceil_div(wl.rows, 128) : 1;
+  wl.rg_rows = ceil_div(wl.rows, wl.nrg);
+  int nsplit = umma ? 148 / (units * wl.nrg) : ceil_div(2 * 148, units);
   const int min_pages = umma ? 8 : 2;
   const int max_split = d->max_sel_pages >= min_pages ? d->max_sel_pages / min_pages : 1;
   if (nsplit > max_split) nsplit = max_split;
@@ -51,7 +54,7 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   wl.split_lse_off = off;
   off = align_up(off + (size_t)units * wl.nsplit * wl.rows * sizeof(float), 256);
   wl.counters_off = off;
-  off = align_up(off + (size_t)2 * units * sizeof(unsigned int), 256);
+  off = align_up(off + (size_t)4 * units * sizeof(unsigned int), 256);
   wl.total = off;
   return wl;
 }

@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
   if (p.nsplit == 1) return;
 
   __shared__ unsigned int s_ticket;
-  combine_splits_last_cta<D>(p, unit, b, h, rows, G, R, &s_ticket);
+  combine_splits_last_cta<D>(p, unit, b, h, rows, G, R, &s_ticket, 0, rows, &p.counters[unit]);
 }
 
 template <typename T, int D, int RPW>
@@ -275,11 +275,13 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
   prm.sel_count = sel_count; prm.part_o = part_o; prm.part_lse = part_lse;
   prm.split_o = reinterpret_cast<float*>(ws + wl.split_o_off);
   prm.split_lse = reinterpret_cast<float*>(ws + wl.split_lse_off);
-  prm.counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off);
+  prm.counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;   // [units][nrg]
   prm.B = d->batch; prm.h_q = d->num_q_heads; prm.h_k = d->num_kv_heads; prm.max_pages = d->max_pages_per_seq;
   prm.k_max = d->max_sel_pages; prm.window = d->window; prm.nsplit = wl.nsplit;
   prm.pages_per_split = wl.pages_per_split;
   prm.scale_log2 = d->sm_scale * kLog2e;
+  prm.nrg = 1;
+  prm.rg_rows = wl.rows;
   if (d->dtype == RETRO_BF16) {
     // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu).  The scalar
     // path stays reachable for debugging (RETRO_ATTEND_PATH=simt) and for row blocks above one 128-row tile.
@@ -287,7 +289,11 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
       const char* e = std::getenv("RETRO_ATTEND_PATH");
       return e != nullptr && e[0] == 's';
     }();
-    if (!force_simt && wl.rows <= 128) return launch_attend_umma(d, prm, s);
+    if (!force_simt) {
+      prm.nrg = wl.nrg;
+      prm.rg_rows = wl.rg_rows;
+      return launch_attend_umma(d, prm, s);
+    }
     return dispatch_rpw<__nv_bfloat16, 128>(d, prm, s);
   }
   return dispatch_rpw<float, 64>(d, prm, s);

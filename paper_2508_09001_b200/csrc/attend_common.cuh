@@ -13,6 +13,7 @@ struct AttendParams {
   const int32_t* sel_count; float* part_o; float* part_lse; float* split_o; float* split_lse;
   unsigned int* counters;
   int B, h_q, h_k, max_pages, k_max, window, nsplit, pages_per_split;
+  int nrg, rg_rows;   // query-row groups of the tensor-core path (rows > 128): CTA (split, group) owns rg_rows rows
   float scale_log2;   // sm_scale * log2(e)
 };
 
@@ -23,20 +24,22 @@ struct AttendParams {
 // Called by every thread of the CTA after it wrote its split partial (normalised o, base-2 lse) to the
 // workspace.  The last CTA of the (b, KV head) unit to arrive merges the nsplit partials (Eq. 8 applied to
 // splits: weights 2^(lse_s - max)) into part_o / part_lse (natural-log lse).  D = 128 or 64; one warp per row.
+// Rows [row_begin, row_end) of the unit are combined; `counter` is the arrival counter of that row group.
 template <int D>
 __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, size_t unit, int b, int h, int rows,
-                                                        int G, int R, unsigned int* s_ticket) {
+                                                        int G, int R, unsigned int* s_ticket, int row_begin,
+                                                        int row_end, unsigned int* counter) {
   constexpr int kCh = D / 32;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
   // Release: every thread's partial stores happen-before the barrier; thread 0's acq_rel ticket is cumulative.
   __syncthreads();
-  if (tid == 0) *s_ticket = ticket_acq_rel(&p.counters[unit]);
+  if (tid == 0) *s_ticket = ticket_acq_rel(counter);
   RETRO_COMBINE_STAMP(24);
   __syncthreads();
   RETRO_COMBINE_STAMP(25);
   if (*s_ticket != (unsigned)(p.nsplit - 1)) return;
-  if (tid == 0) p.counters[unit] = 0;   // leave the workspace consistent for the next call
-  for (int rho = warp; rho < rows; rho += nwarps) {
+  if (tid == 0) *counter = 0;   // leave the workspace consistent for the next call
+  for (int rho = row_begin + warp; rho < row_end; rho += nwarps) {
     const float* lse_s = p.split_lse + unit * p.nsplit * rows + rho;
     const float* o_s = p.split_o + (unit * p.nsplit * rows + rho) * D + lane * kCh;
     const size_t o_stride = (size_t)rows * D;

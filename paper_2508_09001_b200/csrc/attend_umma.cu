@@ -29,7 +29,6 @@
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
 
-#include <cstdio>
 #include <cstdlib>
 
 #ifdef RETRO_STAMPS
@@ -240,11 +239,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
 
-  const int split = blockIdx.x, h = blockIdx.y, b = blockIdx.z;
+  const int split = blockIdx.x % p.nsplit, rg = blockIdx.x / p.nsplit, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   [[maybe_unused]] const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
   STAMP(cta0 && tid == 0, 0);
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
+  const int row0 = rg * p.rg_rows;                      // this CTA's query rows: [row0, row0 + rows_cta) of the unit
+  const int rows_cta = min(p.rg_rows, rows - row0);
   const size_t unit = (size_t)b * p.h_k + h;
 
   // ---- prologue.  Barriers and TMEM do not depend on the previous kernel: set them up before waiting for it.
@@ -284,8 +285,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
       const int rho = i >> 4, c = i & 15;
       uint4 v = make_uint4(0, 0, 0, 0);
-      if (rho < rows) {
-        const int r = rho / G, g = rho - r * G;
+      if (rho < rows_cta) {
+        const int r = (row0 + rho) / G, g = (row0 + rho) - r * G;
         v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
       }
       const int half = c >> 3, ch = c & 7;
@@ -296,11 +297,11 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   if (tid < 3) s_flag[tid] = 0;
   for (int c = tid; c < NT; c += kUmmaThreads) {
     int pos = -1, off = 0;
-    if (c < rows) {
-      const int r = c / G, g = c - r * G;
+    if (c < rows_cta) {
+      const int r = (row0 + c) / G, g = (row0 + c) - r * G;
       pos = p.q_pos[b * R + r];
       if (pos > t || pos < t - p.window) pos = -1;
-      off = p.nsplit > 1 ? c * 128 : (r * p.h_q + h * G + g) * 128;
+      off = p.nsplit > 1 ? (row0 + c) * 128 : (r * p.h_q + h * G + g) * 128;
     }
     s_colpos[c] = pos;
     s_coloff[c] = off;
@@ -568,7 +569,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       // thread = channel `key`; its NC rows: O = (O_hi + O_lo) / L, 128 B coalesced per warp and row
 #pragma unroll
       for (int i = 0; i < NCH; ++i) {
-        if (cbeg + 4 * i < rows) {                          // warp-uniform
+        if (cbeg + 4 * i < rows_cta) {                      // warp-uniform
           uint32_t oh[4], ol[4];
           tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
           tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
@@ -576,7 +577,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int c = cbeg + 4 * i + u;
-            if (c < rows) {
+            if (c < rows_cta) {
               const float l = s_L[c];
               const float inv = l > 0.f ? rcp_approx(l) : 0.f;
               const int off = s_coloff[c];
@@ -590,7 +591,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     }
   } else {
     // no page for this split: empty partial for every row
-    for (int rho = tid; rho < rows; rho += kUmmaThreads) {
+    for (int rho = row0 + tid; rho < row0 + rows_cta; rho += kUmmaThreads) {
       if (p.nsplit > 1) {
         p.split_lse[(unit * p.nsplit + split) * rows + rho] = -INFINITY;
       } else {
@@ -609,7 +610,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
   }
   if (p.nsplit == 1) return;
-  combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket);
+  combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket, row0, row0 + rows_cta,
+                               &p.counters[unit * p.nrg + rg]);
   STAMP(cta0 && tid == 0, 22);
 }
 
@@ -662,7 +664,7 @@ static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const Umma
                                         cudaSharedmemCarveoutMaxShared));
     smem_allowed = smem;
   }
-  RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit, d->num_kv_heads, d->batch), dim3(kUmmaThreads), smem, s, prm, cfg, mk,
+  RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit * prm.nrg, d->num_kv_heads, d->batch), dim3(kUmmaThreads), smem, s, prm, cfg, mk,
                                mv));
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
@@ -690,8 +692,7 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
     cache[slot] = c;
     hit = &cache[slot];
   }
-  const int rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
-  const int nch = ceil_div(rows, 16), NT = 16 * nch;
+  const int nch = ceil_div(prm.rg_rows, 16), NT = 16 * nch;
   if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
   // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~2-3 KB static; two CTAs per SM up to
   // Prefer two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in flight per CTA).
@@ -711,9 +712,6 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   if (slots > 6) slots = 6;
   cfg.NK = slots / 2;             // a V block lives longer (it waits for the softmax of its own block)
   cfg.NV = slots - cfg.NK;
-  if (const char* e = std::getenv("RETRO_UMMA_PLAN")) {   // TEMP probe: "NP NK NV"
-    sscanf(e, "%d %d %d", &cfg.NP, &cfg.NK, &cfg.NV);
-  }
   int cols = 32;
   while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
   if (cols > kTmemCols) return RETRO_ERR_UNSUPPORTED;

@@ -29,9 +29,6 @@ void set_cuda_error(cudaError_t e);
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
-// CTAs of the tensor-core attend kernel that share one SM.
-inline int umma_ctas_per_sm(int /*rows*/) { return 1; }
-
 int validate_desc(const retro_desc_t* d);  // RETRO_OK / RETRO_ERR_ARG / RETRO_ERR_UNSUPPORTED
 
 // ---- workspace layout (host + device agree through this struct) --------------------------------
@@ -39,11 +36,12 @@ struct WorkspaceLayout {
   size_t scores_off;    // double [B][h_k][max_pages]
   size_t split_o_off;   // float  [B][h_k][nsplit][rows][d]
   size_t split_lse_off; // float  [B][h_k][nsplit][rows]
-  size_t counters_off;  // uint32 [B][h_k] split arrival counters (+ [B][h_k] score-chunk counters)
+  size_t counters_off;  // uint32 [4][B][h_k]: score-chunk counters first, then split arrival counters per row group
   size_t total;
   int nsplit;           // split-KV factor of the attend kernel
   int pages_per_split;
   int rows;             // G * (w+1)
+  int nrg, rg_rows;     // query-row groups of the tensor-core attend path (one group unless rows > 128)
 };
 WorkspaceLayout workspace_layout(const retro_desc_t* d);
 

@@ -428,7 +428,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
                         void* workspace, cudaStream_t s) {
   char* ws = static_cast<char*>(workspace);
   double* scores = reinterpret_cast<double*>(ws + wl.scores_off);
-  unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off);   // [units] score-chunk arrivals
   // at most ONE wave of CTAs (two are resident per SM: 128 registers x 256 threads), each streaming whole batches
   // of 64 pages: the per-CTA costs (q staging, arrival ticket) amortise over several batches when there are many
   // units, and no unit waits for a second wave before its last CTA can select
