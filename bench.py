@@ -282,7 +282,7 @@ def main():
         "metric": METRIC, "value": us_layer, "unit": UNIT, "n_gpus": ri.world_size, "steps": steps, "warmup": warmup,
         "ms_per_step": ms / steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": cfg.dtype, "data": "synthetic", "config": config_dict(cfg, L), "impl": "ours",
-        "gpu_launches": steps * L * hs.KERNELS_PER_LAYER_STEP,
+        "gpu_launches": steps * (L * hs.KERNELS_PER_LAYER_STEP + hs.KERNELS_PER_STEP),
         "aggregate_layer_steps_per_s": ri.world_size * steps * L / (ms / 1000.0),
         "path_hbm": {"algorithmic_bytes_per_layer_step": bytes_model["total"],
                      "achieved_gbs": bytes_model["total"] / (us_layer * 1e-6) / 1e9,

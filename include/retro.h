@@ -187,6 +187,21 @@ int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, in
                          int32_t pool_steps /*HOST*/, int32_t* seq_lens, void* q_win, int32_t* q_pos,
                          void* q_cur_out /*optional [B][h_q][d]*/, void* stream);
 
+/* The same bookkeeping for n_layers independent layers in ONE launch (one CTA per layer).  Used by the synthetic
+ * benchmark, where every layer's pre-generated query stream advances at the start of a step - the stand-in for
+ * the QKV projections that feed this path in a model.  `table` is a DEVICE array of n_layers records of DEVICE
+ * pointers; every layer uses `desc`'s shapes and a query pool of pool_steps steps. */
+typedef struct retro_advance_rec {
+  const void* q_pool;     /* [pool_steps][B][h_q][d] T */
+  int32_t* step_counter;  /* [1]                       */
+  int32_t* seq_lens;      /* [B]                       */
+  void* q_win;            /* [B][w+1][h_q][d] T        */
+  int32_t* q_pos;         /* [B][w+1]                  */
+  void* q_cur_out;        /* [B][h_q][d] T, may be NULL */
+} retro_advance_rec_t;
+int retro_window_advance_layers(const retro_desc_t* desc, const retro_advance_rec_t* table /*DEVICE*/,
+                                int32_t n_layers, int32_t pool_steps /*HOST*/, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ EXPORTED = [
     "retro_workspace_bytes", "retro_workspace_init", "retro_error_string", "retro_last_cuda_error",
     "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
-    "retro_window_advance",
+    "retro_window_advance", "retro_window_advance_layers",
 ]
 
 
@@ -173,6 +173,12 @@ def retro_window_advance(desc, q_new_or_pool, step_counter, pool_steps, seq_lens
     _check(_lib().retro_window_advance(C.byref(desc), _p(q_new_or_pool), _p(step_counter), C.c_int32(pool_steps),
                                        _p(seq_lens), _p(q_win), _p(q_pos), _p(q_cur_out), _stream(stream)),
            "retro_window_advance")
+
+
+def retro_window_advance_layers(desc, table, n_layers, pool_steps, stream=None):
+    """table: device int64 tensor [n_layers][6] of device pointers (retro_advance_rec_t records)."""
+    _check(_lib().retro_window_advance_layers(C.byref(desc), _p(table), C.c_int32(n_layers), C.c_int32(pool_steps),
+                                              _stream(stream)), "retro_window_advance_layers")
 
 
 def retro_decode_step(desc, state: RetroLayerState, q_win, q_pos, q_cur, out, out_lse=None, stream=None):

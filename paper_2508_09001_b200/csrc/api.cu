@@ -176,6 +176,14 @@ int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, in
                                (cudaStream_t)stream);
 }
 
+int retro_window_advance_layers(const retro_desc_t* desc, const retro_advance_rec_t* table, int32_t n_layers,
+                                int32_t pool_steps, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(table);
+  if (n_layers < 1 || pool_steps < 1) return RETRO_ERR_ARG;
+  return launch_window_advance_layers(desc, table, n_layers, pool_steps, (cudaStream_t)stream);
+}
+
 static int check_state(const retro_desc_t* desc, const retro_layer_state_t* st) {
   if (st == nullptr) return RETRO_ERR_ARG;
   RETRO_CHECK_PTR(st->k_pages); RETRO_CHECK_PTR(st->v_pages); RETRO_CHECK_PTR(st->block_table);

@@ -164,13 +164,10 @@ int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new
 
 // ---- window ring bookkeeping: seq_lens++, q_win[slot] <- q_new, q_pos[slot] <- new position -----------
 // Single CTA (the payload is B*h_q*256 bytes).  All threads read the step counter before thread 0 bumps it.
-__global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __restrict__ q_src, int32_t* step_counter,
-                                                               int pool_steps, int32_t* seq_lens, uint4* q_win,
-                                                               int32_t* q_pos, uint4* q_cur_out, int B, int h_q,
-                                                               int rows) {
+__device__ __forceinline__ void window_advance_cta(const uint4* __restrict__ q_src, int32_t* step_counter,
+                                                   int pool_steps, int32_t* seq_lens, uint4* q_win, int32_t* q_pos,
+                                                   uint4* q_cur_out, int B, int h_q, int rows) {
   __shared__ int s_pos[64];
-  pdl_wait();
-  pdl_trigger();
   const int row_chunks = h_q * 16;   // uint4 per [h_q][d] block (a q row is 256 B)
   size_t src_off = 0;
   if (step_counter != nullptr) src_off = (size_t)(*step_counter % pool_steps) * B * row_chunks;
@@ -195,12 +192,39 @@ __global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __res
   if (threadIdx.x == 0 && step_counter != nullptr) *step_counter += 1;
 }
 
+__global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __restrict__ q_src, int32_t* step_counter,
+                                                               int pool_steps, int32_t* seq_lens, uint4* q_win,
+                                                               int32_t* q_pos, uint4* q_cur_out, int B, int h_q,
+                                                               int rows) {
+  pdl_wait();
+  pdl_trigger();
+  window_advance_cta(q_src, step_counter, pool_steps, seq_lens, q_win, q_pos, q_cur_out, B, h_q, rows);
+}
+
+// one CTA per layer record
+__global__ void __launch_bounds__(1024) window_advance_layers_kernel(const retro_advance_rec_t* __restrict__ table,
+                                                                      int pool_steps, int B, int h_q, int rows) {
+  pdl_wait();
+  pdl_trigger();
+  const retro_advance_rec_t rec = table[blockIdx.x];
+  window_advance_cta((const uint4*)rec.q_pool, rec.step_counter, pool_steps, rec.seq_lens, (uint4*)rec.q_win,
+                     rec.q_pos, (uint4*)rec.q_cur_out, B, h_q, rows);
+}
+
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
                           int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s) {
   if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
   RETRO_CUDA_TRY(launch_kernel(window_advance_kernel, dim3(1), dim3(1024), 0, s, (const uint4*)q_new_or_pool,
                                step_counter, pool_steps, seq_lens, (uint4*)q_win, q_pos, (uint4*)q_cur_out, d->batch,
                                d->num_q_heads, d->window + 1));
+  return RETRO_OK;
+}
+
+int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_t* table, int n_layers,
+                                 int pool_steps, cudaStream_t s) {
+  if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
+  RETRO_CUDA_TRY(launch_kernel(window_advance_layers_kernel, dim3(n_layers), dim3(1024), 0, s, table, pool_steps,
+                               d->batch, d->num_q_heads, d->window + 1));
   return RETRO_OK;
 }
 

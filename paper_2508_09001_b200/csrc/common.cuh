@@ -62,6 +62,8 @@ int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const 
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
 int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
                      const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s);
+int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_t* table, int n_layers,
+                                 int pool_steps, cudaStream_t s);
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
                           int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s);
 

@@ -14,7 +14,8 @@ import torch
 from . import binding as rb
 from . import workload as wl
 
-KERNELS_PER_LAYER_STEP = 6   # window_advance, page_bounds, page_score, topk_mask, attend, merge
+KERNELS_PER_LAYER_STEP = 4   # page_bounds, select_pages (score + top-k + mask), attend, merge
+KERNELS_PER_STEP = 1         # window_advance_layers: every layer's query stream advances in one launch
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -135,14 +136,19 @@ class DecodeStack:
             self.counters.append(torch.zeros(1, dtype=torch.int32, device=self.device))
             if keep_inputs:
                 self.inputs.append(inp)
+        # device table of retro_advance_rec_t records (q_pool, step_counter, seq_lens, q_win, q_pos, q_cur_out)
+        self.advance_table = torch.tensor(
+            [[pool.data_ptr(), ctr.data_ptr(), buf.seq_lens.data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(),
+              buf.q_cur.data_ptr()] for buf, pool, ctr in zip(self.layers, self.q_pools, self.counters)],
+            dtype=torch.int64, device=self.device)
         torch.cuda.synchronize(self.device)
 
     def enqueue_step(self, stream=None):
-        """One decode step of every layer: advance the synthetic query stream, then S1..S4."""
+        """One decode step: advance every layer's synthetic query stream (one launch: the stand-in for the QKV
+        projections that feed this path), then S1..S4 layer by layer."""
         d = self.desc
-        for buf, pool, ctr in zip(self.layers, self.q_pools, self.counters):
-            rb.retro_window_advance(d, pool, ctr, self.pool_steps, buf.seq_lens, buf.q_win, buf.q_pos, buf.q_cur,
-                                    stream)
+        rb.retro_window_advance_layers(d, self.advance_table, self.n_layers, self.pool_steps, stream)
+        for buf in self.layers:
             rb.retro_decode_step(d, buf.state, buf.q_win, buf.q_pos, buf.q_cur, buf.out, None, stream)
 
     def enqueue_stage(self, stage: str, stream=None):
