@@ -36,7 +36,10 @@ NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {   # profiles/r01b_summary.md: dram__bytes_read.sum + dram__bytes_write.sum per launch
+    "c2": {"attend": 4349440.0, "select": 8537088.0},
+    "c5": {"attend": 139238912.0, "select": 69750016.0},
+}
 
 
 def measured_hbm_peak():
@@ -309,11 +312,16 @@ def main():
         line["stages_us"] = stages
         line["stages_gbs"] = {k: sb[k] / (stages[k] * 1e-6) / 1e9 for k in stages}
         line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
-                            "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(dom), "peak_source": peak_src,
+                            "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload, {}).get(dom) if (args.window is None and args.budget is None) else None,
+                            "peak_source": peak_src,
                             "algorithmic_bytes_per_launch": sb[dom], "launch_us": stages[dom],
                             "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS}
         line["attend_arith_intensity_flop_per_byte"] = hs.attend_flops(cfg, seq_now) / bytes_model["kv"]
 
+        # every stage against its own algorithmic bytes (the path has two HBM streams: digests and KV pages)
+        line["stage_rooflines"] = {k: {"achieved_gbs": sb[k] / (stages[k] * 1e-6) / 1e9,
+                                       "frac": sb[k] / (stages[k] * 1e-6) / 1e9 / peak,
+                                       "algorithmic_bytes_per_launch": sb[k], "launch_us": stages[k]} for k in stages}
         if args.lite:
             line["e2e"] = None
             if ri.rank == 0:
@@ -341,6 +349,10 @@ def main():
         stack_inputs_free(stack)
         del stack
         torch.cuda.empty_cache()
+        # ---- bandwidth point: the same attend kernel where the step is large enough to be HBM-bound rather than
+        # launch/latency-bound (C5 sweep point B8, 32k context, budget 8192 tokens, w = 8; 4 layers) ----
+        if ri.rank == 0 and ri.world_size == 1 and args.workload == "c2" and args.window is None:
+            line["bandwidth_point"] = bandwidth_point(peak, dev)
         if cfg.window > 0 and not args.no_w0:
             cfg0 = workload_cfg(args.workload, n_steps=warmup + steps + 80, window=0)
             stack0, graph0, ms0 = run_stack(cfg0, L, steps, warmup, seed_off, barrier)
@@ -356,6 +368,33 @@ def main():
     if ri.world_size > 1:
         dist.destroy_process_group()
     return 0
+
+
+def bandwidth_point(peak, dev):
+    """Stage timing of the attend kernel on the C5 point (w = 8, budget 8192 tokens), 4 layers, CUDA events."""
+    import torch
+    from paper_2508_09001_b200 import harness as hs
+    from paper_2508_09001_b200 import workload as wl
+    cfg = wl.c5(8, 8192, n_steps=64)
+    n_l = 4
+    stack = hs.DecodeStack(cfg, n_l, 32)
+    for _ in range(cfg.window + 4):          # fill the retro window; leaves valid selections for the stage replay
+        stack.enqueue_step()
+    torch.cuda.synchronize()
+    g = hs.capture_graph(lambda: stack.enqueue_stage("attend"), warmup=1)
+    for _ in range(3):
+        g.replay()
+    it = 20
+    us = time_graph(g, it) * 1000.0 / (it * n_l)
+    nbytes = hs.stage_bytes(cfg, stack.seq_lens_host())["attend"]
+    out = {"workload": cfg.name, "kernel": "attend", "bound": "hbm", "launch_us": us,
+           "algorithmic_bytes_per_launch": nbytes, "achieved": nbytes / (us * 1e-6) / 1e9, "peak": peak, "unit": "GB/s",
+           "frac": nbytes / (us * 1e-6) / 1e9 / peak,
+           "frac_of_nominal_8TBs": nbytes / (us * 1e-6) / 1e9 / NOMINAL_HBM_GBS,
+           "l2": "4 layers x 268 MB of selected pages, one launch per layer: every launch reads from HBM"}
+    del g, stack
+    torch.cuda.empty_cache()
+    return out
 
 
 def stack_inputs_free(stack):
