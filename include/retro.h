@@ -179,6 +179,15 @@ int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* 
                            const void* host_q_new, const void* host_k_new, const void* host_v_new,
                            void* host_out, void* stream);
 
+/* NEXT-1: UpdateKV of Alg. 1 line 2 (Sec. 2.4): overwrite the K
+ * and V rows of up to n_upd past tokens per sequence with the caller's re-embedded K^, V^.
+ * positions [B][n_upd] int32 (-1 or >= seq_len: skipped), k_hat / v_hat [B][n_upd][h_k][d] T, all DEVICE.
+ * The digests of the touched pages become stale: follow with
+ * retro_update_page_bounds(pos_begin = oldest overwritten position, max_touched_pages = ceil(w / P) + 1). */
+int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_hat, const int32_t* positions,
+                    int32_t n_upd /*HOST*/, const int32_t* block_table, const int32_t* seq_lens, void* k_pages,
+                    void* v_pages, void* stream);
+
 /* Window-ring bookkeeping used by the two calls above and by the synthetic benchmark: seq_lens[b] += 1;
  * row (new position mod (w+1)) of q_win <- q_new[b], q_pos <- new position.  q_new [B][h_q][d] T.
  * If step_counter != NULL, q_new is taken as q_pool[(*step_counter) % pool_steps] ([pool][B][h_q][d]) and the

@@ -18,6 +18,7 @@ mask A / list M | Alg. 2; Sec. C.2 PAPER.md:448 | select_pages
 attention       | Eq. 2 / 6 / 7; Alg.1 l.6  | sparse_attend
 merge           | Eq. 8-9; Alg. 1 l.7           | merge_partials, merge_output_cache
 output cache    | Sec. 2.3 push/update/pop PAPER.md:83-85; l.8    | merge_output_cache
+KV overwrite    | Alg. 1 l.2 UpdateKV PAPER.md:391; Sec. 2.4 :87-93 | update_kv (+ update_page_bounds)
 
 Readings of silent / garbled passages (full list with reasons in DESIGN.md "Readings"):
   Q2  GQA: per-q-head Eq. 1 scores are SUMMED over the q heads of a KV head (flag: max).
@@ -99,6 +100,26 @@ def update_page_bounds(desc, k_pages, block_table, seq_lens, pos_begin, bounds):
                 bounds[b, h, j, 0, :] = keys.max(axis=0)       # Kmax
                 bounds[b, h, j, 1, :] = keys.min(axis=0)       # Kmin
     return bounds
+
+
+# --------------------------------------------------------------------------------------------
+# UpdateKV (Alg. 1 line 2; Sec. 2.4): "overwrite stale KV entries" of the past
+# window tokens with their re-embedded K^, V^.  The digests of the touched pages are then stale too: the caller
+# refreshes them with update_page_bounds(pos_begin = oldest overwritten position).
+# --------------------------------------------------------------------------------------------
+def update_kv(desc, k_pages, v_pages, block_table, seq_lens, positions, k_hat, v_hat):
+    """positions [B][n_upd] (-1 = skip; must be < seq_len), k_hat / v_hat [B][n_upd][h_k][d].  In place."""
+    P = desc.page_size
+    for b in range(desc.batch):
+        for u in range(positions.shape[1]):
+            pos = int(positions[b, u])
+            if pos < 0 or pos >= int(seq_lens[b]):
+                continue
+            phys = int(block_table[b, pos // P])
+            for h in range(desc.num_kv_heads):
+                k_pages[phys, h, pos % P, :] = k_hat[b, u, h, :]
+                v_pages[phys, h, pos % P, :] = v_hat[b, u, h, :]
+    return k_pages, v_pages
 
 
 # --------------------------------------------------------------------------------------------

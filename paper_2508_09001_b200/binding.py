@@ -23,7 +23,7 @@ EXPORTED = [
     "retro_workspace_bytes", "retro_workspace_init", "retro_error_string", "retro_last_cuda_error",
     "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
-    "retro_window_advance", "retro_window_advance_layers",
+    "retro_window_advance", "retro_window_advance_layers", "retro_update_kv",
 ]
 
 
@@ -173,6 +173,14 @@ def retro_window_advance(desc, q_new_or_pool, step_counter, pool_steps, seq_lens
     _check(_lib().retro_window_advance(C.byref(desc), _p(q_new_or_pool), _p(step_counter), C.c_int32(pool_steps),
                                        _p(seq_lens), _p(q_win), _p(q_pos), _p(q_cur_out), _stream(stream)),
            "retro_window_advance")
+
+
+def retro_update_kv(desc, k_hat, v_hat, positions, block_table, seq_lens, k_pages, v_pages, stream=None):
+    """UpdateKV (Alg. 1 line 2): k_hat / v_hat [B][n_upd][h_k][d], positions [B][n_upd] int32 (-1 = skip)."""
+    n_upd = int(positions.shape[1])
+    _check(_lib().retro_update_kv(C.byref(desc), _p(k_hat), _p(v_hat), _p(positions), C.c_int32(n_upd),
+                                  _p(block_table), _p(seq_lens), _p(k_pages), _p(v_pages), _stream(stream)),
+           "retro_update_kv")
 
 
 def retro_window_advance_layers(desc, table, n_layers, pool_steps, stream=None):

@@ -176,6 +176,17 @@ int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, in
                                (cudaStream_t)stream);
 }
 
+int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_hat, const int32_t* positions,
+                    int32_t n_upd, const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
+                    void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(k_hat); RETRO_CHECK_PTR(v_hat); RETRO_CHECK_PTR(positions); RETRO_CHECK_PTR(block_table);
+  RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
+  if (n_upd < 1) return RETRO_ERR_ARG;
+  return launch_update_kv(desc, k_hat, v_hat, positions, n_upd, block_table, seq_lens, k_pages, v_pages,
+                          (cudaStream_t)stream);
+}
+
 int retro_window_advance_layers(const retro_desc_t* desc, const retro_advance_rec_t* table, int32_t n_layers,
                                 int32_t pool_steps, void* stream) {
   RETRO_CHECK_DESC(desc);

@@ -162,6 +162,44 @@ int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new
   return RETRO_OK;
 }
 
+// ---- UpdateKV (Alg. 1 line 2; Sec. 2.4): overwrite the rows of past tokens with K^, V^ ----------
+template <typename T, int D, int P>
+__global__ void update_kv_kernel(const T* __restrict__ k_hat, const T* __restrict__ v_hat,
+                                 const int32_t* __restrict__ positions, const int32_t* __restrict__ block_table,
+                                 const int32_t* __restrict__ seq_lens, T* __restrict__ k_pages,
+                                 T* __restrict__ v_pages, int B, int n_upd, int h_k, int max_pages) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;   // one 16 B chunk each: [B][n_upd][h_k][2][16]
+  pdl_wait();
+  pdl_trigger();
+  if (idx >= B * n_upd * h_k * 32) return;
+  const int col = idx & 15, kv = (idx >> 4) & 1, h = (idx >> 5) % h_k;
+  const int u = (idx / (32 * h_k)) % n_upd, b = idx / (32 * h_k * n_upd);
+  const int pos = positions[b * n_upd + u];
+  if (pos < 0 || pos >= seq_lens[b] || pos / P >= max_pages) return;
+  const int phys = block_table[(size_t)b * max_pages + pos / P];
+  const T* src = (kv ? v_hat : k_hat) + (((size_t)b * n_upd + u) * h_k + h) * D;
+  T* dst = (kv ? v_pages : k_pages) + (((size_t)phys * h_k + h) * P + pos % P) * D;
+  reinterpret_cast<uint4*>(dst)[col] = reinterpret_cast<const uint4*>(src)[col];
+}
+
+int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat, const int32_t* positions, int n_upd,
+                     const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
+                     cudaStream_t s) {
+  const int n = d->batch * n_upd * d->num_kv_heads * 32;
+  const int block = 128, grid = ceil_div(n, block);
+  if (d->dtype == RETRO_BF16) {
+    RETRO_CUDA_TRY(launch_kernel(update_kv_kernel<__nv_bfloat16, 128, 16>, dim3(grid), dim3(block), 0, s,
+                                 (const __nv_bfloat16*)k_hat, (const __nv_bfloat16*)v_hat, positions, block_table,
+                                 seq_lens, (__nv_bfloat16*)k_pages, (__nv_bfloat16*)v_pages, d->batch, n_upd,
+                                 d->num_kv_heads, d->max_pages_per_seq));
+  } else {
+    RETRO_CUDA_TRY(launch_kernel(update_kv_kernel<float, 64, 16>, dim3(grid), dim3(block), 0, s, (const float*)k_hat,
+                                 (const float*)v_hat, positions, block_table, seq_lens, (float*)k_pages,
+                                 (float*)v_pages, d->batch, n_upd, d->num_kv_heads, d->max_pages_per_seq));
+  }
+  return RETRO_OK;
+}
+
 // ---- window ring bookkeeping: seq_lens++, q_win[slot] <- q_new, q_pos[slot] <- new position -----------
 // Single CTA (the payload is B*h_q*256 bytes).  All threads read the step counter before thread 0 bumps it.
 __device__ __forceinline__ void window_advance_cta(const uint4* __restrict__ q_src, int32_t* step_counter,

@@ -62,6 +62,9 @@ int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const 
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
 int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
                      const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s);
+int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat, const int32_t* positions, int n_upd,
+                     const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
+                     cudaStream_t s);
 int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_t* table, int n_layers,
                                  int pool_steps, cudaStream_t s);
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,

@@ -6,6 +6,7 @@ import numpy as np
 import pytest
 import torch
 
+from oracle import retro_oracle as orc
 from paper_2508_09001_b200 import binding as rb
 from paper_2508_09001_b200 import workload as wl
 from tests import gpu_harness as GH
@@ -157,6 +158,37 @@ def test_append_kv_and_window_advance_match_pregenerated_pool():
         assert torch.equal(buf.q_win.cpu()[q_pos >= 0], q_win[q_pos >= 0])
         assert torch.equal(buf.q_cur.cpu(), inp.q_all[s])
     assert torch.equal(buf.k_pages, ref_k) and torch.equal(buf.v_pages, ref_v)
+
+
+def test_update_kv_overwrite_and_digest_refresh_match_oracle():
+    """NEXT-1: retro_update_kv + retro_update_page_bounds(pos_begin = t - w) against the oracle, bit-exact."""
+    cfg = wl.shrink(wl.c2(), (300, 77), 4, window=8, budget_tokens=128, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    L = torch.tensor([303, 80], dtype=torch.int32)
+    buf.seq_lens.copy_(L)
+    buf.rebuild_bounds()
+    layer = H.oracle_layer(inp)
+    layer.prefill_bounds(L.numpy())
+    g = torch.Generator().manual_seed(11)
+    w = cfg.window
+    positions = torch.stack([torch.arange(int(l) - 1 - w, int(l) - 1, dtype=torch.int32) for l in L])   # t-w .. t-1
+    positions[1, 2] = -1
+    k_hat = torch.randn((2, w, cfg.num_kv_heads, cfg.head_dim), generator=g).to(torch.bfloat16)
+    v_hat = torch.randn((2, w, cfg.num_kv_heads, cfg.head_dim), generator=g).to(torch.bfloat16)
+    rb.retro_update_kv(desc, k_hat.cuda(), v_hat.cuda(), positions.cuda(), buf.block_table, buf.seq_lens,
+                       buf.k_pages, buf.v_pages)
+    pos_begin = (L - 1 - w).to(torch.int32).cuda()
+    rb.retro_update_page_bounds(desc, buf.k_pages, buf.block_table, buf.seq_lens, pos_begin, 2, buf.bounds)
+    torch.cuda.synchronize()
+    orc.update_kv(layer.desc, layer.k_pages, layer.v_pages, layer.block_table, L.numpy(), positions.numpy(),
+                  k_hat.double().numpy(), v_hat.double().numpy())
+    orc.update_page_bounds(layer.desc, layer.k_pages, layer.block_table, L.numpy(), (L - 1 - w).numpy(), layer.bounds)
+    assert np.array_equal(buf.k_pages.double().cpu().numpy(), layer.k_pages)
+    assert np.array_equal(buf.v_pages.double().cpu().numpy(), layer.v_pages)
+    for b in range(2):
+        n = -(-int(L[b]) // 16)
+        assert np.array_equal(buf.bounds[b, :, :n].double().cpu().numpy(), layer.bounds[b, :, :n])
 
 
 def _to_cpu(inp):

@@ -382,3 +382,44 @@ def test_effective_budget_grows_with_window():
         fb.select(m)
     own = len(fb.seen(2, 2, 0)); grown = len(fb.seen(2, 6, 0))
     assert own == 6 and own <= grown <= 6 * 5
+
+
+# ------------------------------------------------------------------------------- NEXT-1 UpdateKV
+def test_update_kv_overwrites_exactly_the_named_rows_and_digests_follow():
+    """Catches: wrong block-table indirection or in-page offset, K/V swapped, head stride, skipped -1 entries
+    being written, and digests not following the overwrite (incremental refresh == bulk recompute)."""
+    cfg = wl.shrink(wl.c2(), (45,), 4, window=3, budget_tokens=64, num_q_heads=4, num_kv_heads=2, head_dim=8)
+    inp = wl.make_layer_inputs(cfg)
+    layer = H.oracle_layer(inp)
+    L = 47
+    seq = np.array([L])
+    layer.prefill_bounds(seq)
+    k0, v0 = H.seq_tokens(inp, 0, L)
+    rng = np.random.default_rng(3)
+    positions = np.array([[44, -1, 46, 31]], dtype=np.int32)          # two pages, one skipped entry
+    # the oracle layer holds the pools as float32 arrays: use float32-representable replacement rows
+    k_hat = rng.standard_normal((1, 4, cfg.num_kv_heads, cfg.head_dim)).astype(np.float32).astype(np.float64)
+    v_hat = rng.standard_normal((1, 4, cfg.num_kv_heads, cfg.head_dim)).astype(np.float32).astype(np.float64)
+    orc.update_kv(layer.desc, layer.k_pages, layer.v_pages, layer.block_table, seq, positions, k_hat, v_hat)
+    # plain definition on the logical token sequence
+    k1, v1 = k0.copy(), v0.copy()
+    for u, pos in enumerate(positions[0]):
+        if pos >= 0:
+            k1[pos], v1[pos] = k_hat[0, u], v_hat[0, u]
+    P = cfg.page_size
+    for l in range(L):
+        phys = int(layer.block_table[0, l // P])
+        assert np.array_equal(layer.k_pages[phys, :, l % P], k1[l])
+        assert np.array_equal(layer.v_pages[phys, :, l % P], v1[l])
+    # digests: refresh from the oldest overwritten position, compare with brute force over every page
+    orc.update_page_bounds(layer.desc, layer.k_pages, layer.block_table, seq, np.array([31]), layer.bounds)
+    for j in range(-(-L // P)):
+        rows = k1[j * P:min((j + 1) * P, L)]
+        assert np.array_equal(layer.bounds[0, :, j, 0], rows.max(axis=0))
+        assert np.array_equal(layer.bounds[0, :, j, 1], rows.min(axis=0))
+    # overwriting rows with their own values is the identity
+    before = layer.k_pages.copy()
+    same = np.stack([k1[[44, 46]]])
+    orc.update_kv(layer.desc, layer.k_pages, layer.v_pages, layer.block_table, seq, np.array([[44, 46]]),
+                  same, np.stack([v1[[44, 46]]]))
+    assert np.array_equal(layer.k_pages, before)
