@@ -60,6 +60,23 @@ def test_c5_shape_shrunk_sweep_points(w, budget):
     print("c5s errs", w, budget, GH.lockstep(inp, w + 6))
 
 
+@pytest.mark.parametrize("name,kw", [
+    ("c2", dict(prompt_lens=(1003,), n_steps=14)),                                   # 8 splits per unit
+    ("c5w8", dict(prompt_lens=(1500, 1490, 1333), n_steps=14, batch=3)),             # 8 KV heads x 3 sequences
+    ("c5w0", dict(prompt_lens=(1500, 1490), n_steps=5, batch=2, window=0)),          # plain Quest, no cache
+    ("c5w32", dict(prompt_lens=(1500, 1490), n_steps=38, batch=2, window=32, budget_tokens=512)),   # 2 row groups
+    ("c4", dict(prompt_lens=(3001, 2990), n_steps=12, batch=2, budget_tokens=512)),  # GQA 7
+])
+def test_whole_step_entry_point_bf16(name, kw):
+    """retro_decode_step (the call bench.py captures into its graph) against the oracle: selections bit-exact,
+    out / out_lse / cache within tolerance, every step, no teacher forcing."""
+    base = {"c2": wl.c2(), "c5w8": wl.c5(8, 1024), "c5w0": wl.c5(0, 1024), "c5w32": wl.c5(32, 512), "c4": wl.c4()}[name]
+    kw = dict(kw)
+    cfg = wl.shrink(base, kw.pop("prompt_lens"), kw.pop("n_steps"), **kw)
+    inp = wl.make_layer_inputs(cfg)
+    print("whole-step errs", name, GH.lockstep(inp, cfg.n_steps, use_decode_step=True))
+
+
 def test_multi_block_splits_shrunk():
     """32 units x 128 pages: every attend CTA walks several 128-key blocks (ring reuse, lazy rescale, P buffers)."""
     cfg = wl.shrink(wl.c5(8, 2048), (2500, 2491, 2333, 2100), 12, batch=4)
@@ -110,6 +127,13 @@ def test_c2_full_context_sampled_steps():
     inp = wl.make_layer_inputs(cfg, device="cuda")
     inp = _to_cpu(inp)
     print("c2 full errs", GH.lockstep(inp, 12))
+
+
+def test_c2_full_context_whole_step_entry_point():
+    """FULL C2 through retro_decode_step, exactly the call bench.py captures into its graph."""
+    cfg = wl.c2(n_steps=11)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c2 full whole-step errs", GH.lockstep(inp, 11, use_decode_step=True))
 
 
 def test_c4_full_context_sampled_steps():
