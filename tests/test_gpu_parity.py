@@ -96,6 +96,20 @@ def test_edge_single_page_and_budget_one():
     GH.lockstep(inp, 14)
 
 
+def test_edge_budget_zero_selects_nothing():
+    """budget 0: empty page lists, every partial is (0, -inf), outputs are zeros / -inf (window ramp-up included)."""
+    cfg = wl.shrink(wl.c2(), (200,), 5, budget_tokens=16, window=2)
+    inp = wl.make_layer_inputs(cfg)
+    GH.lockstep(inp, 5, budget_pages=0, k_max=4)
+
+
+def test_edge_max_group_and_window_three_row_groups():
+    """G = 8 with w = 32: 264 query rows per KV head = three row groups of 88 rows in the tensor-core kernel."""
+    cfg = wl.shrink(wl.c5(32, 512), (900, 890), 36, batch=2, num_q_heads=16, num_kv_heads=2)
+    inp = wl.make_layer_inputs(cfg)
+    print("G8 w32 errs", GH.lockstep(inp, 36))
+
+
 def test_edge_pure_topk_and_group_max():
     cfg = wl.shrink(wl.c2(), (777,), 12, budget_tokens=128, window=4)
     inp = wl.make_layer_inputs(cfg)
