@@ -217,12 +217,11 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, c
   const WorkspaceLayout wl = workspace_layout(desc);
   if (st->workspace_bytes < wl.total) return RETRO_ERR_WORKSPACE;
   cudaStream_t s = (cudaStream_t)stream;
-  // S1: the newest token's page.  pos_begin = seq_len - 1 is expressed by passing seq_lens with a -1 bias:
-  // the bounds kernel takes pos_begin from an array, so the per-step path uses the dedicated "tail" mode.
-  rc = launch_update_page_bounds(desc, st->k_pages, st->block_table, st->seq_lens, nullptr, 1, st->bounds, s);
-  if (rc != RETRO_OK) return rc;
+  // S1 + S2: the digest of the newest token's page is rebuilt inside the select kernel (by the warp that scores
+  // that page) and written back, so the step needs no separate digest launch.
   rc = launch_select_pages(desc, wl, q_cur, st->bounds, st->seq_lens, st->budget_pages, st->last_loaded,
-                           st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s);
+                           st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s, st->k_pages,
+                           st->block_table);
   if (rc != RETRO_OK) return rc;
   rc = launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
                             st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s);

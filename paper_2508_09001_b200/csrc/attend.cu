@@ -283,8 +283,8 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
   prm.nrg = 1;
   prm.rg_rows = wl.rows;
   if (d->dtype == RETRO_BF16) {
-    // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu).  The scalar
-    // path stays reachable for debugging (RETRO_ATTEND_PATH=simt) and for row blocks above one 128-row tile.
+    // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu; more than 128
+    // rows run as row groups).  The scalar path stays reachable for debugging (RETRO_ATTEND_PATH=simt).
     static const bool force_simt = [] {
       const char* e = std::getenv("RETRO_ATTEND_PATH");
       return e != nullptr && e[0] == 's';

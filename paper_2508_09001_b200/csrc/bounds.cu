@@ -5,52 +5,9 @@
 // P*d*esize contiguous bytes; the warp streams it with 128-bit loads (a row of 256 B = 16 lanes), reduces
 // across the two half-warps with one shuffle and writes the [Kmax;Kmin] record (512 B) with 128-bit stores.
 #include "common.cuh"
+#include "digest.cuh"
 
 namespace retro {
-
-template <typename T> struct Vec16;
-template <> struct Vec16<float> {
-  __device__ static __forceinline__ uint4 vmax(uint4 a, uint4 b) {
-    uint4 r;
-    r.x = __float_as_uint(fmaxf(__uint_as_float(a.x), __uint_as_float(b.x)));
-    r.y = __float_as_uint(fmaxf(__uint_as_float(a.y), __uint_as_float(b.y)));
-    r.z = __float_as_uint(fmaxf(__uint_as_float(a.z), __uint_as_float(b.z)));
-    r.w = __float_as_uint(fmaxf(__uint_as_float(a.w), __uint_as_float(b.w)));
-    return r;
-  }
-  __device__ static __forceinline__ uint4 vmin(uint4 a, uint4 b) {
-    uint4 r;
-    r.x = __float_as_uint(fminf(__uint_as_float(a.x), __uint_as_float(b.x)));
-    r.y = __float_as_uint(fminf(__uint_as_float(a.y), __uint_as_float(b.y)));
-    r.z = __float_as_uint(fminf(__uint_as_float(a.z), __uint_as_float(b.z)));
-    r.w = __float_as_uint(fminf(__uint_as_float(a.w), __uint_as_float(b.w)));
-    return r;
-  }
-};
-template <> struct Vec16<__nv_bfloat16> {
-  __device__ static __forceinline__ uint32_t max2(uint32_t a, uint32_t b) {
-    __nv_bfloat162 r = __hmax2(*reinterpret_cast<__nv_bfloat162*>(&a), *reinterpret_cast<__nv_bfloat162*>(&b));
-    return *reinterpret_cast<uint32_t*>(&r);
-  }
-  __device__ static __forceinline__ uint32_t min2(uint32_t a, uint32_t b) {
-    __nv_bfloat162 r = __hmin2(*reinterpret_cast<__nv_bfloat162*>(&a), *reinterpret_cast<__nv_bfloat162*>(&b));
-    return *reinterpret_cast<uint32_t*>(&r);
-  }
-  __device__ static __forceinline__ uint4 vmax(uint4 a, uint4 b) {
-    return make_uint4(max2(a.x, b.x), max2(a.y, b.y), max2(a.z, b.z), max2(a.w, b.w));
-  }
-  __device__ static __forceinline__ uint4 vmin(uint4 a, uint4 b) {
-    return make_uint4(min2(a.x, b.x), min2(a.y, b.y), min2(a.z, b.z), min2(a.w, b.w));
-  }
-};
-
-__device__ __forceinline__ uint4 shfl_xor_u4(uint4 v, int m) {
-  v.x = __shfl_xor_sync(0xffffffffu, v.x, m);
-  v.y = __shfl_xor_sync(0xffffffffu, v.y, m);
-  v.z = __shfl_xor_sync(0xffffffffu, v.z, m);
-  v.w = __shfl_xor_sync(0xffffffffu, v.w, m);
-  return v;
-}
 
 // Row of D elements = kRowBytes; 16 lanes cover 256 B.  Instantiated for rows of exactly 256 B
 // ({f32, d64} and {bf16, d128}): two rows per warp pass.
@@ -79,34 +36,9 @@ __global__ void __launch_bounds__(128) page_bounds_kernel(const T* __restrict__ 
   const int n_valid = min(P, L - j * P);
   const int phys = block_table[(size_t)b * max_pages + j];
   const uint4* tile = reinterpret_cast<const uint4*>(k_pages + ((size_t)phys * h_k + h) * P * D);
-  const int sub = lane >> 4;   // which of the two rows of a pass
-  const int col = lane & 15;   // 16-byte column within the row
-  uint4 vmax = make_uint4(0, 0, 0, 0), vmin = make_uint4(0, 0, 0, 0);
-  bool have = false;
-#pragma unroll
-  for (int r0 = 0; r0 < P; r0 += 2) {
-    const int row = r0 + sub;
-    if (row < n_valid) {
-      const uint4 v = __ldg(tile + row * 16 + col);
-      if (!have) {
-        vmax = v; vmin = v; have = true;
-      } else {
-        vmax = Vec16<T>::vmax(vmax, v);
-        vmin = Vec16<T>::vmin(vmin, v);
-      }
-    }
-  }
-  // combine the two half-warps; the odd half may be empty when n_valid == 1
-  uint4 omax = shfl_xor_u4(vmax, 16), omin = shfl_xor_u4(vmin, 16);
-  const bool ohave = __shfl_xor_sync(0xffffffffu, (int)have, 16) != 0;
-  if (have && ohave) {
-    vmax = Vec16<T>::vmax(vmax, omax);
-    vmin = Vec16<T>::vmin(vmin, omin);
-  } else if (!have) {
-    vmax = omax; vmin = omin;
-  }
+  const uint4 mine = warp_page_digest<T, P>(tile, n_valid, lane);
   uint4* rec = reinterpret_cast<uint4*>(bounds + (((size_t)b * h_k + h) * max_pages + j) * 2 * D);
-  rec[lane] = sub == 0 ? vmax : vmin;   // lanes 0..15 -> Kmax (256 B), lanes 16..31 -> Kmin (256 B)
+  rec[lane] = mine;   // lanes 0..15 -> Kmax (256 B), lanes 16..31 -> Kmin (256 B)
 }
 
 int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const int32_t* block_table,

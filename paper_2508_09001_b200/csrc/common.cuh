@@ -52,7 +52,8 @@ int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const 
 int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
                         const int32_t* seq_lens, const int32_t* budget_pages, int32_t* last_loaded,
                         int32_t* sel_pages, int32_t* sel_prev, int32_t* sel_count, double* scores_out,
-                        void* workspace, cudaStream_t s);
+                        void* workspace, cudaStream_t s, const void* k_pages_refresh = nullptr,
+                        const int32_t* block_table = nullptr);   // k_pages_refresh: S1 of the newest page in line
 int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_win, const int32_t* q_pos,
                          const void* k_pages, const void* v_pages, const int32_t* block_table,
                          const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,

@@ -14,6 +14,7 @@
 // ascending page indices with ties resolved to the lower index, and the same pass does Alg. 2's
 // M.append(A[p]); A[p] <- t.
 #include "common.cuh"
+#include "digest.cuh"
 
 namespace retro {
 
@@ -252,11 +253,14 @@ __device__ __forceinline__ void topk_mask_block(
 
 template <typename T, int D, bool kGroupMax>
 __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
-    const T* __restrict__ q_cur, const T* __restrict__ bounds, const int32_t* __restrict__ seq_lens,
+    const T* __restrict__ q_cur, const T* bounds, const int32_t* __restrict__ seq_lens,
     const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
     int32_t* __restrict__ sel_prev, int32_t* __restrict__ sel_count, double* scores, double* __restrict__ scores_out,
     unsigned int* counters, int h_q, int h_k, int max_pages, int k_max, int P, int group_reduce, int force_last,
-    int pages_per_cta /*multiple of kPagesPerCta*/) {
+    int pages_per_cta /*multiple of kPagesPerCta*/,
+    // S1 in line (retro_decode_step): the warp that owns the newest page recomputes its digest from the K tile,
+    // patches the staged record and writes it back to `bounds`.  k_pages == NULL: digests are up to date.
+    const T* __restrict__ k_pages, const int32_t* __restrict__ block_table, T* bounds_out) {
   static_assert(2 * D * sizeof(T) == 512, "digest record must be 512 bytes");
   constexpr int kVals = Rec<T>::kVals;
   // digest ring [kStages][64 records x 512 B]; the unit's last CTA reuses it for the top-k keys
@@ -301,6 +305,17 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     fence_mbar_init();
     for (int it = 0; it < min(kStages, nbatch); ++it) issue_batch(it);
   }
+  // S1 in line: the warp that will reduce the newest page (j_last) rebuilds its digest while the first batches fly
+  const int j_last = n_pages - 1;
+  const bool own_last = k_pages != nullptr && j_last >= cta_page0 && j_last < page_end &&
+                        ((j_last - cta_page0) % kPagesPerCta) / kPagesPerWarp == warp;   // warp-uniform
+  uint4 fresh = make_uint4(0, 0, 0, 0);
+  if (own_last) {
+    const int phys = block_table[(size_t)b * max_pages + j_last];
+    const uint4* tile = reinterpret_cast<const uint4*>(k_pages + ((size_t)phys * h_k + h) * P * D);
+    fresh = warp_page_digest<T, 16>(tile, seq_lens[b] - j_last * P, lane);
+    reinterpret_cast<uint4*>(bounds_out + (row + j_last) * 2 * D)[lane] = fresh;
+  }
   // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
   for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) {
     const int c = i % D;
@@ -320,6 +335,10 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
   auto reduce_store = [&](const unsigned char* stage, int page0) {
     const int jbase = page0 + warp * kPagesPerWarp;
     const uint4* rec = reinterpret_cast<const uint4*>(stage) + warp * kPagesPerWarp * 32 + lane;
+    if (own_last && j_last >= page0 && j_last < page0 + kPagesPerCta) {   // patch the staged (stale) record
+      reinterpret_cast<uint4*>(const_cast<unsigned char*>(stage))[(j_last - page0) * 32 + lane] = fresh;
+      __syncwarp();
+    }
     double acc[kPagesPerWarp];
     if constexpr (!kGroupMax) {
 #pragma unroll
@@ -425,7 +444,7 @@ extern "C" int retro_debug_read_sel_stamps(unsigned long long* host_out) {
 int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
                         const int32_t* seq_lens, const int32_t* budget_pages, int32_t* last_loaded,
                         int32_t* sel_pages, int32_t* sel_prev, int32_t* sel_count, double* scores_out,
-                        void* workspace, cudaStream_t s) {
+                        void* workspace, cudaStream_t s, const void* k_pages_refresh, const int32_t* block_table) {
   char* ws = static_cast<char*>(workspace);
   double* scores = reinterpret_cast<double*>(ws + wl.scores_off);
   unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off);   // [units] score-chunk arrivals
@@ -442,6 +461,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   const size_t keys_bytes = (size_t)d->max_pages_per_seq * sizeof(uint64_t);
   const size_t smem = keys_bytes > (size_t)kStages * kStageBytes ? keys_bytes : (size_t)kStages * kStageBytes;
   auto launch = [&](auto kern, auto* qp, auto* bp) -> int {
+    auto* bw = bp;   // the same digest array, writable for the in-line S1 refresh
     // raise the dynamic shared-memory limit once per kernel instantiation (not a stream operation)
     static const void* raised[8];
     static size_t raised_to[8];
@@ -457,7 +477,8 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
     RETRO_CUDA_TRY(launch_kernel(kern, grid, dim3(kScoreWarps * 32), smem, s, qp, bp, seq_lens, budget_pages,
                                  last_loaded, sel_pages, sel_prev, sel_count, scores, scores_out, counters,
                                  d->num_q_heads, d->num_kv_heads, d->max_pages_per_seq, d->max_sel_pages,
-                                 d->page_size, d->group_reduce, d->force_last_page, pages_per_cta));
+                                 d->page_size, d->group_reduce, d->force_last_page, pages_per_cta,
+                                 (decltype(qp))k_pages_refresh, block_table, const_cast<decltype(bw)>(bw)));
     return RETRO_OK;
   };
   const bool gmax = d->group_reduce == RETRO_GROUP_MAX;

@@ -14,7 +14,7 @@ import torch
 from . import binding as rb
 from . import workload as wl
 
-KERNELS_PER_LAYER_STEP = 4   # page_bounds, select_pages (score + top-k + mask), attend, merge
+KERNELS_PER_LAYER_STEP = 3   # select_pages (newest digest + score + top-k + mask), attend, merge
 KERNELS_PER_STEP = 1         # window_advance_layers: every layer's query stream advances in one launch
 
 

@@ -142,6 +142,10 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
             # whole-step entry point: no teacher forcing possible, so only used where selections are tie-free
             rb.retro_decode_step(desc, buf.state, buf.q_win, buf.q_pos, buf.q_cur, buf.out, buf.out_lse)
             torch.cuda.synchronize()
+            g_bounds = buf.bounds.float().cpu().numpy()      # S1 runs inside the select kernel on this path
+            for b in range(B):
+                j = (int(seq_lens[b]) - 1) // cfg.page_size
+                assert np.array_equal(g_bounds[b, :, j], layer.bounds[b, :, j].astype(np.float32)), "digest of newest page"
             assert np.array_equal(buf.sel_pages.cpu().numpy(), res["sel_pages"])
             if cfg.window > 0:      # w = 0: no past rows, the mask list is not used (A is optional there)
                 assert np.array_equal(buf.sel_prev.cpu().numpy(), res["sel_prev"])
