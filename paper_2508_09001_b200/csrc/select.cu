@@ -278,6 +278,14 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
   pdl_trigger();
   const int b = blockIdx.z, h = blockIdx.y;
   const int G = h_q / h_k;
+  // the group's query values go out together with the length: the first round trip covers both (blockDim = 2 D)
+  T q_raw[kMaxGroup];
+  {
+    const int c = threadIdx.x % D;
+#pragma unroll
+    for (int g = 0; g < kMaxGroup; ++g)
+      if (g < G) q_raw[g] = q_cur[((size_t)b * h_q + h * G + g) * D + c];
+  }
   const int n_pages = (seq_lens[b] + P - 1) / P;
   const int cta_page0 = blockIdx.x * pages_per_cta;
   const size_t row = ((size_t)b * h_k + h) * max_pages;
@@ -317,14 +325,18 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     reinterpret_cast<uint4*>(bounds_out + (row + j_last) * 2 * D)[lane] = fresh;
   }
   // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
-  for (int i = threadIdx.x; i < 2 * D; i += blockDim.x) {
-    const int c = i % D;
+  static_assert(kScoreWarps * 32 == 2 * D || kScoreWarps * 32 == 4 * D, "one thread per element of [q+ ; q-]");
+  if (threadIdx.x < 2 * D) {
+    const int i = threadIdx.x;
     const bool neg = i >= D;
     double acc = 0.0;
-    for (int g = 0; g < G; ++g) {
-      const double qv = (double)Elem<T>::to_f32(q_cur[((size_t)b * h_q + h * G + g) * D + c]);
-      const double part = neg ? fmin(qv, 0.0) : fmax(qv, 0.0);
-      if (!kGroupMax) acc += part; else s_q[g][i] = part;
+#pragma unroll
+    for (int g = 0; g < kMaxGroup; ++g) {
+      if (g < G) {
+        const double qv = (double)Elem<T>::to_f32(q_raw[g]);
+        const double part = neg ? fmin(qv, 0.0) : fmax(qv, 0.0);
+        if (!kGroupMax) acc += part; else s_q[g][i] = part;
+      }
     }
     if (!kGroupMax) s_q[0][i] = acc;
   }
