@@ -65,9 +65,10 @@ __device__ __forceinline__ uint64_t order_key(double s) {
 }
 
 // exclusive block scan of one int per thread (NT threads, NT / 32 <= 32 warps); returns the exclusive prefix,
-// *total = block sum
+// *total = block sum.  One barrier per call: the warp totals alternate between two buffers (`phase` counts the
+// calls), so a buffer is rewritten only after every thread has passed the barrier of the call in between.
 template <int NT>
-__device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int* total) {
+__device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[2][32]*/, int* total, int& phase) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   int inc = v;
 #pragma unroll
@@ -75,23 +76,19 @@ __device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[33]*/, int*
     const int n = __shfl_up_sync(0xffffffffu, inc, o);
     if (lane >= o) inc += n;
   }
-  __syncthreads();   // protect s_warp reuse
-  if (lane == 31) s_warp[warp] = inc;
+  int* buf = s_warp + (phase & 1) * 32;
+  ++phase;
+  if (lane == 31) buf[warp] = inc;
   __syncthreads();
-  if (warp == 0) {
-    int w = lane < NT / 32 ? s_warp[lane] : 0;
-    int winc = w;
+  int before = 0, sum = 0;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int n = __shfl_up_sync(0xffffffffu, winc, o);
-      if (lane >= o) winc += n;
-    }
-    s_warp[lane] = winc - w;
-    if (lane == 31) s_warp[32] = winc;
+  for (int w = 0; w < NT / 32; ++w) {
+    const int tw = buf[w];
+    before += w < warp ? tw : 0;
+    sum += tw;
   }
-  __syncthreads();
-  *total = s_warp[32];
-  return s_warp[warp] + inc - v;
+  *total = sum;
+  return before + inc - v;
 }
 
 // Executed by all NT threads of one CTA for unit (b, h); scores are read through L2 (written by other CTAs).
@@ -103,7 +100,8 @@ __device__ __forceinline__ void topk_mask_block(
     int P, int force_last) {
   constexpr int kTopkThreads = NT;
   __shared__ int s_hist[kBuckets];
-  __shared__ int s_warp[33];
+  __shared__ int s_warp[64];
+  int scan_phase = 0;
   __shared__ uint64_t s_red[2][32];
   __shared__ uint64_t s_lo, s_width;
   __shared__ int s_need, s_done;
@@ -177,7 +175,7 @@ __device__ __forceinline__ void topk_mask_block(
 #pragma unroll
       for (int u = 0; u < kPer; ++u) { cbk[u] = s_hist[kBuckets - 1 - (tid * kPer + u)]; csum += cbk[u]; }
       int total;
-      int run = block_excl_scan<NT>(csum, s_warp, &total);   // keys in strictly higher buckets
+      int run = block_excl_scan<NT>(csum, s_warp, &total, scan_phase);   // keys in strictly higher buckets
       int hit = -1, above = 0, cnt = 0;
 #pragma unroll
       for (int u = 0; u < kPer; ++u) {
@@ -218,7 +216,7 @@ __device__ __forceinline__ void topk_mask_block(
       else if (key > thr_lo) { above_bits |= 1ull << (i - i0); ++above_cnt; }   // off wrapped <=> key < thr_lo
     }
   int tot_packed;
-  const int before = block_excl_scan<NT>(above_cnt | (band_cnt << 16), s_warp, &tot_packed);   // (ends all reads of keys[])
+  const int before = block_excl_scan<NT>(above_cnt | (band_cnt << 16), s_warp, &tot_packed, scan_phase);   // (ends all reads of keys[])
   int above_rank = before & 0xffff, band_rank = before >> 16;
   const int tot_sel = (tot_packed & 0xffff) + min(tot_packed >> 16, need_in_band);
   int32_t* sel_s = reinterpret_cast<int32_t*>(keys);           // selected pages, ascending; reuses the key storage
