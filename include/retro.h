@@ -188,6 +188,19 @@ int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_h
                     int32_t n_upd /*HOST*/, const int32_t* block_table, const int32_t* seq_lens, void* k_pages,
                     void* v_pages, void* stream);
 
+/* NEXT-2.  Relative budget policy on the device (budget = 0.15 x context length,
+ * at least 256 tokens, re-evaluated every step): budget_pages[b] = max(1, max(min_tokens,
+ * seq_lens[b] * ratio_permille / 1000) / page_size), integer arithmetic.  seq_lens, budget_pages: DEVICE [B]. */
+int retro_budget_policy(const retro_desc_t* desc, const int32_t* seq_lens, int32_t ratio_permille /*HOST*/,
+                        int32_t min_tokens /*HOST*/, int32_t* budget_pages, void* stream);
+
+/* NEXT-2: Alg. 2 on its own, for a page set S_t chosen by another selector (the method is
+ * selector-agnostic): for every page p of sel_pages[b][h][0..sel_count): sel_prev <- A[p];
+ * A[p] <- t (t = seq_lens[b] - 1); entries past sel_count get -1.  Pages of one (b, h) list must be distinct.
+ * Follow with retro_sparse_attend and retro_merge_output_cache.  All pointers DEVICE. */
+int retro_build_mask(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_count,
+                     const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, void* stream);
+
 /* Window-ring bookkeeping used by the two calls above and by the synthetic benchmark: seq_lens[b] += 1;
  * row (new position mod (w+1)) of q_win <- q_new[b], q_pos <- new position.  q_new [B][h_q][d] T.
  * If step_counter != NULL, q_new is taken as q_pool[(*step_counter) % pool_steps] ([pool][B][h_q][d]) and the

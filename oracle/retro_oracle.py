@@ -18,6 +18,8 @@ mask A / list M | Alg. 2; Sec. C.2 PAPER.md:448 | select_pages
 attention       | Eq. 2 / 6 / 7; Alg.1 l.6  | sparse_attend
 merge           | Eq. 8-9; Alg. 1 l.7           | merge_partials, merge_output_cache
 output cache    | Sec. 2.3 push/update/pop PAPER.md:83-85; l.8    | merge_output_cache
+budget policy   | relative budget 0.15, floor 256 tokens, PAPER.md:122 | budget_policy
+external S_t    | Alg. 2 alone (selector-agnostic use)  | build_mask
 KV overwrite    | Alg. 1 l.2 UpdateKV PAPER.md:391; Sec. 2.4 :87-93 | update_kv (+ update_page_bounds)
 
 Readings of silent / garbled passages (full list with reasons in DESIGN.md "Readings"):
@@ -187,6 +189,34 @@ def select_pages(desc, scores, seq_lens, budget_pages, last_loaded):
                     sel_prev[b, h, i] = last_loaded[b, h, p]   # M.append(A[p])
                     last_loaded[b, h, p] = t                   # A[p] <- t
     return sel_pages, sel_prev, sel_count
+
+
+# --------------------------------------------------------------------------------------------
+# NEXT-2  relative budget ("relative KV cache budget of 0.15, which dynamically changes the budget to
+# context length x 0.15 as decoding continues, with the minimum budget of 256 tokens") and Alg. 2 alone for a page
+# set chosen by another selector (the method is selector-agnostic).
+# --------------------------------------------------------------------------------------------
+def budget_policy(desc, seq_lens, ratio_permille=150, min_tokens=256):
+    """budget_pages[b] = floor(max(min_tokens, floor(seq_len * ratio)) / P), at least 1 (integer arithmetic:
+    the ratio is given in 1/1000 so both sides take the same integer decision)."""
+    out = np.zeros(desc.batch, dtype=np.int32)
+    for b in range(desc.batch):
+        tokens = max(int(min_tokens), (int(seq_lens[b]) * int(ratio_permille)) // 1000)
+        out[b] = max(1, tokens // desc.page_size)
+    return out
+
+
+def build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded):
+    """Alg. 2 lines 3-6 for a GIVEN S_t: M.append(A[p]); A[p] <- t.  Returns sel_prev (M)."""
+    sel_prev = np.full_like(sel_pages, -1)
+    for b in range(desc.batch):
+        t = int(seq_lens[b]) - 1
+        for h in range(desc.num_kv_heads):
+            for i in range(int(sel_count[b, h])):
+                p = int(sel_pages[b, h, i])
+                sel_prev[b, h, i] = last_loaded[b, h, p]
+                last_loaded[b, h, p] = t
+    return sel_prev
 
 
 # --------------------------------------------------------------------------------------------

@@ -24,6 +24,7 @@ EXPORTED = [
     "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
     "retro_window_advance", "retro_window_advance_layers", "retro_update_kv",
+    "retro_budget_policy", "retro_build_mask",
 ]
 
 
@@ -173,6 +174,18 @@ def retro_window_advance(desc, q_new_or_pool, step_counter, pool_steps, seq_lens
     _check(_lib().retro_window_advance(C.byref(desc), _p(q_new_or_pool), _p(step_counter), C.c_int32(pool_steps),
                                        _p(seq_lens), _p(q_win), _p(q_pos), _p(q_cur_out), _stream(stream)),
            "retro_window_advance")
+
+
+def retro_budget_policy(desc, seq_lens, budget_pages, ratio_permille=150, min_tokens=256, stream=None):
+    """Relative budget on the device: budget_pages[b] from seq_lens[b]."""
+    _check(_lib().retro_budget_policy(C.byref(desc), _p(seq_lens), C.c_int32(ratio_permille), C.c_int32(min_tokens),
+                                      _p(budget_pages), _stream(stream)), "retro_budget_policy")
+
+
+def retro_build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded, sel_prev, stream=None):
+    """Alg. 2 alone for an externally chosen page set."""
+    _check(_lib().retro_build_mask(C.byref(desc), _p(sel_pages), _p(sel_count), _p(seq_lens), _p(last_loaded),
+                                   _p(sel_prev), _stream(stream)), "retro_build_mask")
 
 
 def retro_update_kv(desc, k_hat, v_hat, positions, block_table, seq_lens, k_pages, v_pages, stream=None):

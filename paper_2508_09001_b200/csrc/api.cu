@@ -176,6 +176,22 @@ int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, in
                                (cudaStream_t)stream);
 }
 
+int retro_budget_policy(const retro_desc_t* desc, const int32_t* seq_lens, int32_t ratio_permille, int32_t min_tokens,
+                        int32_t* budget_pages, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(budget_pages);
+  if (ratio_permille < 0 || min_tokens < 0) return RETRO_ERR_ARG;
+  return launch_budget_policy(desc, seq_lens, ratio_permille, min_tokens, budget_pages, (cudaStream_t)stream);
+}
+
+int retro_build_mask(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_count,
+                     const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(last_loaded);
+  RETRO_CHECK_PTR(sel_prev);
+  return launch_build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded, sel_prev, (cudaStream_t)stream);
+}
+
 int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_hat, const int32_t* positions,
                     int32_t n_upd, const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                     void* stream) {

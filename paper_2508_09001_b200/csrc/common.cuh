@@ -63,6 +63,10 @@ int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const 
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
 int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
                      const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s);
+int launch_budget_policy(const retro_desc_t* d, const int32_t* seq_lens, int ratio_permille, int min_tokens,
+                         int32_t* budget_pages, cudaStream_t s);
+int launch_build_mask(const retro_desc_t* d, const int32_t* sel_pages, const int32_t* sel_count,
+                      const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, cudaStream_t s);
 int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat, const int32_t* positions, int n_upd,
                      const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                      cudaStream_t s);

@@ -229,6 +229,42 @@ def test_update_kv_overwrite_and_digest_refresh_match_oracle():
         assert np.array_equal(buf.bounds[b, :, :n].double().cpu().numpy(), layer.bounds[b, :, :n])
 
 
+def test_budget_policy_and_build_mask_match_oracle():
+    """NEXT-2: device-side relative budget and Alg. 2 alone (external selector), bit-exact against the oracle."""
+    cfg = wl.shrink(wl.c5(8, 1024), (1500, 40, 1714), 4, batch=3)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    layer = H.oracle_layer(inp)
+    L = np.array([1503, 43, 1717], dtype=np.int32)
+    buf.seq_lens.copy_(torch.from_numpy(L))
+    rb.retro_budget_policy(desc, buf.seq_lens, buf.budget_pages, 150, 256)
+    torch.cuda.synchronize()
+    assert buf.budget_pages.cpu().tolist() == orc.budget_policy(layer.desc, L).tolist() == [16, 16, 16]
+    rb.retro_budget_policy(desc, buf.seq_lens, buf.budget_pages, 500, 64)
+    torch.cuda.synchronize()
+    assert buf.budget_pages.cpu().tolist() == orc.budget_policy(layer.desc, L, 500, 64).tolist()
+    # an "external selector": arbitrary distinct pages per (b, h), two rounds so that A carries state
+    g = torch.Generator().manual_seed(5)
+    k_max = desc.max_sel_pages
+    for rnd in range(2):
+        sel = torch.full((3, cfg.num_kv_heads, k_max), -1, dtype=torch.int32)
+        cnt = torch.zeros((3, cfg.num_kv_heads), dtype=torch.int32)
+        for b in range(3):
+            npg = -(-int(L[b]) // 16)
+            for h in range(cfg.num_kv_heads):
+                c = min(npg, int(torch.randint(1, k_max + 1, (1,), generator=g)))
+                sel[b, h, :c] = torch.sort(torch.randperm(npg, generator=g)[:c]).values.int()
+                cnt[b, h] = c
+        buf.sel_pages.copy_(sel); buf.sel_count.copy_(cnt)
+        rb.retro_build_mask(desc, buf.sel_pages, buf.sel_count, buf.seq_lens, buf.last_loaded, buf.sel_prev)
+        torch.cuda.synchronize()
+        want = orc.build_mask(layer.desc, sel.numpy(), cnt.numpy(), L, layer.last_loaded)
+        assert np.array_equal(buf.sel_prev.cpu().numpy(), want)
+        assert np.array_equal(buf.last_loaded.cpu().numpy(), layer.last_loaded)
+        L = L + 1
+        buf.seq_lens.copy_(torch.from_numpy(L))
+
+
 def _to_cpu(inp):
     return wl.LayerInputs(inp.cfg, inp.k_pages.cpu(), inp.v_pages.cpu(), inp.block_table.cpu(), inp.q_all.cpu(),
                           inp.prompt_lens.cpu(), inp.outlier_channels.cpu())

@@ -10,6 +10,7 @@ import os
 from fractions import Fraction
 
 import numpy as np
+from dataclasses import replace as dataclasses_replace
 import pytest
 import torch
 
@@ -423,3 +424,32 @@ def test_update_kv_overwrites_exactly_the_named_rows_and_digests_follow():
     orc.update_kv(layer.desc, layer.k_pages, layer.v_pages, layer.block_table, seq, np.array([[44, 46]]),
                   same, np.stack([v1[[44, 46]]]))
     assert np.array_equal(layer.k_pages, before)
+
+
+# ------------------------------------------------------------------------------- NEXT-2 budget policy, Alg. 2 alone
+def test_budget_policy_values_from_the_papers_rule():
+    """budget = 0.15 x context length, minimum 256 tokens.  Hand-computed values (page 16):
+    32768 -> 4915 tokens -> 307 pages; 1000 -> 150 < 256 -> 16 pages; 1707 -> 256.05 -> 256 -> 16 pages;
+    1714 -> 257 tokens -> 16 pages; 131072 -> 19660 -> 1228 pages."""
+    desc = dataclasses_replace(_desc_small(4, 4), batch=5, page_size=16)
+    got = orc.budget_policy(desc, np.array([32768, 1000, 1707, 1714, 131072]))
+    assert got.tolist() == [307, 16, 16, 16, 1228]
+    assert orc.budget_policy(desc, np.array([10, 10, 10, 10, 10]), ratio_permille=150, min_tokens=0).tolist() == [1] * 5
+
+
+def test_build_mask_alone_equals_the_select_epilogue():
+    """Alg. 2 run on its own over the S_t that select_pages chose must reproduce select_pages' M and A."""
+    cfg = wl.shrink(wl.c2(), (200,), 6, window=3, budget_tokens=64, num_q_heads=4, num_kv_heads=2, head_dim=8)
+    inp = wl.make_layer_inputs(cfg)
+    a = H.oracle_layer(inp); b = H.oracle_layer(inp)
+    a.prefill_bounds(np.array([200])); b.prefill_bounds(np.array([200]))
+    budget = np.array([cfg.budget_pages], dtype=np.int32)
+    for s in range(6):
+        L = np.array([201 + s])
+        for lay in (a, b):
+            orc.update_page_bounds(lay.desc, lay.k_pages, lay.block_table, L, L - 1, lay.bounds)
+        scores = orc.page_scores(a.desc, H.np64(inp.q_all[s]), a.bounds, L)
+        sp, sv, sc = orc.select_pages(a.desc, scores, L, budget, a.last_loaded)
+        sv2 = orc.build_mask(b.desc, sp, sc, L, b.last_loaded)
+        assert np.array_equal(sv, sv2) and np.array_equal(a.last_loaded, b.last_loaded)
+    assert (a.last_loaded >= 0).any()
