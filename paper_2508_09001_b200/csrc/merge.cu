@@ -73,9 +73,10 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
   if (threadIdx.x < R) {
     const int r = threadIdx.x;
     const int p = q_pos[b * R + r];
+    const int cp = cache_pos[b * w + slot];          // unconditional: rides the same round trip as q_pos
     if (p >= 0 && p <= t && p >= t - w) {
       if (p == t) { if (t % w == slot) s_cur_row = r; }
-      else if (p % w == slot) { s_past_row = r; s_ppast = p; s_cached = (cache_pos[b * w + slot] == p) ? 1 : 0; }
+      else if (p % w == slot) { s_past_row = r; s_ppast = p; s_cached = (cp == p) ? 1 : 0; }
     }
   }
   __syncthreads();
