@@ -45,6 +45,8 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   if (nsplit < 1) nsplit = 1;
   wl.pages_per_split = ceil_div(d->max_sel_pages, nsplit);
   if (umma) wl.pages_per_split = ceil_div(wl.pages_per_split, 8) * 8;
+  // the page list of a split lives in shared memory: very large budgets take more splits (and waves) instead
+  if (umma && wl.pages_per_split > 1024) wl.pages_per_split = 1024;
   wl.nsplit = ceil_div(d->max_sel_pages, wl.pages_per_split);
   size_t off = 0;
   wl.scores_off = off;

@@ -110,6 +110,14 @@ def test_edge_max_group_and_window_three_row_groups():
     print("G8 w32 errs", GH.lockstep(inp, 36))
 
 
+def test_edge_dense_budget_above_the_page_list_cap():
+    """80 units (a single split each by the one-wave rule) with 1101 selected pages: the 1024-page cap on a
+    split's shared-memory page list forces a second split; budget = whole cache, so the result is dense attention."""
+    cfg = wl.shrink(wl.c5(1, 17616), (17600,) * 10, 2, batch=10)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("dense 1101 pages errs", GH.lockstep(inp, 2, check_scores=False))
+
+
 def test_edge_pure_topk_and_group_max():
     cfg = wl.shrink(wl.c2(), (777,), 12, budget_tokens=128, window=4)
     inp = wl.make_layer_inputs(cfg)
