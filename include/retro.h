@@ -64,7 +64,8 @@ extern "C" {
 #define RETRO_GROUP_MAX 1
 
 /* Supported instantiations: {RETRO_F32, head_dim 64, page_size 16}, {RETRO_BF16, head_dim 128, page_size 16}.
- * Limits: window <= 32, group (h_q / h_k) <= 8, max_pages_per_seq <= 24576. */
+ * Limits: window <= 32, group (h_q / h_k) <= 8, max_pages_per_seq <= 16384, batch <= 65535 (<= 64 for the
+ * window-advance helpers). */
 typedef struct retro_desc {
   int32_t batch;             /* B                                                              */
   int32_t num_q_heads;       /* h_q                                                            */

@@ -118,6 +118,14 @@ def test_edge_dense_budget_above_the_page_list_cap():
     print("dense 1101 pages errs", GH.lockstep(inp, 2, check_scores=False))
 
 
+def test_edge_maximum_pages_per_sequence():
+    """262 140-token context = 16 384 pages, the library's page limit (128 KB of top-k keys in shared memory)."""
+    cfg = wl.shrink(wl.c4(), (262138,), 2, batch=1, num_q_heads=4, num_kv_heads=2, window=1)
+    assert cfg.max_pages_per_seq == 16384
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("max pages errs", GH.lockstep(inp, 2))
+
+
 def test_edge_pure_topk_and_group_max():
     cfg = wl.shrink(wl.c2(), (777,), 12, budget_tokens=128, window=4)
     inp = wl.make_layer_inputs(cfg)
