@@ -279,6 +279,7 @@ def main():
     assert torch.isfinite(stack.layers[-1].out.float()).all()
 
     seq_now = stack.seq_lens_host()
+    workload_stats = selection_stats(stack.layers[0], cfg)
     bytes_model = hs.stage_bytes(cfg, seq_now)
     peak, peak_src = measured_hbm_peak()
     line = {
@@ -291,7 +292,7 @@ def main():
                      "achieved_gbs": bytes_model["total"] / (us_layer * 1e-6) / 1e9,
                      "frac_of_measured": bytes_model["total"] / (us_layer * 1e-6) / 1e9 / peak,
                      "frac_of_nominal_8TBs": bytes_model["total"] / (us_layer * 1e-6) / 1e9 / NOMINAL_HBM_GBS},
-        "clocks": clocks,
+        "clocks": clocks, "workload_stats": workload_stats,
     }
 
     if not args.no_extras:
@@ -370,6 +371,32 @@ def main():
     if ri.world_size > 1:
         dist.destroy_process_group()
     return 0
+
+
+def selection_stats(buf, cfg):
+    """Statistics of the synthetic workload from layer 0's last step (host-side torch ops on the kernel's
+    outputs; nothing of the method is computed here): how many selected pages were also selected at the previous
+    step (the paper reports ~83 % on real activations) and which fraction of (past row, selected
+    page) pairs is unmasked, i.e. supplementary work of the retro rows."""
+    import torch
+    if cfg.window == 0:
+        return None
+    cnt = buf.sel_count.cpu()
+    prev = buf.sel_prev.cpu()
+    qpos = buf.q_pos.cpu()
+    seq = buf.seq_lens.cpu()
+    tot = ov = pairs = unmasked = 0
+    for b in range(cfg.batch):
+        t = int(seq[b]) - 1
+        past = [int(p) for p in qpos[b].tolist() if 0 <= p < t]
+        for h in range(cfg.num_kv_heads):
+            pv = prev[b, h, :int(cnt[b, h])]
+            tot += pv.numel()
+            ov += int((pv == t - 1).sum())
+            for p in past:
+                pairs += pv.numel()
+                unmasked += int((pv < p).sum())
+    return {"adjacent_step_page_overlap": ov / max(tot, 1), "unmasked_past_row_page_pairs": unmasked / max(pairs, 1)}
 
 
 def bandwidth_point(peak, dev):
