@@ -281,6 +281,44 @@ def test_budget_policy_and_build_mask_match_oracle():
         buf.seq_lens.copy_(torch.from_numpy(L))
 
 
+def test_decode_step_host_end_to_end_matches_oracle():
+    """retro_decode_step_host (bench.py's e2e leg): pinned host q / k / v of the new token in, window ring and
+    KV append on the device, whole step, `out` back on the host - against the oracle, every step."""
+    cfg = wl.shrink(wl.c2(), (1003,), 12)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    layer = H.oracle_layer(inp)
+    B, w, P = cfg.batch, cfg.window, cfg.page_size
+    prompt = np.asarray(cfg.prompt_lens)
+    layer.prefill_bounds(prompt)
+    buf.seq_lens.copy_(torch.from_numpy(prompt.astype(np.int32)))
+    buf.rebuild_bounds()
+    dt = torch.bfloat16
+    dq = torch.empty((B, cfg.num_q_heads, cfg.head_dim), dtype=dt, device="cuda")
+    dk = torch.empty((B, cfg.num_kv_heads, cfg.head_dim), dtype=dt, device="cuda")
+    dv = torch.empty_like(dk)
+    io = rb.RetroStepIO(dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(),
+                        buf.out.data_ptr())
+    hout = torch.empty((B, w + 1, cfg.num_q_heads, cfg.head_dim), dtype=dt).pin_memory()
+    atol, rtol = GH.TOL[cfg.dtype]
+    for s in range(12):
+        hq = inp.q_all[s].cpu().contiguous().pin_memory()
+        hk = torch.empty((B, cfg.num_kv_heads, cfg.head_dim), dtype=dt)
+        hv = torch.empty_like(hk)
+        for b in range(B):
+            pos = cfg.prompt_lens[b] + s
+            phys = int(inp.block_table[b, pos // P])
+            hk[b], hv[b] = inp.k_pages[phys, :, pos % P].cpu(), inp.v_pages[phys, :, pos % P].cpu()
+        hk, hv = hk.pin_memory(), hv.pin_memory()
+        rb.retro_decode_step_host(desc, buf.state, io, hq, hk, hv, hout)
+        torch.cuda.synchronize()
+        q_win, q_pos = wl.make_q_window(inp, s)
+        res = layer.step(H.np64(q_win), q_pos.numpy(), H.np64(inp.q_all[s].cpu()), inp.seq_lens_at(s).cpu().numpy(),
+                         np.full(B, cfg.budget_pages, dtype=np.int32))
+        assert np.array_equal(buf.sel_pages.cpu().numpy(), res["sel_pages"])
+        GH.close(hout.float().numpy(), res["out"], atol, rtol, f"e2e step {s} out")
+
+
 def _to_cpu(inp):
     return wl.LayerInputs(inp.cfg, inp.k_pages.cpu(), inp.v_pages.cpu(), inp.block_table.cpu(), inp.q_all.cpu(),
                           inp.prompt_lens.cpu(), inp.outlier_channels.cpu())
