@@ -94,8 +94,8 @@ __device__ __forceinline__ int block_excl_scan(int v, int* s_warp /*[2][32]*/, i
 // Executed by all NT threads of one CTA for unit (b, h); scores are read through L2 (written by other CTAs).
 template <int NT>
 __device__ __forceinline__ void topk_mask_block(
-    uint64_t* keys /*shared [max_pages]*/, const double* scores, const int32_t* __restrict__ seq_lens,
-    const int32_t* __restrict__ budget_pages, int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
+    uint64_t* keys /*shared [max_pages]*/, const double* scores, int L /*seq_lens[b]*/, int budget /*budget_pages[b]*/,
+    int32_t* __restrict__ last_loaded, int32_t* __restrict__ sel_pages,
     int32_t* __restrict__ sel_prev, int32_t* __restrict__ sel_count, int b, int h, int h_k, int max_pages, int k_max,
     int P, int force_last) {
   constexpr int kTopkThreads = NT;
@@ -107,10 +107,9 @@ __device__ __forceinline__ void topk_mask_block(
   __shared__ int s_need, s_done;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int L = seq_lens[b];
   const int t = L - 1;
   const int n_pages = L > 0 ? (L + P - 1) / P : 0;
-  int k = min(min(budget_pages[b], n_pages), k_max);
+  int k = min(min(budget, n_pages), k_max);
   k = max(k, 0);
   const size_t row = ((size_t)b * h_k + h);
   int32_t* out_pages = sel_pages + row * k_max;
@@ -284,7 +283,9 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     for (int g = 0; g < kMaxGroup; ++g)
       if (g < G) q_raw[g] = q_cur[((size_t)b * h_q + h * G + g) * D + c];
   }
-  const int n_pages = (seq_lens[b] + P - 1) / P;
+  const int budget_b = budget_pages[b];       // only the unit's last CTA needs it: fetched with the first round trip
+  const int seq_len_b = seq_lens[b];
+  const int n_pages = (seq_len_b + P - 1) / P;
   const int cta_page0 = blockIdx.x * pages_per_cta;
   const size_t row = ((size_t)b * h_k + h) * max_pages;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -439,7 +440,7 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
 #endif
   SSTAMP(u0, 3);
   if (threadIdx.x == 0) counters[unit] = 0;   // leave the workspace consistent for the next call
-  topk_mask_block<kScoreWarps * 32>(reinterpret_cast<uint64_t*>(smem_raw), scores, seq_lens, budget_pages,
+  topk_mask_block<kScoreWarps * 32>(reinterpret_cast<uint64_t*>(smem_raw), scores, seq_len_b, budget_b,
                                     last_loaded, sel_pages, sel_prev, sel_count, b, h, h_k, max_pages, k_max, P,
                                     force_last);
   SSTAMP(u0, 9);
