@@ -7,6 +7,10 @@ namespace retro {
 
 static std::atomic<int> g_last_cuda_error{0};
 void set_cuda_error(cudaError_t e) { g_last_cuda_error.store((int)e); }
+std::mutex& host_mutex() {
+  static std::mutex m;
+  return m;
+}
 
 int validate_desc(const retro_desc_t* d) {
   if (d == nullptr) return RETRO_ERR_ARG;

@@ -241,6 +241,7 @@ static int launch_simt(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   const size_t smem = (size_t)kStages * 2 * 16 * D * sizeof(T) + (size_t)rows * D * sizeof(T) +
                       (size_t)3 * prm.pages_per_split * sizeof(int32_t) + 8 + kStages * sizeof(uint64_t);
   auto kern = attend_simt_kernel<T, D, RPW>;
+  std::lock_guard<std::mutex> lock(host_mutex());
   static size_t smem_allowed = 0;   // per instantiation; raised on demand (not a stream operation)
   if (smem > smem_allowed) {
     RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

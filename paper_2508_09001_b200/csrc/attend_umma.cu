@@ -640,6 +640,7 @@ static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const Umma
 
 int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStream_t s) {
   // the encode is pure host work (~1 us); cache the maps per (pool pair, shape)
+  std::lock_guard<std::mutex> lock(host_mutex());
   struct Cached { const void* k; const void* v; int phys, hk; CUtensorMap mk, mv; };
   constexpr int kCache = 64;
   static Cached cache[kCache];

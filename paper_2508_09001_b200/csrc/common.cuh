@@ -5,6 +5,8 @@
 #include <stdint.h>
 #include <stdlib.h>
 
+#include <mutex>
+
 #include "../../include/retro.h"
 
 namespace retro {
@@ -25,6 +27,10 @@ void set_cuda_error(cudaError_t e);
     }                                             \
   } while (0)
 #define RETRO_LAUNCH_CHECK() RETRO_CUDA_TRY(cudaGetLastError())
+
+// Host-side launcher state (tensor-map cache, raised shared-memory limits) is guarded by one mutex, so the entry
+// points may be called from several host threads; apart from that and the last CUDA error there is no global state.
+std::mutex& host_mutex();   // api.cu
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }

@@ -474,6 +474,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   auto launch = [&](auto kern, auto* qp, auto* bp) -> int {
     auto* bw = bp;   // the same digest array, writable for the in-line S1 refresh
     // raise the dynamic shared-memory limit once per kernel instantiation (not a stream operation)
+    std::lock_guard<std::mutex> lock(host_mutex());
     static const void* raised[8];
     static size_t raised_to[8];
     int slot = -1;
