@@ -127,6 +127,7 @@ __device__ __forceinline__ void topk_mask_block(
 
   if (!take_all && k_sel > 0) {
     uint64_t kmin = ~0ull, kmax = 0ull;
+#pragma unroll 4
     for (int i = tid; i < m; i += kTopkThreads) {
       const uint64_t key = order_key(__ldcg(scores + row * max_pages + i));
       keys[i] = key;
@@ -162,11 +163,19 @@ __device__ __forceinline__ void topk_mask_block(
       const int shift = nbits > 11 ? nbits - 11 : 0;
       for (int i = tid; i < kBuckets; i += kTopkThreads) s_hist[i] = 0;
       __syncthreads();
-      for (int i = tid; i < m; i += kTopkThreads) {
-        const uint64_t off = keys[i] - lo;
-        if (off <= range) atomicAdd(&s_hist[(int)(off >> shift)], 1);
+      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 11);
+      for (int i0 = tid; i0 < m; i0 += 8 * kTopkThreads) {   // loads first: they cannot be hoisted over the atomics
+        uint64_t kk[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) kk[u] = keys[min(i0 + u * kTopkThreads, m - 1)];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const uint64_t off = kk[u] - lo;
+          if (i0 + u * kTopkThreads < m && off <= range) atomicAdd(&s_hist[(int)(off >> shift)], 1);
+        }
       }
       __syncthreads();
+      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 12);
       // thread i owns kBuckets / NT consecutive buckets, highest first: scanning threads in order walks buckets
       // downward
       constexpr int kPer = kBuckets / NT;
@@ -175,6 +184,7 @@ __device__ __forceinline__ void topk_mask_block(
       for (int u = 0; u < kPer; ++u) { cbk[u] = s_hist[kBuckets - 1 - (tid * kPer + u)]; csum += cbk[u]; }
       int total;
       int run = block_excl_scan<NT>(csum, s_warp, &total, scan_phase);   // keys in strictly higher buckets
+      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 13);
       int hit = -1, above = 0, cnt = 0;
 #pragma unroll
       for (int u = 0; u < kPer; ++u) {
@@ -191,6 +201,9 @@ __device__ __forceinline__ void topk_mask_block(
         s_done = (cnt == need - above || shift == 0) ? 1 : 0;
       }
       __syncthreads();
+#ifdef RETRO_STAMPS
+      if (b == 0 && h == 0 && tid == 0) g_sel_stamps[10] = g_sel_stamps[0] + pass + 1;
+#endif
       if (s_done) break;
     }
     thr_lo = s_lo;
