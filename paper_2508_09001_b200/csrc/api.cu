@@ -61,6 +61,8 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   off = align_up(off + (size_t)units * wl.nsplit * wl.rows * sizeof(float), 256);
   wl.counters_off = off;
   off = align_up(off + (size_t)4 * units * sizeof(unsigned int), 256);
+  wl.slot_counters_off = off;   // (zeroed by retro_workspace_init together with the counters before it)
+  off = align_up(off + (size_t)d->batch * (d->window + 1) * sizeof(unsigned int), 256);
   wl.total = off;
   return wl;
 }
@@ -245,9 +247,20 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, c
                            st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s, st->k_pages,
                            st->block_table);
   if (rc != RETRO_OK) return rc;
+  // S3; on the tensor-core path with several splits the attend kernel leaves its split partials uncombined and
+  // ONE kernel does the split combine and S4 (the partials and the cache operands ride the same round trip)
+  bool deferred = true;
   rc = launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
-                            st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s);
+                            st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s,
+                            &deferred);
   if (rc != RETRO_OK) return rc;
+  if (deferred) {
+    char* ws = static_cast<char*>(st->workspace);
+    return launch_combine_merge(desc, reinterpret_cast<const float*>(ws + wl.split_o_off),
+                                reinterpret_cast<const float*>(ws + wl.split_lse_off), wl.nsplit, wl.rows, st->part_o,
+                                st->part_lse, q_pos, st->seq_lens, st->cache_o, st->cache_lse, st->cache_pos, out,
+                                out_lse, reinterpret_cast<unsigned int*>(ws + wl.slot_counters_off), s);
+  }
   return launch_merge_output_cache(desc, st->part_o, st->part_lse, q_pos, st->seq_lens, st->cache_o, st->cache_lse,
                                    st->cache_pos, out, out_lse, s);
 }

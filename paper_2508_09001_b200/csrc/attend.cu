@@ -268,8 +268,12 @@ static int dispatch_rpw(const retro_desc_t* d, const AttendParams& prm, cudaStre
 int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_win, const int32_t* q_pos,
                          const void* k_pages, const void* v_pages, const int32_t* block_table,
                          const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,
-                         const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s) {
+                         const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s,
+                         bool* defer_combine) {
   AttendParams prm;
+  const bool may_defer = defer_combine != nullptr && *defer_combine;
+  if (defer_combine != nullptr) *defer_combine = false;
+  prm.defer_combine = 0;
   char* ws = static_cast<char*>(workspace);
   prm.q_win = q_win; prm.q_pos = q_pos; prm.k_pages = k_pages; prm.v_pages = v_pages;
   prm.block_table = block_table; prm.seq_lens = seq_lens; prm.sel_pages = sel_pages; prm.sel_prev = sel_prev;
@@ -293,6 +297,10 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
     if (!force_simt) {
       prm.nrg = wl.nrg;
       prm.rg_rows = wl.rg_rows;
+      if (may_defer && wl.nsplit > 1) {
+        prm.defer_combine = 1;
+        *defer_combine = true;
+      }
       return launch_attend_umma(d, prm, s);
     }
     return dispatch_rpw<__nv_bfloat16, 128>(d, prm, s);

@@ -13,6 +13,7 @@ struct AttendParams {
   const int32_t* sel_count; float* part_o; float* part_lse; float* split_o; float* split_lse;
   unsigned int* counters;
   int B, h_q, h_k, max_pages, k_max, window, nsplit, pages_per_split;
+  int defer_combine;   // 1: leave the split partials in the workspace (a combine + merge kernel follows)
   int nrg, rg_rows;   // query-row groups of the tensor-core path (rows > 128): CTA (split, group) owns rg_rows rows
   float scale_log2;   // sm_scale * log2(e)
 };

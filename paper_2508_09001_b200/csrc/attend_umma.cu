@@ -577,7 +577,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
   }
-  if (p.nsplit == 1) return;
+  if (p.nsplit == 1 || p.defer_combine) return;
   combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket, row0, row0 + rows_cta,
                                &p.counters[unit * p.nrg + rg]);
   STAMP(cta0 && tid == 0, 22);

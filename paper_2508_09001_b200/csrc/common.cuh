@@ -42,6 +42,7 @@ struct WorkspaceLayout {
   size_t scores_off;    // double [B][h_k][max_pages]
   size_t split_o_off;   // float  [B][h_k][nsplit][rows][d]
   size_t split_lse_off; // float  [B][h_k][nsplit][rows]
+  size_t slot_counters_off;  // uint32 [B][w+1]: arrivals per (sequence, cache slot) of the combine + merge kernel
   size_t counters_off;  // uint32 [4][B][h_k]: score-chunk counters first, then split arrival counters per row group
   size_t total;
   int nsplit;           // split-KV factor of the attend kernel
@@ -63,7 +64,12 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
 int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_win, const int32_t* q_pos,
                          const void* k_pages, const void* v_pages, const int32_t* block_table,
                          const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,
-                         const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s);
+                         const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s,
+                         bool* defer_combine = nullptr);   // in: allowed; out: the split partials were left uncombined
+int launch_combine_merge(const retro_desc_t* d, const float* split_o, const float* split_lse, int nsplit, int rows,
+                         float* part_o, float* part_lse, const int32_t* q_pos, const int32_t* seq_lens, float* cache_o,
+                         float* cache_lse, int32_t* cache_pos, void* out, float* out_lse, unsigned int* slot_counters,
+                         cudaStream_t s);
 int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
                               const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
