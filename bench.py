@@ -312,7 +312,8 @@ def main():
         ach = sb[dom] / (stages[dom] * 1e-6) / 1e9
         line["stages_us"] = stages
         line["stages_note"] = ("each stage = its C-ABI call launched alone, L times back to back; inside retro_decode_step "
-                               "S1 (bounds) is not a launch of its own: the select kernel rebuilds the newest page's digest")
+                               "S1 (bounds) is not a launch of its own (the select kernel rebuilds the newest page's digest) "
+                               "and the attend kernel's split combine runs together with S4 in one combine + merge kernel")
         line["stages_gbs"] = {k: sb[k] / (stages[k] * 1e-6) / 1e9 for k in stages}
         line["roofline"] = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s",
                             "frac": ach / peak, "traffic": NCU_TRAFFIC_BYTES.get(args.workload, {}).get(dom) if (args.window is None and args.budget is None) else None,
