@@ -209,86 +209,99 @@ __global__ void __launch_bounds__(256) combine_merge_kernel(
   const int past = s_past_row, cur = s_cur_row, p_past = s_ppast;
   const bool cached = past >= 0 && s_cpos == p_past;
   const bool evict = past >= 0 && p_past == t - w;
-  if (warp < G) {
-    const int hq = h * G + warp;
-    // combine of one row: all split loads in flight at once (8 per pass)
-    auto combine = [&](int r, float (&o)[4], float& lse_nat) {
-      const int rho = r * G + warp;
-      const float* ls = split_lse + unit * nsplit * rows + rho;
-      const float* os = split_o + (unit * nsplit * rows + rho) * D + lane * 4;
-      const size_t stride = (size_t)rows * D;
-      float mx = -INFINITY;
-      for (int s = lane; s < nsplit; s += 32) mx = fmaxf(mx, __ldcg(ls + (size_t)s * rows));
-      mx = warp_max(mx);
-      o[0] = o[1] = o[2] = o[3] = 0.f;
-      float wsum = 0.f;
-      for (int s0 = 0; s0 < nsplit; s0 += 8) {
-        float4 v[8];
-        float wg[8];
+  // Work items: (past row | current row) x q head of the group.  With G <= 4 the eight warps take one item each
+  // (both rows in parallel); otherwise warp g takes both rows of head g.  Phase 1 loads, combines, merges and
+  // writes `out`; the cache is rewritten in phase 2, after a barrier: the slot popped by the row at t-w is the
+  // slot the current row is pushed into.
+  const bool one_item = 2 * G <= 8;
+  float4 res_k[2];
+  float lse_k[2];
+  bool wr_k[2] = {false, false};
+  int hq_k[2] = {0, 0};
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int s = min(s0 + u, nsplit - 1);
-          v[u] = __ldcg(reinterpret_cast<const float4*>(os + (size_t)s * stride));
-          const float l = __ldcg(ls + (size_t)s * rows);
-          wg[u] = (s0 + u < nsplit && l > -INFINITY) ? exp2f(l - mx) : 0.f;
-        }
+  for (int kind = 0; kind < 2; ++kind) {
+    const bool active = one_item ? (warp >= kind * G && warp < (kind + 1) * G) : (warp < G);
+    const int g = one_item ? warp - kind * G : warp;
+    const int r = kind == 0 ? past : cur;
+    if (!active || r < 0) continue;
+    const int hq = h * G + g;
+    hq_k[kind] = hq;
+    const size_t ce = w > 0 ? ((size_t)b * w + x) * h_q + hq : 0;
+    // every operand of the item goes out before the first use: split partials (first 8), their lse, the cache
+    const int rho = r * G + g;
+    const float* ls = split_lse + unit * nsplit * rows + rho;
+    const float* os = split_o + (unit * nsplit * rows + rho) * D + lane * 4;
+    const size_t stride = (size_t)rows * D;
+    float4 v[8];
+    auto load8 = [&](int s_first) {
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          if (wg[u] > 0.f) {            // an empty split's o is unspecified: never multiply it
-            wsum += wg[u];
-            o[0] = fmaf(wg[u], v[u].x, o[0]); o[1] = fmaf(wg[u], v[u].y, o[1]);
-            o[2] = fmaf(wg[u], v[u].z, o[2]); o[3] = fmaf(wg[u], v[u].w, o[3]);
+      for (int u = 0; u < 8; ++u)
+        v[u] = __ldcg(reinterpret_cast<const float4*>(os + (size_t)min(s_first + u, nsplit - 1) * stride));
+    };
+    load8(0);
+    float lc = -INFINITY;
+    float4 vc = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (kind == 0 && cached) {
+      lc = cache_lse[ce];
+      vc = *reinterpret_cast<const float4*>(cache_o + ce * D + lane * 4);
+    }
+    float mx = -INFINITY;
+    for (int s = lane; s < nsplit; s += 32) mx = fmaxf(mx, __ldcg(ls + (size_t)s * rows));
+    mx = warp_max(mx);
+    float o[4] = {0.f, 0.f, 0.f, 0.f};
+    float wsum = 0.f;
+    if (mx > -INFINITY) {
+      for (int s0 = 0; s0 < nsplit; s0 += 32) {
+        const int sl = s0 + lane;
+        const float l_mine = sl < nsplit ? __ldcg(ls + (size_t)sl * rows) : -INFINITY;
+        const float w_mine = exp2f(l_mine - mx);           // lane s holds the weight of split s0 + s; 0 if empty
+        const int cnt = min(32, nsplit - s0);
+        for (int s1 = 0; s1 < cnt; s1 += 8) {
+          if (s0 + s1 > 0) load8(s0 + s1);
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            float wg = __shfl_sync(0xffffffffu, w_mine, (s1 + u) & 31);
+            if (s1 + u >= cnt) wg = 0.f;
+            if (wg > 0.f) {                                // an empty split's o is unspecified: never multiply it
+              wsum += wg;
+              o[0] = fmaf(wg, v[u].x, o[0]); o[1] = fmaf(wg, v[u].y, o[1]);
+              o[2] = fmaf(wg, v[u].z, o[2]); o[3] = fmaf(wg, v[u].w, o[3]);
+            }
           }
         }
       }
-      const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
-      o[0] *= inv; o[1] *= inv; o[2] *= inv; o[3] *= inv;
-      lse_nat = wsum > 0.f ? (mx + log2f(wsum)) * kLn2f : -INFINITY;
-      const size_t e = ((size_t)b * R + r) * h_q + hq;
-      *reinterpret_cast<float4*>(part_o + e * D + lane * 4) = make_float4(o[0], o[1], o[2], o[3]);
-      if (lane == 0) part_lse[e] = lse_nat;
-    };
-    const size_t ce = w > 0 ? ((size_t)b * w + x) * h_q + hq : 0;
-    if (past >= 0) {
-      float lc = -INFINITY;
-      float4 vc = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (cached) {                       // issued before the combine's loads are consumed: same round trip
-        lc = cache_lse[ce];
-        vc = *reinterpret_cast<const float4*>(cache_o + ce * D + lane * 4);
-      }
-      float o[4], lp;
-      combine(past, o, lp);
-      float4 res;
-      float lse;
-      if (lc == -INFINITY) { res = make_float4(o[0], o[1], o[2], o[3]); lse = lp; }
-      else if (lp == -INFINITY) { res = vc; lse = lc; }
-      else {
-        const float m2 = fmaxf(lc, lp);
-        const float wc = __expf(lc - m2), wp = __expf(lp - m2);
-        const float iv = 1.f / (wc + wp);
-        res.x = (wc * vc.x + wp * o[0]) * iv; res.y = (wc * vc.y + wp * o[1]) * iv;
-        res.z = (wc * vc.z + wp * o[2]) * iv; res.w = (wc * vc.w + wp * o[3]) * iv;
-        lse = m2 + __logf(wc + wp);
-      }
-      const size_t e = ((size_t)b * R + past) * h_q + hq;
-      OutVec<__nv_bfloat16>::store(out + e * D + lane * 4, res);
-      if (lane == 0 && out_lse != nullptr) out_lse[e] = lse;
-      if (!evict) {
-        *reinterpret_cast<float4*>(cache_o + ce * D + lane * 4) = res;
-        if (lane == 0) cache_lse[ce] = lse;
-      }
     }
-    if (cur >= 0) {   // push O_org of the current query (this warp has already read the popped row)
-      float o[4], lq;
-      combine(cur, o, lq);
-      const float4 res = make_float4(o[0], o[1], o[2], o[3]);
-      const size_t e = ((size_t)b * R + cur) * h_q + hq;
-      OutVec<__nv_bfloat16>::store(out + e * D + lane * 4, res);
-      if (lane == 0 && out_lse != nullptr) out_lse[e] = lq;
-      if (w > 0) {
-        *reinterpret_cast<float4*>(cache_o + ce * D + lane * 4) = res;
-        if (lane == 0) cache_lse[ce] = lq;
-      }
+    const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
+    o[0] *= inv; o[1] *= inv; o[2] *= inv; o[3] *= inv;
+    const float lp = wsum > 0.f ? (mx + log2f(wsum)) * kLn2f : -INFINITY;
+    const size_t e = ((size_t)b * R + r) * h_q + hq;
+    *reinterpret_cast<float4*>(part_o + e * D + lane * 4) = make_float4(o[0], o[1], o[2], o[3]);
+    if (lane == 0) part_lse[e] = lp;
+    float4 res;
+    float lse;
+    if (lc == -INFINITY) { res = make_float4(o[0], o[1], o[2], o[3]); lse = lp; }
+    else if (lp == -INFINITY) { res = vc; lse = lc; }
+    else {
+      const float m2 = fmaxf(lc, lp);
+      const float wc = __expf(lc - m2), wp = __expf(lp - m2);
+      const float iv = 1.f / (wc + wp);
+      res.x = (wc * vc.x + wp * o[0]) * iv; res.y = (wc * vc.y + wp * o[1]) * iv;
+      res.z = (wc * vc.z + wp * o[2]) * iv; res.w = (wc * vc.w + wp * o[3]) * iv;
+      lse = m2 + __logf(wc + wp);
+    }
+    OutVec<__nv_bfloat16>::store(out + e * D + lane * 4, res);
+    if (lane == 0 && out_lse != nullptr) out_lse[e] = lse;
+    res_k[kind] = res;
+    lse_k[kind] = lse;
+    wr_k[kind] = w > 0 && (kind == 0 ? !evict : true);
+  }
+  __syncthreads();                        // every cache read of this (slot, KV head) is done
+#pragma unroll
+  for (int kind = 0; kind < 2; ++kind) {
+    if (wr_k[kind]) {
+      const size_t ce = ((size_t)b * w + x) * h_q + hq_k[kind];
+      *reinterpret_cast<float4*>(cache_o + ce * D + lane * 4) = res_k[kind];
+      if (lane == 0) cache_lse[ce] = lse_k[kind];
     }
   }
   if (w > 0) {
