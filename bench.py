@@ -5,7 +5,8 @@
 
 A "step" is one decode step of an L-layer stack (default L = 32, Llama-3.1-8B depth): for every layer, in
 Alg. 1's order, digest refresh (S1) -> page score + top-k + mask (S2) -> fused multi-query
-sparse attention (S3) -> output-cache merge (S4), all through the C ABI.  Each layer has its own K/V pool,
+sparse attention (S3) -> output-cache merge (S4), all through the C ABI (`retro_decode_step`: three launches per
+layer - select with S1 in line, attend, split combine + merge).  Each layer has its own K/V pool,
 digests, mask and cache, so consecutive layer-steps do not share L2 (about 13 MB touched per layer-step, 430 MB
 per step >> 126 MB L2).  One step is captured in a CUDA graph (every step-varying value lives in device memory)
 and replayed K times between CUDA events.  Prints ONE JSON line (rank 0).
