@@ -101,6 +101,7 @@ def test_edge_budget_zero_selects_nothing():
     cfg = wl.shrink(wl.c2(), (200,), 5, budget_tokens=16, window=2)
     inp = wl.make_layer_inputs(cfg)
     GH.lockstep(inp, 5, budget_pages=0, k_max=4)
+    GH.lockstep(inp, 5, budget_pages=0, k_max=16, use_decode_step=True)     # empty splits through combine + merge
 
 
 def test_edge_max_group_and_window_three_row_groups():
