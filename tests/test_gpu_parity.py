@@ -66,11 +66,12 @@ def test_c5_shape_shrunk_sweep_points(w, budget):
     ("c5w0", dict(prompt_lens=(1500, 1490), n_steps=5, batch=2, window=0)),          # plain Quest, no cache
     ("c5w32", dict(prompt_lens=(1500, 1490), n_steps=38, batch=2, window=32, budget_tokens=512)),   # 2 row groups
     ("c4", dict(prompt_lens=(3001, 2990), n_steps=12, batch=2, budget_tokens=512)),  # GQA 7
+    ("c5b20", dict(prompt_lens=tuple(600 - 7 * i for i in range(20)), n_steps=11, batch=20)),   # 160 units: one split
 ])
 def test_whole_step_entry_point_bf16(name, kw):
     """retro_decode_step (the call bench.py captures into its graph) against the oracle: selections bit-exact,
     out / out_lse / cache within tolerance, every step, no teacher forcing."""
-    base = {"c2": wl.c2(), "c5w8": wl.c5(8, 1024), "c5w0": wl.c5(0, 1024), "c5w32": wl.c5(32, 512), "c4": wl.c4()}[name]
+    base = {"c2": wl.c2(), "c5w8": wl.c5(8, 1024), "c5w0": wl.c5(0, 1024), "c5w32": wl.c5(32, 512), "c4": wl.c4(), "c5b20": wl.c5(8, 512)}[name]
     kw = dict(kw)
     cfg = wl.shrink(base, kw.pop("prompt_lens"), kw.pop("n_steps"), **kw)
     inp = wl.make_layer_inputs(cfg)
