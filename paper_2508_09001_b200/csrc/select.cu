@@ -273,9 +273,8 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     const T* __restrict__ k_pages, const int32_t* __restrict__ block_table, T* bounds_out) {
   static_assert(2 * D * sizeof(T) == 512, "digest record must be 512 bytes");
   constexpr int kVals = Rec<T>::kVals;
-  // digest ring [kStages][64 records x 512 B]; the unit's last CTA reuses it for the top-k keys
+  // digest rings [warp][kStages][8 records x 512 B]; the unit's last CTA reuses the space for the top-k keys
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  __shared__ __align__(8) uint64_t s_full[kStages];
   [[maybe_unused]] const bool u0 = blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0;
   SSTAMP(u0 && blockIdx.x == 0, 0);
   unsigned long long t_begin = 0;
@@ -306,25 +305,28 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     for (int j = max(cta_page0, n_pages) + threadIdx.x; j < min(cta_page0 + pages_per_cta, max_pages); j += blockDim.x)
       scores_out[row + j] = -INFINITY;
   if (cta_page0 < n_pages) {
-  // the digest stream does not depend on q: start the first batch before q is staged; afterwards one batch
-  // of 8 records per lane stays in flight while the previous one is reduced
-  // The digest records of consecutive pages are contiguous: one bulk copy (TMA unit, cp.async.bulk + mbarrier)
-  // brings a whole batch of 64 records (32 KB) into the shared-memory ring, kStages batches in flight per CTA,
-  // so the bytes in flight are bounded by shared memory, not by registers.
+  // The digest stream does not depend on q: it starts before q is staged.  Every warp streams its own pages
+  // (8 records = 4 KB per batch, lane l copies the 16 B it will read) with cp.async (LDGSTS, 16 B per lane) into a
+  // warp-private ring of kStages buffers: bytes in flight are bounded by shared memory, not registers, and the
+  // pipeline needs no CTA-wide barrier (cp.async.wait_group + __syncwarp per batch).
   const int page_end = min(cta_page0 + pages_per_cta, n_pages);
   const int nbatch = (page_end - cta_page0 + kPagesPerCta - 1) / kPagesPerCta;
-  auto issue_batch = [&](int it) {   // thread 0
-    const int p0 = cta_page0 + it * kPagesPerCta;
-    const uint32_t bytes = (uint32_t)min(kPagesPerCta, page_end - p0) * (2 * D * sizeof(T));
-    const int st = it % kStages;
-    mbar_expect_tx(&s_full[st], bytes);
-    bulk_g2s(smem_raw + (size_t)st * kStageBytes, bounds + (row + p0) * 2 * D, bytes, &s_full[st]);
+  unsigned char* wring = smem_raw + (size_t)warp * kStages * (kPagesPerWarp * 512);
+  auto issue_batch = [&](int it) {   // all lanes; always one commit group, possibly empty
+    if (it < nbatch) {
+      const int jb = cta_page0 + it * kPagesPerCta + warp * kPagesPerWarp;
+      const uint32_t dst = smem_u32(wring + (size_t)(it % kStages) * (kPagesPerWarp * 512)) + lane * 16;
+      const unsigned char* src = reinterpret_cast<const unsigned char*>(bounds + (row + jb) * 2 * D) + lane * 16;
+#pragma unroll
+      for (int i = 0; i < kPagesPerWarp; ++i)
+        if (jb + i < n_pages)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + i * 512), "l"(src + (size_t)i * 512)
+                       : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
   };
-  if (threadIdx.x == 0) {
-    for (int i = 0; i < kStages; ++i) mbar_init(&s_full[i], 1);
-    fence_mbar_init();
-    for (int it = 0; it < min(kStages, nbatch); ++it) issue_batch(it);
-  }
+#pragma unroll
+  for (int it = 0; it < kStages - 1; ++it) issue_batch(it);
   // S1 in line: the warp that will reduce the newest page (j_last) rebuilds its digest while the first batches fly
   const int j_last = n_pages - 1;
   const bool own_last = k_pages != nullptr && j_last >= cta_page0 && j_last < page_end &&
@@ -356,13 +358,11 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
   double qreg[kVals];
 #pragma unroll
   for (int c = 0; c < kVals; ++c) qreg[c] = s_q[0][lane * kVals + c];
-  auto reduce_store = [&](const unsigned char* stage, int page0) {
+  auto reduce_store = [&](unsigned char* wstage /*this warp's 8 records*/, int page0) {
     const int jbase = page0 + warp * kPagesPerWarp;
-    const uint4* rec = reinterpret_cast<const uint4*>(stage) + warp * kPagesPerWarp * 32 + lane;
-    if (own_last && j_last >= page0 && j_last < page0 + kPagesPerCta) {   // patch the staged (stale) record
-      reinterpret_cast<uint4*>(const_cast<unsigned char*>(stage))[(j_last - page0) * 32 + lane] = fresh;
-      __syncwarp();
-    }
+    const uint4* rec = reinterpret_cast<const uint4*>(wstage) + lane;
+    if (own_last && j_last >= jbase && j_last < jbase + kPagesPerWarp)   // patch the staged (stale) record
+      reinterpret_cast<uint4*>(wstage)[(j_last - jbase) * 32 + lane] = fresh;   // (each lane reads back its own 16 B)
     double acc[kPagesPerWarp];
     if constexpr (!kGroupMax) {
 #pragma unroll
@@ -434,12 +434,13 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
     }
   };
   for (int it = 0; it < nbatch; ++it) {
-    const int st = it % kStages;
-    mbar_wait(&s_full[st], (it / kStages) & 1);
-    reduce_store(smem_raw + (size_t)st * kStageBytes, cta_page0 + it * kPagesPerCta);
-    __syncthreads();                                   // every warp is done with the stage: refill it
-    if (threadIdx.x == 0 && it + kStages < nbatch) issue_batch(it + kStages);
+    issue_batch(it + kStages - 1);                     // refills the buffer reduced in the previous iteration
+    asm volatile("cp.async.wait_group %0;" ::"n"(kStages - 1) : "memory");
+    __syncwarp();
+    reduce_store(wring + (size_t)(it % kStages) * (kPagesPerWarp * 512), cta_page0 + it * kPagesPerCta);
+    __syncwarp();
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
   }   // cta_page0 < n_pages
   // ---- the last CTA of the unit to get here selects (release: barrier, then one cumulative fence) ----
   const size_t unit = (size_t)b * h_k + h;
