@@ -473,11 +473,14 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   char* ws = static_cast<char*>(workspace);
   double* scores = reinterpret_cast<double*>(ws + wl.scores_off);
   unsigned int* counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off);   // [units] score-chunk arrivals
-  // at most ONE wave of CTAs (two are resident per SM: 128 registers x 256 threads), each streaming whole batches
-  // of 64 pages: the per-CTA costs (q staging, arrival ticket) amortise over several batches when there are many
-  // units, and no unit waits for a second wave before its last CTA can select
+  // at most ONE wave of CTAs (three are resident per SM), each streaming whole batches of 64 pages: the per-CTA
+  // costs (q staging, arrival ticket) amortise over several batches, and no unit waits for a second wave before
+  // its last CTA can select
   const int units = d->batch * d->num_kv_heads;
-  int nchunk = (3 * 148) / units;
+  // a small digest set (latency-bound launch, e.g. 9 MB on C2) takes one CTA per SM: fewer, fatter CTAs and fewer
+  // arrival tickets; a large one (bandwidth-bound) fills the three resident CTAs per SM
+  const size_t digest_bytes = (size_t)units * d->max_pages_per_seq * 512;
+  int nchunk = ((digest_bytes >= ((size_t)32 << 20) ? 3 : 1) * 148) / units;
   if (nchunk < 1) nchunk = 1;
   const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerCta);
   if (nchunk > max_chunks) nchunk = max_chunks;
