@@ -38,8 +38,8 @@ FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
 NCU_TRAFFIC_BYTES = {   # profiles/r01e_summary.md: dram__bytes_read.sum + dram__bytes_write.sum per launch
-    "c2": {"attend": 4348416.0, "select": 8507136.0},
-    "c5": {"attend": 140435000.0, "select": 68354560.0},
+    "c2": {"attend": 4348416.0, "select": 8500736.0},
+    "c5": {"attend": 140435000.0, "select": 68467200.0},
 }
 
 
