@@ -53,6 +53,7 @@ def measured_hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+CORR_RHO = 0.0                               # --corr: persistence / AR(1) coefficient of the query stream
 C5_POINT = {"window": 8, "budget": 4096}     # the C5 sweep point `--workload c5` runs (see --window / --budget)
 
 
@@ -72,6 +73,8 @@ def workload_cfg(name: str, n_steps: int, window=None):
         raise SystemExit(f"unknown workload {name}")
     if window is not None:
         cfg = cfg.replace(window=window, name=cfg.name + f"_w{window}")
+    if CORR_RHO > 0.0:     # correlated-query mode of the workload generator, separately labelled
+        cfg = cfg.replace(corr_rho=CORR_RHO, name=cfg.name + f"_corr{CORR_RHO:g}")
     return cfg
 
 
@@ -217,7 +220,7 @@ def config_dict(cfg, n_layers):
     return {"workload": cfg.name, "batch": cfg.batch, "num_q_heads": cfg.num_q_heads,
             "num_kv_heads": cfg.num_kv_heads, "head_dim": cfg.head_dim, "page_size": cfg.page_size,
             "context": max(cfg.prompt_lens), "budget_tokens": cfg.budget_tokens, "window": cfg.window,
-            "layers_per_step": n_layers,
+            "layers_per_step": n_layers, "query_correlation_rho": cfg.corr_rho,
             "l2": "inputs larger than L2: each layer-step reads its own layer's digests+pages; "
                   f"{n_layers} independent layer states per step"}
 
@@ -234,9 +237,13 @@ def main():
     ap.add_argument("--oracle-steps", type=int, default=8)
     ap.add_argument("--window", type=int, default=None, help="C5 sweep: retro window w (past queries)")
     ap.add_argument("--budget", type=int, default=None, help="C5 sweep: budget in tokens")
+    ap.add_argument("--corr", type=float, default=0.0,
+                    help="correlated-query mode: planted keys persist / noise is AR(1) with this rho (default: i.i.d.)")
     ap.add_argument("--no-w0", action="store_true", help="skip the w=0 overhead run (sweeps measure w=0 themselves)")
     ap.add_argument("--lite", action="store_true", help="sweep point: stage timing only (no e2e, cpu baseline, w=0 run)")
     args = ap.parse_args()
+    global CORR_RHO
+    CORR_RHO = args.corr
     if args.window is not None:
         C5_POINT["window"] = args.window
     if args.budget is not None:

@@ -27,6 +27,10 @@ dataset is used or needed.  The recipe:
     sentinel `PAD_VALUE`; a kernel that leaks them produces visibly wrong output.
   * Seeds: torch.Generator(device).manual_seed(base_seed + 1000*layer + b),
     base_seed = 20250801 + config index.
+  * Optional "correlated" mode (`corr_rho` > 0; the default i.i.d. queries are the
+    compute-worst case): every planted key persists from the previous step with probability rho and the
+    noise is AR(1) with coefficient rho, which raises the adjacent-step page overlap towards what the paper
+    reports on real activations (~80 %).
 
 Generators run on whatever torch device is asked for (CPU here, CUDA on the GPU
 box); parity tests copy the SAME generated arrays to the other side.
@@ -60,6 +64,7 @@ class RetroConfig:
     strata: bool = False       # C4: planted keys spread uniformly over the context
     n_outlier: int = 4
     outlier_scale: float = 8.0
+    corr_rho: float = 0.0      # "correlated" mode: planted keys persist / noise is AR(1) with this rho
 
     @property
     def group(self) -> int:
@@ -222,6 +227,18 @@ def make_layer_inputs(cfg: RetroConfig, layer: int = 0, device="cpu",
             else:
                 idx = (u * span).floor().long()
             idx = torch.minimum(idx, t[:, None, None])                                # [n_q][hq][n_pl]
+            if cfg.corr_rho > 0.0:
+                # correlated mode: each planted key is kept from the previous step with probability rho (else the
+                # fresh draw above), and the noise is AR(1) with coefficient rho and unit variance.  Extra draws
+                # come AFTER the i.i.d. ones, so K/V and the rho = 0 queries are unchanged.
+                keep = torch.rand((n_q, hq, cfg.n_planted), generator=g_b, device=dev, dtype=torch.float64) < cfg.corr_rho
+                keep[0] = False
+                steps_i = torch.arange(n_q, device=dev)[:, None, None].expand_as(idx)
+                last_fresh = torch.cummax(torch.where(keep, torch.zeros_like(steps_i), steps_i), dim=0).values
+                idx = torch.gather(idx, 0, last_fresh)                                # <= t of that earlier step <= t
+                c = math.sqrt(1.0 - cfg.corr_rho ** 2)
+                for i in range(1, n_q):
+                    noise[i] = cfg.corr_rho * noise[i - 1] + c * noise[i]
             kv_head = (torch.arange(hq, device=dev) // G)[None, :, None].expand_as(idx)
             planted = k_seq.float()[idx, kv_head]                                     # [n_q][hq][n_pl][d]
             q_all[:, b] = (noise + cfg.beta * planted.sum(dim=2)).to(dt)

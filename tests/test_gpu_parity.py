@@ -53,6 +53,15 @@ def test_c4_shape_shrunk_gqa7():
     print("c4s errs", GH.lockstep(inp, 20))
 
 
+@pytest.mark.parametrize("use_step", [False, True])
+def test_c2_shape_correlated_queries_high_page_overlap(use_step):
+    """Correlated mode: most selected pages repeat from step to step, so most (past row, page)
+    pairs are masked (the regime the paper reports on real activations)."""
+    cfg = wl.shrink(wl.c2(), (2003,), 30, corr_rho=0.95)
+    inp = wl.make_layer_inputs(cfg)
+    print("c2 correlated errs", GH.lockstep(inp, 30, use_decode_step=use_step))
+
+
 @pytest.mark.parametrize("w,budget", [(0, 512), (1, 1024), (32, 512)])
 def test_c5_shape_shrunk_sweep_points(w, budget):
     cfg = wl.shrink(wl.c5(w, budget), (1500, 1490), w + 6, batch=2)
