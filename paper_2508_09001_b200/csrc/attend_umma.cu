@@ -231,10 +231,29 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   pdl_wait();
   pdl_trigger();
-  // Global loads that depend on nothing are issued first (count, length, the list entries of this split, Q);
-  // only block_table[j] is a second round trip.
+  // Global loads that depend on nothing are issued first (count, length, Q, q_pos, the list entries of this
+  // split): Q and q_pos are held in registers across the list loop so that their round trip overlaps the list's
+  // (in program order after it they were issued only once block_table[j], the one dependent load, had returned).
   const int count = p.sel_count[unit];
   const int L = p.seq_lens[b];
+  constexpr int kQIter = (NT * 16 + kUmmaThreads - 1) / kUmmaThreads;
+  uint4 q_regs[kQIter];
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
+#pragma unroll
+    for (int it = 0; it < kQIter; ++it) {
+      const int i = tid + it * kUmmaThreads;                   // NT rows x 16 chunks of 16 B
+      const int rho = i >> 4, c = i & 15;
+      q_regs[it] = make_uint4(0, 0, 0, 0);
+      if (i < NT * 16 && rho < rows_cta) {
+        const int r = (row0 + rho) / G, g = (row0 + rho) - r * G;
+        q_regs[it] = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
+      }
+    }
+  }
+  static_assert(NT <= kUmmaThreads, "one thread per padded row");
+  int my_pos_raw = -1;
+  if (tid < rows_cta) my_pos_raw = __ldg(p.q_pos + b * R + (row0 + tid) / G);
   for (int i = tid; i < pps; i += kUmmaThreads) {
     const int idx = split * pps + i;
     int j = 0, prev = 0;
@@ -248,17 +267,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     s_list[pps + i] = prev;
     s_list[2 * pps + i] = phys;
   }
-  {
-    const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
-    for (int i = tid; i < NT * 16; i += kUmmaThreads) {        // NT rows x 16 chunks of 16 B
+#pragma unroll
+  for (int it = 0; it < kQIter; ++it) {
+    const int i = tid + it * kUmmaThreads;
+    if (i < NT * 16) {
       const int rho = i >> 4, c = i & 15;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (rho < rows_cta) {
-        const int r = (row0 + rho) / G, g = (row0 + rho) - r * G;
-        v = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
-      }
       const int half = c >> 3, ch = c & 7;
-      *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = v;
+      *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = q_regs[it];
     }
   }
   const int t = L - 1;
@@ -267,7 +282,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     int pos = -1, off = 0;
     if (c < rows_cta) {
       const int r = (row0 + c) / G, g = (row0 + c) - r * G;
-      pos = p.q_pos[b * R + r];
+      pos = my_pos_raw;
       if (pos > t || pos < t - p.window) pos = -1;
       off = p.nsplit > 1 ? (row0 + c) * 128 : (r * p.h_q + h * G + g) * 128;
     }
