@@ -37,9 +37,9 @@ NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {   # profiles/r01e_summary.md: dram__bytes_read.sum + dram__bytes_write.sum per launch
-    "c2": {"attend": 4348416.0, "select": 8500736.0},
-    "c5": {"attend": 140435000.0, "select": 68467200.0},
+NCU_TRAFFIC_BYTES = {   # attend: profiles/r01f_summary.md, select: profiles/r01e_summary.md (kernel unchanged since)
+    "c2": {"attend": 4348672.0, "select": 8500736.0},
+    "c5": {"attend": 139311104.0, "select": 68467200.0},
 }
 
 
