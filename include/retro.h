@@ -202,6 +202,20 @@ int retro_budget_policy(const retro_desc_t* desc, const int32_t* seq_lens, int32
 int retro_build_mask(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_count,
                      const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, void* stream);
 
+/* NEXT-4: per-step diagnostics of the retrospective rows, computed from the outputs of
+ * retro_select_pages / retro_sparse_attend / retro_merge_output_cache of the SAME step (call it after the merge):
+ *   supp_pages[b][h][r] = number of this step's selected pages that window row r reads (sel_prev_j < q_pos[b][r]
+ *       and first token of the page <= q_pos[b][r]); for the current row this is the pages it can see.  Summed
+ *       over the steps a query stays in the window it is that query's EFFECTIVE KV budget in pages.
+ *   supp_mass[b][r][g] = exp(part_lse - out_lse): the share of the row's merged softmax mass contributed by this
+ *       step's pages (supplementary attention); 1 for the current row, 0 for an empty partial.
+ * Rows with q_pos = -1 (or outside [t - w, t]) give 0.  supp_pages [B][h_k][w+1] int32, supp_mass [B][w+1][h_q]
+ * f32, all DEVICE.  Not part of retro_decode_step; one small launch. */
+int retro_step_diagnostics(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_prev,
+                           const int32_t* sel_count, const int32_t* q_pos, const int32_t* seq_lens,
+                           const float* part_lse, const float* out_lse, int32_t* supp_pages, float* supp_mass,
+                           void* stream);
+
 /* Window-ring bookkeeping used by the two calls above and by the synthetic benchmark: seq_lens[b] += 1;
  * row (new position mod (w+1)) of q_win <- q_new[b], q_pos <- new position.  q_new [B][h_q][d] T.
  * If step_counter != NULL, q_new is taken as q_pool[(*step_counter) % pool_steps] ([pool][B][h_q][d]) and the

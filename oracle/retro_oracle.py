@@ -20,6 +20,7 @@ merge           | Eq. 8-9; Alg. 1 l.7           | merge_partia
 output cache    | Sec. 2.3 push/update/pop PAPER.md:83-85; l.8    | merge_output_cache
 budget policy   | relative budget 0.15, floor 256 tokens, PAPER.md:122 | budget_policy
 external S_t    | Alg. 2 alone (selector-agnostic use)  | build_mask
+diagnostics     | effective KV budget PAPER.md:62; suppl. attention :435-456 | step_diagnostics
 KV overwrite    | Alg. 1 l.2 UpdateKV PAPER.md:391; Sec. 2.4 :87-93 | update_kv (+ update_page_bounds)
 
 Readings of silent / garbled passages (full list with reasons in DESIGN.md "Readings"):
@@ -217,6 +218,30 @@ def build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded):
                 sel_prev[b, h, i] = last_loaded[b, h, p]
                 last_loaded[b, h, p] = t
     return sel_prev
+
+
+def step_diagnostics(desc, sel_pages, sel_prev, sel_count, q_pos, seq_lens, part_lse, out_lse):
+    """Per step and window row: supp_pages[b][h][r] = selected pages from which the row attends at least one
+    token (they enlarge its effective KV budget); supp_mass[b][r][g] = e^{lse_part - lse_merged},
+    the share of the merged softmax mass that this step's pages supply."""
+    R = desc.window + 1
+    G = desc.group
+    supp_pages = np.zeros((desc.batch, desc.num_kv_heads, R), dtype=np.int32)
+    supp_mass = np.zeros((desc.batch, R, desc.num_q_heads))
+    for b in range(desc.batch):
+        t = int(seq_lens[b]) - 1
+        for r in range(R):
+            p = int(q_pos[b, r])
+            if p < 0 or p > t or p < t - desc.window:
+                continue
+            for h in range(desc.num_kv_heads):
+                for i in range(int(sel_count[b, h])):
+                    one = attend_token_list(desc, p, seq_lens[b], sel_pages[b, h, i:i + 1], sel_prev[b, h, i:i + 1], 1)
+                    supp_pages[b, h, r] += 1 if len(one) > 0 else 0
+                for g in range(h * G, (h + 1) * G):
+                    if part_lse[b, r, g] > NEG_INF:
+                        supp_mass[b, r, g] = math.exp(part_lse[b, r, g] - out_lse[b, r, g])
+    return supp_pages, supp_mass
 
 
 # --------------------------------------------------------------------------------------------

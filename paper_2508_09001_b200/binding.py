@@ -24,7 +24,7 @@ EXPORTED = [
     "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
     "retro_window_advance", "retro_window_advance_layers", "retro_update_kv",
-    "retro_budget_policy", "retro_build_mask",
+    "retro_budget_policy", "retro_build_mask", "retro_step_diagnostics",
 ]
 
 
@@ -186,6 +186,14 @@ def retro_build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded, sel_prev
     """Alg. 2 alone for an externally chosen page set."""
     _check(_lib().retro_build_mask(C.byref(desc), _p(sel_pages), _p(sel_count), _p(seq_lens), _p(last_loaded),
                                    _p(sel_prev), _stream(stream)), "retro_build_mask")
+
+
+def retro_step_diagnostics(desc, sel_pages, sel_prev, sel_count, q_pos, seq_lens, part_lse, out_lse, supp_pages,
+                           supp_mass, stream=None):
+    """Per-step effective-budget / supplementary-attention counters."""
+    _check(_lib().retro_step_diagnostics(C.byref(desc), _p(sel_pages), _p(sel_prev), _p(sel_count), _p(q_pos),
+                                         _p(seq_lens), _p(part_lse), _p(out_lse), _p(supp_pages), _p(supp_mass),
+                                         _stream(stream)), "retro_step_diagnostics")
 
 
 def retro_update_kv(desc, k_hat, v_hat, positions, block_table, seq_lens, k_pages, v_pages, stream=None):

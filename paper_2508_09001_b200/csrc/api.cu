@@ -200,6 +200,19 @@ int retro_build_mask(const retro_desc_t* desc, const int32_t* sel_pages, const i
   return launch_build_mask(desc, sel_pages, sel_count, seq_lens, last_loaded, sel_prev, (cudaStream_t)stream);
 }
 
+int retro_step_diagnostics(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_prev,
+                           const int32_t* sel_count, const int32_t* q_pos, const int32_t* seq_lens,
+                           const float* part_lse, const float* out_lse, int32_t* supp_pages, float* supp_mass,
+                           void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(q_pos);
+  RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(out_lse); RETRO_CHECK_PTR(supp_pages);
+  RETRO_CHECK_PTR(supp_mass);
+  if (desc->num_q_heads / desc->num_kv_heads > 32) return RETRO_ERR_UNSUPPORTED;
+  return launch_step_diagnostics(desc, sel_pages, sel_prev, sel_count, q_pos, seq_lens, part_lse, out_lse,
+                                 supp_pages, supp_mass, (cudaStream_t)stream);
+}
+
 int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_hat, const int32_t* positions,
                     int32_t n_upd, const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                     void* stream) {

@@ -79,6 +79,10 @@ int launch_budget_policy(const retro_desc_t* d, const int32_t* seq_lens, int rat
                          int32_t* budget_pages, cudaStream_t s);
 int launch_build_mask(const retro_desc_t* d, const int32_t* sel_pages, const int32_t* sel_count,
                       const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, cudaStream_t s);
+int launch_step_diagnostics(const retro_desc_t* d, const int32_t* sel_pages, const int32_t* sel_prev,
+                            const int32_t* sel_count, const int32_t* q_pos, const int32_t* seq_lens,
+                            const float* part_lse, const float* out_lse, int32_t* supp_pages, float* supp_mass,
+                            cudaStream_t s);
 int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat, const int32_t* positions, int n_upd,
                      const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                      cudaStream_t s);

@@ -40,6 +40,50 @@ __global__ void build_mask_kernel(const int32_t* __restrict__ sel_pages, const i
   }
 }
 
+// NEXT-4 diagnostics.  Per step and window row: how many of the step's selected pages the row
+// may read (the pages that ENLARGE its effective KV budget) and which share of the row's merged
+// softmax mass they carry (supplementary attention).  One CTA per (KV head, sequence).
+__global__ void step_diagnostics_kernel(const int32_t* __restrict__ sel_pages, const int32_t* __restrict__ sel_prev,
+                                        const int32_t* __restrict__ sel_count, const int32_t* __restrict__ q_pos,
+                                        const int32_t* __restrict__ seq_lens, const float* __restrict__ part_lse,
+                                        const float* __restrict__ out_lse, int32_t* __restrict__ supp_pages,
+                                        float* __restrict__ supp_mass, int h_q, int h_k, int k_max, int R, int P) {
+  pdl_wait();
+  pdl_trigger();
+  const int h = blockIdx.x, b = blockIdx.y, G = h_q / h_k;
+  const size_t unit = (size_t)b * h_k + h;
+  const int t = seq_lens[b] - 1;
+  const int count = min(sel_count[unit], k_max);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
+  for (int r = warp; r < R; r += nwarp) {           // one warp per window row
+    int pos = q_pos[b * R + r];
+    if (pos > t || pos < t - (R - 1)) pos = -1;
+    int n = 0;
+    if (pos >= 0)
+      for (int i = lane; i < count; i += 32) {
+        const int j = sel_pages[unit * k_max + i];
+        n += (sel_prev[unit * k_max + i] < pos && (long long)j * P <= pos) ? 1 : 0;   // same rule as the attend kernel
+      }
+    n = __reduce_add_sync(0xffffffffu, n);
+    if (lane == 0) supp_pages[unit * R + r] = n;
+    if (lane < G) {
+      const size_t o = ((size_t)b * R + r) * h_q + h * G + lane;
+      const float pl = part_lse[o];
+      supp_mass[o] = (pos >= 0 && pl > -INFINITY) ? __expf(pl - out_lse[o]) : 0.f;
+    }
+  }
+}
+
+int launch_step_diagnostics(const retro_desc_t* d, const int32_t* sel_pages, const int32_t* sel_prev,
+                            const int32_t* sel_count, const int32_t* q_pos, const int32_t* seq_lens,
+                            const float* part_lse, const float* out_lse, int32_t* supp_pages, float* supp_mass,
+                            cudaStream_t s) {
+  RETRO_CUDA_TRY(launch_kernel(step_diagnostics_kernel, dim3(d->num_kv_heads, d->batch), dim3(256), 0, s, sel_pages,
+                               sel_prev, sel_count, q_pos, seq_lens, part_lse, out_lse, supp_pages, supp_mass,
+                               d->num_q_heads, d->num_kv_heads, d->max_sel_pages, d->window + 1, d->page_size));
+  return RETRO_OK;
+}
+
 int launch_budget_policy(const retro_desc_t* d, const int32_t* seq_lens, int ratio_permille, int min_tokens,
                          int32_t* budget_pages, cudaStream_t s) {
   RETRO_CUDA_TRY(launch_kernel(budget_policy_kernel, dim3(ceil_div(d->batch, 128)), dim3(128), 0, s, seq_lens,

@@ -292,6 +292,34 @@ def test_budget_policy_and_build_mask_match_oracle():
         buf.seq_lens.copy_(torch.from_numpy(L))
 
 
+def test_step_diagnostics_match_oracle():
+    """NEXT-4: effective-budget page counts (bit-exact) and supplementary attention mass per window row, from the
+    oracle's own step outputs (ragged batch, ramp-up rows with q_pos = -1, a page roll-over inside the run)."""
+    cfg = wl.shrink(wl.c5(8, 512), (1500, 40, 1714), 12, batch=3, corr_rho=0.8)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    layer, res = H.run_oracle_trajectory(inp, 12)
+    R = cfg.window + 1
+    supp_pages = torch.full((3, cfg.num_kv_heads, R), -7, dtype=torch.int32, device="cuda")
+    supp_mass = torch.full((3, R, cfg.num_q_heads), -7.0, dtype=torch.float32, device="cuda")
+    for m, r in enumerate(res):
+        k = r["sel_pages"].shape[2]
+        buf.sel_pages[:, :, :k].copy_(torch.from_numpy(r["sel_pages"].astype(np.int32)))
+        buf.sel_prev[:, :, :k].copy_(torch.from_numpy(r["sel_prev"].astype(np.int32)))
+        buf.sel_count.copy_(torch.from_numpy(r["sel_count"].astype(np.int32)))
+        buf.seq_lens.copy_(torch.from_numpy(r["seq_lens"].astype(np.int32)))
+        q_pos = torch.from_numpy(r["q_pos"].astype(np.int32)).cuda()
+        part_lse = torch.from_numpy(r["part_lse"]).float().cuda()
+        out_lse = torch.from_numpy(r["out_lse"]).float().cuda()
+        rb.retro_step_diagnostics(desc, buf.sel_pages, buf.sel_prev, buf.sel_count, q_pos, buf.seq_lens, part_lse,
+                                  out_lse, supp_pages, supp_mass)
+        torch.cuda.synchronize()
+        want_pages, want_mass = orc.step_diagnostics(layer.desc, r["sel_pages"], r["sel_prev"], r["sel_count"],
+                                                     r["q_pos"], r["seq_lens"], r["part_lse"], r["out_lse"])
+        assert np.array_equal(supp_pages.cpu().numpy(), want_pages), m
+        np.testing.assert_allclose(supp_mass.cpu().numpy(), want_mass, atol=2e-5, rtol=1e-4)
+
+
 def test_decode_step_host_end_to_end_matches_oracle():
     """retro_decode_step_host (bench.py's e2e leg): pinned host q / k / v of the new token in, window ring and
     KV append on the device, whole step, `out` back on the host - against the oracle, every step."""

@@ -488,3 +488,38 @@ def test_correlated_workload_raises_page_overlap_and_keeps_the_main_pin():
                 row = wl.ring_slot(cfg, cfg.prompt_lens[b] + s)
                 o, lse = fb.out(s, m)
                 np.testing.assert_allclose(res[m]["out"][b, row], o, rtol=1e-11, atol=1e-12)
+
+
+def test_step_diagnostics_effective_budget_is_the_union_size_and_mass_identity():
+    """Pins for the NEXT-4 counters, against quantities computed another way:
+    (i) summed over the steps a query stays in the window, supp_pages is the number of DISTINCT pages (with a token
+        at or before the query) in the union of the page sets of those steps (form B's explicit sets): every page
+        is counted once, the first time it is loaded (PAPER.md:62 effective KV budget; reading Q9);
+    (ii) 1 - supp_mass at step m equals e^{lse(out, step m-1) - lse(out, step m)} for a past row, supp_mass = 1
+        for the current row (Eq. 8-9)."""
+    cfg = wl.shrink(wl.c2(), (61, 50), 14, batch=2, window=3, budget_tokens=16 * 3,
+                    num_q_heads=4, num_kv_heads=2, head_dim=16)
+    inp = wl.make_layer_inputs(cfg)
+    layer, res = H.run_oracle_trajectory(inp, 14)
+    diag = [orc.step_diagnostics(layer.desc, r["sel_pages"], r["sel_prev"], r["sel_count"], r["q_pos"],
+                                 r["seq_lens"], r["part_lse"], r["out_lse"]) for r in res]
+    P, w = cfg.page_size, cfg.window
+    for b in range(2):
+        fb = H.FormB(inp, b, cfg.budget_pages)
+        for m in range(14):
+            fb.select(m)
+        for s in range(14 - w):                       # queries whose whole window life is inside the run
+            p = cfg.prompt_lens[b] + s
+            row = wl.ring_slot(cfg, p)
+            for h in range(2):
+                total = sum(int(diag[m][0][b, h, row]) for m in range(s, s + w + 1))
+                want = len([j for j in fb.seen(s, s + w, h) if j * P <= p])
+                assert total == want, (b, s, h, total, want)
+            np.testing.assert_allclose(diag[s][1][b, row], 1.0, rtol=0, atol=1e-15)      # current row
+            for m in range(s + 1, s + w + 1):
+                keep = np.exp(res[m - 1]["out_lse"][b, row] - res[m]["out_lse"][b, row])
+                np.testing.assert_allclose(1.0 - diag[m][1][b, row], keep, rtol=0, atol=1e-12)
+    # rows that are not in the window report nothing
+    for b in range(2):
+        empty = [r for r in range(w + 1) if res[0]["q_pos"][b, r] < 0]
+        assert len(empty) == w and np.all(diag[0][0][b][:, empty] == 0) and np.all(diag[0][1][b][empty] == 0)
