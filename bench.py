@@ -288,6 +288,8 @@ def main():
 
     seq_now = stack.seq_lens_host()
     workload_stats = selection_stats(stack.layers[0], cfg)
+    if workload_stats is not None and not args.no_extras and not args.lite:
+        workload_stats["device_counters"] = retro_diagnostics(cfg, seed_off)
     bytes_model = hs.stage_bytes(cfg, seq_now)
     peak, peak_src = measured_hbm_peak()
     line = {
@@ -406,6 +408,46 @@ def selection_stats(buf, cfg):
                 pairs += pv.numel()
                 unmasked += int((pv < p).sum())
     return {"adjacent_step_page_overlap": ov / max(tot, 1), "unmasked_past_row_page_pairs": unmasked / max(pairs, 1)}
+
+
+def retro_diagnostics(cfg, seed_offset, n_steps=48):
+    """Device-side counters of the retrospective rows (retro_step_diagnostics) over `n_steps` decode
+    steps of ONE layer driven through the stand-alone entry points (not timed): the effective KV budget a query
+    ends up with, relative to its own budget, and the softmax mass the retro updates add per step."""
+    import torch
+    from paper_2508_09001_b200 import binding as rb
+    from paper_2508_09001_b200 import harness as hs
+    if cfg.window == 0:
+        return None
+    stack = hs.DecodeStack(cfg, 1, n_steps, seed_offset=seed_offset)
+    d, buf = stack.desc, stack.layers[0]
+    B, hk, hq, R = cfg.batch, cfg.num_kv_heads, cfg.num_q_heads, cfg.window + 1
+    supp_pages = torch.zeros((B, hk, R), dtype=torch.int32, device=stack.device)
+    supp_mass = torch.zeros((B, R, hq), dtype=torch.float32, device=stack.device)
+    pages_acc = torch.zeros((), dtype=torch.float64, device=stack.device)
+    mass_acc = torch.zeros((), dtype=torch.float64, device=stack.device)
+    mass_n = 0
+    counted = 0
+    for s in range(n_steps):
+        rb.retro_window_advance_layers(d, stack.advance_table, 1, stack.pool_steps)
+        for stage in ("bounds", "select", "attend"):
+            stack.enqueue_stage(stage)
+        rb.retro_merge_output_cache(d, buf.part_o, buf.part_lse, buf.q_pos, buf.seq_lens, buf.cache_o, buf.cache_lse,
+                                    buf.cache_pos, buf.out, buf.out_lse)
+        rb.retro_step_diagnostics(d, buf.sel_pages, buf.sel_prev, buf.sel_count, buf.q_pos, buf.seq_lens,
+                                  buf.part_lse, buf.out_lse, supp_pages, supp_mass)
+        if s > cfg.window:                            # window full: every step carries w past rows
+            past = (buf.q_pos >= 0) & (buf.q_pos < (buf.seq_lens - 1)[:, None])          # [B][R]
+            pages_acc += supp_pages.double().sum()
+            mass_acc += (supp_mass.double() * past[:, :, None]).sum()
+            mass_n += int(past.sum()) * hq
+            counted += 1
+    torch.cuda.synchronize()
+    k = min(cfg.budget_pages, -(-min(cfg.prompt_lens) // cfg.page_size))
+    per_unit_step = float(pages_acc) / max(counted * B * hk, 1)     # = pages one query sees over its window life
+    return {"effective_budget_pages_per_query": per_unit_step, "own_budget_pages": k,
+            "effective_budget_ratio": per_unit_step / k,
+            "supplementary_mass_per_past_row_step": float(mass_acc) / max(mass_n, 1), "steps": counted}
 
 
 def bandwidth_point(peak, dev):
