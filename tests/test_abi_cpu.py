@@ -48,6 +48,8 @@ def test_host_side_validation_without_gpu():
     assert rc == rb.RETRO_ERR_ARG
     rc = lib.retro_merge_output_cache(C.byref(good), None, None, None, None, None, None, None, None, None, None)
     assert rc == rb.RETRO_ERR_ARG
+    rc = lib.retro_step_diagnostics(C.byref(good), None, None, None, None, None, None, None, None, None, None)
+    assert rc == rb.RETRO_ERR_ARG
 
 
 def test_workspace_grows_with_window_and_batch():
