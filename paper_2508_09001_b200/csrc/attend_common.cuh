@@ -19,9 +19,6 @@ struct AttendParams {
 };
 
 #ifdef __CUDACC__
-#ifndef RETRO_COMBINE_STAMP
-#define RETRO_COMBINE_STAMP(i) do { } while (0)
-#endif
 // Called by every thread of the CTA after it wrote its split partial (normalised o, base-2 lse) to the
 // workspace.  The last CTA of the (b, KV head) unit to arrive merges the nsplit partials (Eq. 8 applied to
 // splits: weights 2^(lse_s - max)) into part_o / part_lse (natural-log lse).  D = 128 or 64; one warp per row.
@@ -35,9 +32,7 @@ __device__ __forceinline__ void combine_splits_last_cta(const AttendParams& p, s
   // Release: every thread's partial stores happen-before the barrier; thread 0's acq_rel ticket is cumulative.
   __syncthreads();
   if (tid == 0) *s_ticket = ticket_acq_rel(counter);
-  RETRO_COMBINE_STAMP(24);
   __syncthreads();
-  RETRO_COMBINE_STAMP(25);
   if (*s_ticket != (unsigned)(p.nsplit - 1)) return;
   if (tid == 0) *counter = 0;   // leave the workspace consistent for the next call
   for (int rho = row_begin + warp; rho < row_end; rho += nwarps) {

@@ -31,11 +31,6 @@
 
 #include <cstdlib>
 
-#ifdef RETRO_STAMPS
-namespace retro { __device__ void retro_stamp(int i); }
-#define RETRO_COMBINE_STAMP(i) \
-  do { if ((blockIdx.x | blockIdx.y | blockIdx.z) == 0 && threadIdx.x == 64) ::retro::retro_stamp(i); } while (0)
-#endif
 #include "attend_common.cuh"
 
 namespace retro {
@@ -157,18 +152,6 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
   return L;
 }
 
-#ifdef RETRO_STAMPS
-__device__ unsigned long long g_stamps[128];
-__device__ __forceinline__ void stamp(int i) {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
-  g_stamps[i] = t;
-}
-#define STAMP(cond, i) do { if (cond) stamp(i); } while (0)
-__device__ void retro_stamp(int i) { stamp(i); }
-#else
-#define STAMP(cond, i) do { } while (0)
-#endif
 
 struct UmmaCfg {
   int NK, NV;     // K and V ring slots (32 KB each)
@@ -209,8 +192,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
 
   const int split = blockIdx.x % p.nsplit, rg = blockIdx.x / p.nsplit, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  [[maybe_unused]] const bool cta0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
-  STAMP(cta0 && tid == 0, 0);
   const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
   const int row0 = rg * p.rg_rows;                      // this CTA's query rows: [row0, row0 + rows_cta) of the unit
   const int rows_cta = min(p.rg_rows, rows - row0);
@@ -303,7 +284,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_ptr_s;
-  STAMP(cta0 && tid == 0, 1);
 
   if (nblk > 0) {
     if (warp < 2) {
@@ -318,7 +298,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         const int np = min(kPB, n_my - blk * kPB);
         unsigned char* dst = ring + slot * kSlotBytes;
         if (n > 0) mbar_wait(&empty[slot], (n - 1) & 1);
-        STAMP(cta0 && lane == 0 && warp == 0 && blk < 12, 32 + blk * 8 + 7);
         if (elect_one()) {
           mbar_expect_tx(&full[slot], np * 2 * kTileHalfBytes);
           for (int pg = 0; pg < np; ++pg) {
@@ -337,8 +316,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       auto issue_s = [&](int blk) {
         const int slot = blk % cfg.NK, n = blk / cfg.NK;
         mbar_wait(&k_full[slot], n & 1);
-        STAMP(cta0 && lane == 0 && blk == 0, 2);
-        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 3);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t k_addr = smem_u32(smem + lay.ring + slot * kSlotBytes);
@@ -364,10 +341,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         const int slot = blk % cfg.NV, n = blk / cfg.NV;
         const int np = min(kPB, n_my - blk * kPB);
         mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
-        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 4);
         if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
         mbar_wait(&v_full[slot], n & 1);
-        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 5);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t v_addr = smem_u32(smem + lay.ring + (cfg.NK + slot) * kSlotBytes);
@@ -381,7 +356,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           tc_commit(&o_full[blk & 1]);
         }
         __syncwarp();
-        STAMP(cta0 && lane == 0 && blk < 12, 32 + blk * 8 + 6);
       }
     } else if (warp >= 4) {
       // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NC = NT / 4 columns (rows) each =====
@@ -405,8 +379,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         }
         if (st == 0) s_flag[(blk + 1) % 3] = 0;
         mbar_wait(&s_full[blk % cfg.NSB], (blk / cfg.NSB) & 1);
-        STAMP(cta0 && st == 0, 3 + 4 * min(blk, 3));
-        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 0);
         tc_fence_after();
         const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
         // d = s * scale - m_ref (log2 units), -inf where masked; the common block needs nothing else
@@ -433,8 +405,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         }
         if (__any_sync(0xffffffffu, tmax > kRescaleThreshold) && lane == 0) s_flag[blk % 3] = 1;
         softmax_bar();
-        STAMP(cta0 && st == 0, 4 + 4 * min(blk, 3));
-        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 1);
         if (s_flag[blk % 3] != 0) {
           // ---- slow path: exact column max of this block, raise m_ref, rescale O and L ----
           float xs[NC];
@@ -489,7 +459,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           }
         }
         if (cfg.NP == 1 && blk > 0) mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) has read P
-        STAMP(cta0 && st == 0, 5 + 4 * min(blk, 3));
         // ---- P = 2^d as bf16 hi + lo into the MN-major SW128 operand (8-byte stores: NC is a multiple of 4) ----
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
@@ -513,8 +482,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&p_ready[blk % cfg.NP]);   // one arrival per warp (512 would serialise)
-        STAMP(cta0 && st == 0, 6 + 4 * min(blk, 3));
-        STAMP(cta0 && st == 0 && blk < 12, 32 + blk * 8 + 2);
       }
       // ---- epilogue: L per row, O = (O_hi + O_lo) / L through a shared-memory stage, coalesced stores ----
       {
@@ -536,7 +503,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         }
       }
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
-      STAMP(cta0 && st == 0, 20);
       tc_fence_after();
       softmax_bar();                                       // s_L complete
       float* o_base;
@@ -570,7 +536,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           }
         }
       }
-      STAMP(cta0 && st == 0, 23);
     }
   } else {
     // no page for this split: empty partial for every row
@@ -587,7 +552,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   tc_fence_before();
   __syncthreads();
-  STAMP(cta0 && tid == 0, 21);
   if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
@@ -595,14 +559,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   if (p.nsplit == 1 || p.defer_combine) return;
   combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket, row0, row0 + rows_cta,
                                &p.counters[unit * p.nrg + rg]);
-  STAMP(cta0 && tid == 0, 22);
 }
 
-#ifdef RETRO_STAMPS
-extern "C" int retro_debug_read_stamps(unsigned long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_stamps, sizeof(unsigned long long) * 128);
-}
-#endif
 
 // ---- host: tensor maps over the K / V pools viewed as [(phys * h_k + head) * 16 rows][128 channels] ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,

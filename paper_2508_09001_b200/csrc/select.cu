@@ -18,17 +18,6 @@
 
 namespace retro {
 
-#ifdef RETRO_STAMPS
-__device__ unsigned long long g_sel_stamps[32];
-__device__ __forceinline__ void sel_stamp(int i) {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t) :: "memory");
-  g_sel_stamps[i] = t;
-}
-#define SSTAMP(cond, i) do { if (cond) sel_stamp(i); } while (0)
-#else
-#define SSTAMP(cond, i) do { } while (0)
-#endif
 
 constexpr int kScoreWarps = 8;
 constexpr int kPagesPerWarp = 8;
@@ -154,7 +143,6 @@ __device__ __forceinline__ void topk_mask_block(
       if (lane == 0) { s_lo = kmin; s_width = kmax - kmin; s_need = k_sel; s_done = 0; }
     }
     __syncthreads();
-    SSTAMP(b == 0 && h == 0 && tid == 0, 4);
     // range-adaptive radix select: live range [lo, lo + range], `need` keys still to take from it
     for (int pass = 0; pass < 8; ++pass) {
       const uint64_t lo = s_lo, range = s_width;
@@ -163,7 +151,6 @@ __device__ __forceinline__ void topk_mask_block(
       const int shift = nbits > 11 ? nbits - 11 : 0;
       for (int i = tid; i < kBuckets; i += kTopkThreads) s_hist[i] = 0;
       __syncthreads();
-      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 11);
       for (int i0 = tid; i0 < m; i0 += 8 * kTopkThreads) {   // loads first: they cannot be hoisted over the atomics
         uint64_t kk[8];
 #pragma unroll
@@ -175,7 +162,6 @@ __device__ __forceinline__ void topk_mask_block(
         }
       }
       __syncthreads();
-      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 12);
       // thread i owns kBuckets / NT consecutive buckets, highest first: scanning threads in order walks buckets
       // downward
       constexpr int kPer = kBuckets / NT;
@@ -184,7 +170,6 @@ __device__ __forceinline__ void topk_mask_block(
       for (int u = 0; u < kPer; ++u) { cbk[u] = s_hist[kBuckets - 1 - (tid * kPer + u)]; csum += cbk[u]; }
       int total;
       int run = block_excl_scan<NT>(csum, s_warp, &total, scan_phase);   // keys in strictly higher buckets
-      SSTAMP(b == 0 && h == 0 && tid == 0 && pass == 0, 13);
       int hit = -1, above = 0, cnt = 0;
 #pragma unroll
       for (int u = 0; u < kPer; ++u) {
@@ -201,9 +186,6 @@ __device__ __forceinline__ void topk_mask_block(
         s_done = (cnt == need - above || shift == 0) ? 1 : 0;
       }
       __syncthreads();
-#ifdef RETRO_STAMPS
-      if (b == 0 && h == 0 && tid == 0) g_sel_stamps[10] = g_sel_stamps[0] + pass + 1;
-#endif
       if (s_done) break;
     }
     thr_lo = s_lo;
@@ -211,7 +193,6 @@ __device__ __forceinline__ void topk_mask_block(
     need_in_band = s_need;
   }
 
-  SSTAMP(b == 0 && h == 0 && tid == 0, 5);
   // in-order compaction: thread owns a contiguous chunk of candidate indices
   const int per = (m + kTopkThreads - 1) / kTopkThreads;
   const int i0 = min(tid * per, m), i1 = min(i0 + per, m);
@@ -248,7 +229,6 @@ __device__ __forceinline__ void topk_mask_block(
   if (forced && tid == 0 && count < k_max) sel_s[count] = n_pages - 1;
   if (forced) count = min(count + 1, k_max);
   __syncthreads();
-  SSTAMP(b == 0 && h == 0 && tid == 0, 6);
   // Alg. 2: M.append(A[p]); A[p] <- t.  One selected page per thread, so the A gathers overlap.
   for (int i = tid; i < count; i += kTopkThreads) {
     const int j = sel_s[i];
@@ -275,12 +255,6 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
   constexpr int kVals = Rec<T>::kVals;
   // digest rings [warp][kStages][8 records x 512 B]; the unit's last CTA reuses the space for the top-k keys
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  [[maybe_unused]] const bool u0 = blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0;
-  SSTAMP(u0 && blockIdx.x == 0, 0);
-  unsigned long long t_begin = 0;
-#ifdef RETRO_STAMPS
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_begin) :: "memory");
-#endif
   __shared__ double s_q[kGroupMax ? kMaxGroup : 1][2 * D];   // per q head: [q+ ; q-] (GROUP_MAX) ; row 0 = group sum (GROUP_SUM)
   __shared__ unsigned int s_ticket;
   pdl_wait();
@@ -444,27 +418,16 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 3) select_pages_kernel(
   }   // cta_page0 < n_pages
   // ---- the last CTA of the unit to get here selects (release: barrier, then one cumulative fence) ----
   const size_t unit = (size_t)b * h_k + h;
-  SSTAMP(u0 && blockIdx.x == 0, 1);
   __syncthreads();
   if (threadIdx.x == 0) s_ticket = ticket_acq_rel(&counters[unit]);
   __syncthreads();
   if (s_ticket != gridDim.x - 1) return;
-#ifdef RETRO_STAMPS
-  if (u0) g_sel_stamps[2] = t_begin;
-#endif
-  SSTAMP(u0, 3);
   if (threadIdx.x == 0) counters[unit] = 0;   // leave the workspace consistent for the next call
   topk_mask_block<kScoreWarps * 32>(reinterpret_cast<uint64_t*>(smem_raw), scores, seq_len_b, budget_b,
                                     last_loaded, sel_pages, sel_prev, sel_count, b, h, h_k, max_pages, k_max, P,
                                     force_last);
-  SSTAMP(u0, 9);
 }
 
-#ifdef RETRO_STAMPS
-extern "C" int retro_debug_read_sel_stamps(unsigned long long* host_out) {
-  return (int)cudaMemcpyFromSymbol(host_out, g_sel_stamps, sizeof(unsigned long long) * 32);
-}
-#endif
 
 int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
                         const int32_t* seq_lens, const int32_t* budget_pages, int32_t* last_loaded,

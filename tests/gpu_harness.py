@@ -86,10 +86,38 @@ def check_select(cfg, desc, res, g_pages, g_prev, g_count, A_before, A_after_gpu
     return True
 
 
+def sync_from_oracle(buf, layer, cfg):
+    """Upload the oracle's persistent state (mask A, output cache ring) to the device layer: the CUDA path then
+    continues a trajectory the oracle ran alone (single-step checks from a synced state)."""
+    if cfg.window > 0:
+        buf.last_loaded.copy_(torch.from_numpy(layer.last_loaded))
+        buf.cache_o.copy_(torch.from_numpy(layer.cache_o).float())
+        buf.cache_lse.copy_(torch.from_numpy(layer.cache_lse).float())
+        buf.cache_pos.copy_(torch.from_numpy(layer.cache_pos))
+
+
+def _window(inp, s, first_step):
+    cfg = inp.cfg
+    B = cfg.batch
+    q_win = torch.zeros((B, cfg.window + 1, cfg.num_q_heads, cfg.head_dim), dtype=inp.q_all.dtype)
+    q_pos = torch.full((B, cfg.window + 1), -1, dtype=torch.int32)
+    for b in range(B):
+        for ss in range(max(first_step, s - cfg.window), s + 1):
+            pos = cfg.prompt_lens[b] + ss
+            q_win[b, wl.ring_slot(cfg, pos)] = inp.q_all[ss, b].cpu()
+            q_pos[b, wl.ring_slot(cfg, pos)] = pos
+    return q_win, q_pos
+
+
 def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: int = 0, check_scores=True,
-             desc_kw=None, oracle_kw=None, k_max=None, use_decode_step=False):
-    """Run n_steps decode steps on both sides from decode step `start_step` (window empty at start).
-    Returns dict of max abs errors."""
+             desc_kw=None, oracle_kw=None, k_max=None, use_decode_step=False, warm_steps: int = 0,
+             oracle_batch=None, check_from: int = 0):
+    """Run n_steps decode steps on both sides from decode step `start_step`.  With warm_steps = 0 the retro window
+    is empty at start_step; with warm_steps > 0 the ORACLE ALONE first runs decode steps start_step - warm_steps ..
+    start_step - 1 (from an empty window), its state (A, output cache) is uploaded to the device, and the
+    lock-step starts from that synced state with a (partly) filled window.
+    oracle_batch: the sequences the oracle computes (sampled outputs at full size: the (sequence, KV head) units
+    are independent, the CUDA path always runs the whole batch); default all.  Returns dict of max abs errors."""
     H.require_cuda()
     cfg = inp.cfg
     atol, rtol = TOL[cfg.dtype]
@@ -98,43 +126,54 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
     budget = cfg.budget_pages if budget_pages is None else budget_pages
     desc, buf = make_device_layer(inp, budget, k_max=k_max, **desc_kw)
     okw = dict(oracle_kw)
-    if k_max is not None:
-        okw["max_sel_pages"] = k_max
-    else:
-        okw["max_sel_pages"] = max(1, budget)
-    layer = H.oracle_layer(inp, **okw)
+    okw["max_sel_pages"] = k_max if k_max is not None else max(1, budget)
+    bs = list(range(cfg.batch)) if oracle_batch is None else list(oracle_batch)
+    assert warm_steps == 0 or len(bs) == cfg.batch, "a synced start uploads the oracle state of every sequence"
+    nb = len(bs)
+    sub = cfg.replace(batch=nb, prompt_lens=tuple(cfg.prompt_lens[b] for b in bs))
+    layer = H.oracle_layer(inp, batch_rows=bs, **okw)
     dev = buf.seq_lens.device
     B = cfg.batch
     errs = dict(part_o=0.0, part_lse=0.0, out=0.0, cache_o=0.0, scores_rel=0.0)
+    bud_o = np.full(nb, budget, dtype=np.int32)
+    sub_np = lambda t: t.cpu().numpy()[bs]          # device tensor -> host rows of the oracle's sequences
 
     # prefill digests on both sides
+    first_step = start_step - warm_steps
+    assert first_step >= 0
+    layer.prefill_bounds(np.asarray(sub.prompt_lens) + first_step)
+    for s in range(first_step, start_step):          # oracle alone
+        q_win, q_pos = _window(inp, s, first_step)
+        layer.step(H.np64(q_win[bs]), q_pos.numpy()[bs], H.np64(inp.q_all[s].cpu()[bs]),
+                   inp.seq_lens_at(s).cpu().numpy()[bs], bud_o)
     prompt = np.asarray(cfg.prompt_lens) + start_step
-    layer.prefill_bounds(prompt)
+    if warm_steps > 0:                               # digests of the pages the warm steps touched are current
+        layer.prefill_bounds(prompt[bs])
+        sync_from_oracle(buf, layer, cfg)
     buf.seq_lens.copy_(torch.from_numpy(prompt.astype(np.int32)))
     buf.rebuild_bounds()
     torch.cuda.synchronize()
-    nb = -(-int(prompt.max()) // cfg.page_size)
-    g_bounds = buf.bounds.float().cpu().numpy()
-    for b in range(B):
+    for i, b in enumerate(bs):
         npg = -(-int(prompt[b]) // cfg.page_size)
-        assert np.array_equal(g_bounds[b, :, :npg], layer.bounds[b, :, :npg].astype(np.float32)), "prefill digests"
+        assert np.array_equal(buf.bounds[b, :, :npg].float().cpu().numpy(),
+                              layer.bounds[i, :, :npg].astype(np.float32)), "prefill digests"
+
+    def check_newest_digest(seq_lens):
+        for i, b in enumerate(bs):
+            j = (int(seq_lens[b]) - 1) // cfg.page_size
+            assert np.array_equal(buf.bounds[b, :, j].float().cpu().numpy(),
+                                  layer.bounds[i, :, j].astype(np.float32)), "digest of newest page"
 
     pos_begin = torch.zeros(B, dtype=torch.int32, device=dev)
-    scores_out = torch.zeros((B, cfg.num_kv_heads, cfg.max_pages_per_seq), dtype=torch.float64, device=dev)
+    scores_out = (torch.zeros((B, cfg.num_kv_heads, cfg.max_pages_per_seq), dtype=torch.float64, device=dev)
+                  if check_scores and not use_decode_step else None)
+    bs_t = torch.tensor(bs, dtype=torch.long, device=dev)
     for s in range(start_step, start_step + n_steps):
-        # window of decode steps [max(start, s-w), s]
-        q_win = torch.zeros_like(buf.q_win, device="cpu")
-        q_pos = torch.full((B, cfg.window + 1), -1, dtype=torch.int32)
-        for b in range(B):
-            for ss in range(max(start_step, s - cfg.window), s + 1):
-                pos = cfg.prompt_lens[b] + ss
-                q_win[b, wl.ring_slot(cfg, pos)] = inp.q_all[ss, b].cpu()
-                q_pos[b, wl.ring_slot(cfg, pos)] = pos
+        q_win, q_pos = _window(inp, s, first_step)     # decode steps [max(first_step, s-w), s]
         seq_lens = inp.seq_lens_at(s).cpu().numpy()
         q_cur = inp.q_all[s].cpu()
         A_before = layer.last_loaded.copy() if cfg.window > 0 else None
-        res = layer.step(H.np64(q_win), q_pos.numpy(), H.np64(q_cur), seq_lens,
-                         np.full(B, budget, dtype=np.int32))
+        res = layer.step(H.np64(q_win[bs]), q_pos.numpy()[bs], H.np64(q_cur[bs]), seq_lens[bs], bud_o)
 
         buf.seq_lens.copy_(torch.from_numpy(seq_lens))
         buf.q_win.copy_(q_win); buf.q_pos.copy_(q_pos); buf.q_cur.copy_(q_cur)
@@ -142,13 +181,10 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
             # whole-step entry point: no teacher forcing possible, so only used where selections are tie-free
             rb.retro_decode_step(desc, buf.state, buf.q_win, buf.q_pos, buf.q_cur, buf.out, buf.out_lse)
             torch.cuda.synchronize()
-            g_bounds = buf.bounds.float().cpu().numpy()      # S1 runs inside the select kernel on this path
-            for b in range(B):
-                j = (int(seq_lens[b]) - 1) // cfg.page_size
-                assert np.array_equal(g_bounds[b, :, j], layer.bounds[b, :, j].astype(np.float32)), "digest of newest page"
-            assert np.array_equal(buf.sel_pages.cpu().numpy(), res["sel_pages"])
+            check_newest_digest(seq_lens)                 # S1 runs inside the select kernel on this path
+            assert np.array_equal(sub_np(buf.sel_pages), res["sel_pages"]), f"step {s} sel_pages"
             if cfg.window > 0:      # w = 0: no past rows, the mask list is not used (A is optional there)
-                assert np.array_equal(buf.sel_prev.cpu().numpy(), res["sel_prev"])
+                assert np.array_equal(sub_np(buf.sel_prev), res["sel_prev"]), f"step {s} sel_prev"
         else:
             # S1
             pos_begin.copy_(torch.from_numpy((seq_lens - 1).astype(np.int32)))
@@ -156,31 +192,27 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
             # S2
             la = buf.last_loaded if cfg.window > 0 else None
             rb.retro_select_pages(desc, buf.q_cur, buf.bounds, buf.seq_lens, buf.budget_pages, la, buf.sel_pages,
-                                  buf.sel_prev, buf.sel_count, scores_out if check_scores else None, buf.workspace)
+                                  buf.sel_prev, buf.sel_count, scores_out, buf.workspace)
             torch.cuda.synchronize()
-            g_bounds = buf.bounds.float().cpu().numpy()
-            for b in range(B):
-                j = (int(seq_lens[b]) - 1) // cfg.page_size
-                assert np.array_equal(g_bounds[b, :, j], layer.bounds[b, :, j].astype(np.float32)), "digest of newest page"
-            if check_scores:
-                gs = scores_out.cpu().numpy()
-                for b in range(B):
-                    npg = -(-int(seq_lens[b]) // cfg.page_size)
-                    ref = res["scores"][b, :, :npg]
-                    rel = np.abs(gs[b, :, :npg] - ref) / np.maximum(1.0, np.abs(ref))
+            check_newest_digest(seq_lens)
+            if scores_out is not None:
+                gs = sub_np(scores_out)
+                for i in range(nb):
+                    npg = -(-int(seq_lens[bs[i]]) // cfg.page_size)
+                    ref = res["scores"][i, :, :npg]
+                    rel = np.abs(gs[i, :, :npg] - ref) / np.maximum(1.0, np.abs(ref))
                     assert rel.max() < 1e-12, f"fp64 scores differ: {rel.max()}"
                     errs["scores_rel"] = max(errs["scores_rel"], float(rel.max()))
-                    assert np.all(np.isneginf(gs[b, :, npg:]))
-            check_select(cfg, desc, res, buf.sel_pages.cpu().numpy(), buf.sel_prev.cpu().numpy(),
-                         buf.sel_count.cpu().numpy(), A_before,
-                         buf.last_loaded.cpu().numpy() if cfg.window > 0 else None, seq_lens,
+                    assert np.all(np.isneginf(gs[i, :, npg:]))
+            check_select(sub, desc, res, sub_np(buf.sel_pages), sub_np(buf.sel_prev), sub_np(buf.sel_count), A_before,
+                         sub_np(buf.last_loaded) if cfg.window > 0 else None, seq_lens[bs],
                          force_last=desc.force_last_page != 0)
-            # teacher forcing
-            buf.sel_pages.copy_(torch.from_numpy(res["sel_pages"]))
-            buf.sel_prev.copy_(torch.from_numpy(res["sel_prev"]))
-            buf.sel_count.copy_(torch.from_numpy(res["sel_count"]))
+            # teacher forcing (the oracle's sequences; the others keep the device's own selection)
+            buf.sel_pages[bs_t] = torch.from_numpy(res["sel_pages"]).to(dev)
+            buf.sel_prev[bs_t] = torch.from_numpy(res["sel_prev"]).to(dev)
+            buf.sel_count[bs_t] = torch.from_numpy(res["sel_count"]).to(dev)
             if cfg.window > 0:
-                buf.last_loaded.copy_(torch.from_numpy(layer.last_loaded))
+                buf.last_loaded[bs_t] = torch.from_numpy(layer.last_loaded).to(dev)
             # S3
             rb.retro_sparse_attend(desc, buf.q_win, buf.q_pos, buf.k_pages, buf.v_pages, buf.block_table,
                                    buf.seq_lens, buf.sel_pages, buf.sel_prev, buf.sel_count, buf.part_o,
@@ -192,14 +224,17 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
             rb.retro_merge_output_cache(desc, buf.part_o, buf.part_lse, buf.q_pos, buf.seq_lens, co, cl, cp,
                                         buf.out, buf.out_lse)
             torch.cuda.synchronize()
-            errs["part_o"] = max(errs["part_o"], close(buf.part_o.cpu().numpy(), res["part_o"], atol, rtol, f"step {s} part_o"))
-            errs["part_lse"] = max(errs["part_lse"], close(buf.part_lse.cpu().numpy(), res["part_lse"], atol, rtol, f"step {s} part_lse"))
-        errs["out"] = max(errs["out"], close(buf.out.float().cpu().numpy(), res["out"], atol, rtol, f"step {s} out"))
-        close(buf.out_lse.cpu().numpy(), res["out_lse"], atol, rtol, f"step {s} out_lse")
+            if s - start_step >= check_from:
+                errs["part_o"] = max(errs["part_o"], close(sub_np(buf.part_o), res["part_o"], atol, rtol, f"step {s} part_o"))
+                errs["part_lse"] = max(errs["part_lse"], close(sub_np(buf.part_lse), res["part_lse"], atol, rtol, f"step {s} part_lse"))
+        if s - start_step < check_from:
+            continue
+        errs["out"] = max(errs["out"], close(sub_np(buf.out.float()), res["out"], atol, rtol, f"step {s} out"))
+        close(sub_np(buf.out_lse), res["out_lse"], atol, rtol, f"step {s} out_lse")
         if cfg.window > 0:
-            assert np.array_equal(buf.cache_pos.cpu().numpy(), layer.cache_pos), f"step {s} cache_pos"
+            assert np.array_equal(sub_np(buf.cache_pos), layer.cache_pos), f"step {s} cache_pos"
             live = layer.cache_pos >= 0
-            co_g, cl_g = buf.cache_o.cpu().numpy(), buf.cache_lse.cpu().numpy()
+            co_g, cl_g = sub_np(buf.cache_o), sub_np(buf.cache_lse)
             errs["cache_o"] = max(errs["cache_o"], close(co_g[live], layer.cache_o[live], atol, rtol, f"step {s} cache_o"))
             close(cl_g[live], layer.cache_lse[live], atol, rtol, f"step {s} cache_lse")
     return errs

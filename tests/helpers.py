@@ -24,10 +24,14 @@ def oracle_desc(cfg: wl.RetroConfig, **kw) -> orc.OracleDesc:
     return orc.OracleDesc(**d)
 
 
-def oracle_layer(inp: wl.LayerInputs, **kw) -> orc.OracleLayer:
+def oracle_layer(inp: wl.LayerInputs, batch_rows=None, **kw) -> orc.OracleLayer:
+    """batch_rows: the sequences the oracle computes (units are independent; the pools are shared)."""
+    bt = inp.block_table.cpu().numpy()
+    if batch_rows is not None and list(batch_rows) != list(range(inp.cfg.batch)):
+        kw = dict(kw, batch=len(batch_rows))
+        bt = bt[list(batch_rows)]
     desc = oracle_desc(inp.cfg, **kw)
-    return orc.OracleLayer(desc, inp.k_pages.float().cpu().numpy(), inp.v_pages.float().cpu().numpy(),
-                           inp.block_table.cpu().numpy())
+    return orc.OracleLayer(desc, inp.k_pages.float().cpu().numpy(), inp.v_pages.float().cpu().numpy(), bt)
 
 
 def np64(x: torch.Tensor) -> np.ndarray:

@@ -177,22 +177,59 @@ def test_c2_full_context_whole_step_entry_point():
     print("c2 full whole-step errs", GH.lockstep(inp, 11, use_decode_step=True))
 
 
-def test_c4_full_context_sampled_steps():
-    cfg = wl.c4(n_steps=3)
+# ---- FULL-size configurations, retro window FULL for >= 2 checked steps (Alg. 1's Q_{i:t}).
+# The CUDA path runs the whole batch in bench.py's launch configuration; the oracle computes a sample of the
+# sequences (the (sequence, KV head) units are independent), every KV head and every window row of them.
+def test_c3_full_batch_window_full():
+    cfg = wl.c3(n_steps=19)
     inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
-    print("c4 full errs", GH.lockstep(inp, 3))
+    print("c3 full errs", GH.lockstep(inp, 19, oracle_batch=(0, 7, 15), check_scores=False))
 
 
-def test_c3_full_batch_sampled_steps():
-    cfg = wl.c3(n_steps=3)
+def test_c4_full_context_window_full():
+    cfg = wl.c4(n_steps=11)
     inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
-    print("c3 full errs", GH.lockstep(inp, 3))
+    print("c4 full errs", GH.lockstep(inp, 11, oracle_batch=(0, 3)))
 
 
-def test_c5_full_point_w8_budget4096():
-    cfg = wl.c5(8, 4096, n_steps=2)
+def test_c5_full_point_w8_budget4096_window_full():
+    cfg = wl.c5(8, 4096, n_steps=11)
     inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
-    print("c5 full errs", GH.lockstep(inp, 2))
+    print("c5 full errs", GH.lockstep(inp, 11, oracle_batch=(0, 5), check_scores=False))
+
+
+@pytest.mark.parametrize("w,budget", [(16, 4096), (32, 2048), (8, 8192), (2, 512), (4, 1024)])
+def test_c5_full_sweep_points_whole_step(w, budget):
+    """FULL-size C5 sweep points through retro_decode_step (the call bench.py times), no teacher forcing, w + 2
+    steps: the window is full on the last two.  (8, 8192) is the bench line's `bandwidth_point`."""
+    cfg = wl.c5(w, budget, n_steps=w + 2)
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c5 sweep errs", w, budget, GH.lockstep(inp, w + 2, oracle_batch=(0, 5), use_decode_step=True))
+
+
+@pytest.mark.parametrize("use_step", [False, True])
+def test_multi_block_wide_rows_window_full(use_step):
+    """C3 shape shrunk: 128 units (one split each), 128 selected pages = 16 key blocks per CTA, 68 rows (NT = 80,
+    a single P buffer), window full on the last two steps."""
+    cfg = wl.shrink(wl.c3(), tuple(2500 - 61 * b for b in range(16)), 18)
+    inp = wl.make_layer_inputs(cfg)
+    print("multi-block wide errs", GH.lockstep(inp, 18, oracle_batch=(0, 9), use_decode_step=use_step, check_from=8))
+
+
+def test_multi_block_wide_rows_gqa7_window_full():
+    """G = 7 with w = 11: 84 rows (NT = 96), 40 units, several key blocks per CTA, window full at the end."""
+    cfg = wl.shrink(wl.c4(), tuple(2700 - 37 * b for b in range(10)), 14, batch=10, budget_tokens=2048, window=11)
+    inp = wl.make_layer_inputs(cfg)
+    print("multi-block G7 errs", GH.lockstep(inp, 14, oracle_batch=(0, 6), check_from=6))
+
+
+def test_c2_full_context_late_steps_from_synced_state():
+    """C2 near the END of its trajectory (decode steps 4080-4082 of 4096, 36 848-token context): the oracle alone
+    runs the 9 steps before, its mask A and output cache are uploaded, then both sides step from that state."""
+    cfg = wl.c2()
+    inp = _to_cpu(wl.make_layer_inputs(cfg, device="cuda"))
+    print("c2 late errs", GH.lockstep(inp, 3, start_step=4080, warm_steps=9))
+    print("c2 late whole-step errs", GH.lockstep(inp, 3, start_step=4080, warm_steps=9, use_decode_step=True))
 
 
 def test_append_kv_and_window_advance_match_pregenerated_pool():
