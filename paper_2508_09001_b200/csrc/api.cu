@@ -12,6 +12,79 @@ std::mutex& host_mutex() {
   return m;
 }
 
+DeviceInfo device_info() {
+  constexpr int kMaxDev = 64;
+  static DeviceInfo table[kMaxDev];
+  static bool known[kMaxDev];
+  DeviceInfo fallback{-1, 148, 232448};   // B200; used when no device is present (CPU-only symbol / header tests)
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) {
+    (void)cudaGetLastError();
+    return fallback;
+  }
+  std::lock_guard<std::mutex> lock(host_mutex());
+  if (dev < kMaxDev && known[dev]) return table[dev];
+  DeviceInfo di{dev, 148, 232448};
+  int v = 0;
+  if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) di.sm_count = v;
+  if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess && v > 0)
+    di.max_smem_optin = v;
+  if (dev < kMaxDev) { table[dev] = di; known[dev] = true; }
+  return di;
+}
+
+int ensure_dynamic_smem(const void* kern, size_t smem_bytes) {
+  if (smem_bytes <= 48 * 1024) return RETRO_OK;
+  struct Entry { int dev; const void* kern; size_t granted; };
+  constexpr int kEntries = 256;
+  static Entry tab[kEntries];
+  static int n_used = 0;
+  int dev = 0;
+  RETRO_CUDA_TRY(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(host_mutex());
+  Entry* e = nullptr;
+  for (int i = 0; i < n_used && e == nullptr; ++i)
+    if (tab[i].dev == dev && tab[i].kern == kern) e = &tab[i];
+  if (e != nullptr && e->granted >= smem_bytes) return RETRO_OK;
+  RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+  if (e == nullptr && n_used < kEntries) e = &tab[n_used++];   // table full: the attribute is simply set again
+  if (e != nullptr) { e->dev = dev; e->kern = kern; e->granted = smem_bytes; }
+  return RETRO_OK;
+}
+
+bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cluster_x, int min_clusters) {
+  struct Entry { int dev; const void* kern; size_t smem; int cluster; int max_active; };
+  constexpr int kEntries = 256;
+  static Entry tab[kEntries];
+  static int n_used = 0;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+  std::lock_guard<std::mutex> lock(host_mutex());
+  for (int i = 0; i < n_used; ++i)
+    if (tab[i].dev == dev && tab[i].kern == kern && tab[i].smem == smem_bytes && tab[i].cluster == cluster_x)
+      return tab[i].max_active >= min_clusters;
+  int max_active = 0;
+  bool ok = true;
+  if (cluster_x > 8) ok = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+  if (ok) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cluster_x * (min_clusters > 0 ? min_clusters : 1), 1, 1);
+    cfg.blockDim = dim3(block_threads);
+    cfg.dynamicSmemBytes = smem_bytes;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cluster_x;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ok = cudaOccupancyMaxActiveClusters(&max_active, kern, &cfg) == cudaSuccess;
+  }
+  if (!ok) { (void)cudaGetLastError(); max_active = 0; }
+  if (n_used < kEntries) tab[n_used++] = Entry{dev, kern, smem_bytes, cluster_x, max_active};
+  return max_active >= min_clusters;
+}
+
 int validate_desc(const retro_desc_t* d) {
   if (d == nullptr) return RETRO_ERR_ARG;
   if (d->batch <= 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->head_dim <= 0 || d->page_size <= 0 ||
@@ -55,6 +128,8 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   size_t off = 0;
   wl.scores_off = off;
   off = align_up(off + (size_t)units * d->max_pages_per_seq * sizeof(double), 256);
+  wl.amb_idx_off = off;
+  off = align_up(off + (size_t)units * d->max_pages_per_seq * sizeof(int32_t), 256);
   wl.split_o_off = off;
   off = align_up(off + (size_t)units * wl.nsplit * wl.rows * d->head_dim * sizeof(float), 256);
   wl.split_lse_off = off;

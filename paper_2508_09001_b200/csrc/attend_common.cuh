@@ -13,9 +13,12 @@ struct AttendParams {
   const int32_t* sel_count; float* part_o; float* part_lse; float* split_o; float* split_lse;
   unsigned int* counters;
   int B, h_q, h_k, max_pages, k_max, window, nsplit, pages_per_split;
-  int defer_combine;   // 1: leave the split partials in the workspace (a combine + merge kernel follows)
-  int nrg, rg_rows;   // query-row groups of the tensor-core path (rows > 128): CTA (split, group) owns rg_rows rows
+  int nrg, rg_ranks;  // query-row groups of the tensor-core path (rows > 128): the CTAs of group rg own the window
+                      // ranks (t - position) [rg * rg_ranks, (rg + 1) * rg_ranks), i.e. rg_ranks * G query rows
   float scale_log2;   // sm_scale * log2(e)
+  // tensor-core path inside retro_decode_step (fused = 1, nrg == 1): S4 runs in the same kernel
+  int fused;
+  float* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse; unsigned int* seq_counters;
 };
 
 #ifdef __CUDACC__

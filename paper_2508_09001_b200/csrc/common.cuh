@@ -28,9 +28,24 @@ void set_cuda_error(cudaError_t e);
   } while (0)
 #define RETRO_LAUNCH_CHECK() RETRO_CUDA_TRY(cudaGetLastError())
 
-// Host-side launcher state (tensor-map cache, raised shared-memory limits) is guarded by one mutex, so the entry
-// points may be called from several host threads; apart from that and the last CUDA error there is no global state.
+// Host-side launcher state (tensor-map cache, per-device facts, raised shared-memory limits) is guarded by one
+// mutex, so the entry points may be called from several host threads; apart from that and the last CUDA error
+// there is no global state.
 std::mutex& host_mutex();   // api.cu
+
+// Facts about the CURRENT device, queried once per device (api.cu).  Without a device (header / symbol tests on a
+// CPU-only box) the B200 values are assumed.
+struct DeviceInfo {
+  int device;          // ordinal, -1 = no device
+  int sm_count;        // multiProcessorCount
+  int max_smem_optin;  // bytes of dynamic shared memory a CTA may opt in to
+};
+DeviceInfo device_info();
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: remembers per (device, kernel) what was granted.
+int ensure_dynamic_smem(const void* kern, size_t smem_bytes);   // RETRO_OK / RETRO_ERR_CUDA
+// Can `min_clusters` clusters of cluster_x CTAs of this kernel be resident at once on the current device?  Sizes above
+// 8 opt the kernel in to non-portable cluster sizes.  Cached per (device, kernel, shared memory, cluster size).
+bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cluster_x, int min_clusters);
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
@@ -39,7 +54,8 @@ int validate_desc(const retro_desc_t* d);  // RETRO_OK / RETRO_ERR_ARG / RETRO_E
 
 // ---- workspace layout (host + device agree through this struct) --------------------------------
 struct WorkspaceLayout {
-  size_t scores_off;    // double [B][h_k][max_pages]
+  size_t scores_off;    // uint64 [B][h_k][max_pages]: fp64 keys of the select kernel's exact refinement
+  size_t amb_idx_off;   // int32  [B][h_k][max_pages]: the pages those keys belong to
   size_t split_o_off;   // float  [B][h_k][nsplit][rows][d]
   size_t split_lse_off; // float  [B][h_k][nsplit][rows]
   size_t slot_counters_off;  // uint32 [B][w+1]: arrivals per (sequence, cache slot) of the combine + merge kernel
@@ -98,25 +114,87 @@ int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int3
 // start launching (pdl_trigger).  The next kernel's launch latency, CTA scheduling and shared-memory / TMEM
 // set-up overlap the current kernel (also inside a captured CUDA graph); the data dependence is unchanged and at
 // most two kernels are resident at a time (triggering before the wait let the whole chain pile up on the SMs).
-// RETRO_PDL=0 turns the attribute off (griddepcontrol.* are then no-ops).
+// Compiling with -DRETRO_NO_PDL leaves the attribute out (griddepcontrol.* are then no-ops).
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-inline bool pdl_enabled() {
-  static const bool on = [] { const char* e = getenv("RETRO_PDL"); return e == nullptr || e[0] != '0'; }();
-  return on;
+// cluster_x > 1: thread-block cluster of cluster_x CTAs along grid x (gridDim.x must be a multiple of it).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_cluster_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                         int cluster_x, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute attr[2];
+  int n = 0;
+#ifndef RETRO_NO_PDL
+  attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[n].val.programmaticStreamSerializationAllowed = 1;
+  ++n;
+#endif
+  if (cluster_x > 1) {
+    attr[n].id = cudaLaunchAttributeClusterDimension;
+    attr[n].val.clusterDim.x = (unsigned)cluster_x;
+    attr[n].val.clusterDim.y = 1;
+    attr[n].val.clusterDim.z = 1;
+    ++n;
+  }
+  cfg.attrs = attr;
+  cfg.numAttrs = n;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
                                  Args... args) {
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = pdl_enabled() ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+  return launch_cluster_kernel(kern, grid, block, smem, s, 1, args...);
+}
+
+// ---- thread-block clusters: rank, barrier, distributed shared memory --------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+  return r;
+}
+// release / acquire at cluster scope: shared-memory writes (local and remote) before the arrive are visible to
+// every CTA of the cluster after its wait.  Executed by ALL threads of every CTA of the cluster.
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// address of `local_smem_addr` (shared::cta window) in CTA `rank`'s shared memory (shared::cluster window)
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local_smem_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_smem_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void dsmem_st_u32(uint32_t addr, uint32_t v) {
+  asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void dsmem_st_f32(uint32_t addr, float v) {
+  asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void dsmem_st_v4(uint32_t addr, float4 v) {
+  asm volatile("st.shared::cluster.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w)
+               : "memory");
+}
+__device__ __forceinline__ float4 dsmem_ld_v4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr)
+               : "memory");
+  return v;
+}
+__device__ __forceinline__ float dsmem_ld_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void dsmem_red_min_u32(uint32_t addr, uint32_t v) {
+  asm volatile("red.relaxed.cluster.shared::cluster.min.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void dsmem_red_max_u32(uint32_t addr, uint32_t v) {
+  asm volatile("red.relaxed.cluster.shared::cluster.max.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
 // ---- device helpers ---------------------------------------------------------------------------

@@ -111,7 +111,7 @@ def _window(inp, s, first_step):
 
 def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: int = 0, check_scores=True,
              desc_kw=None, oracle_kw=None, k_max=None, use_decode_step=False, warm_steps: int = 0,
-             oracle_batch=None, check_from: int = 0):
+             oracle_batch=None, check_from: int = 0, exact_select=False):
     """Run n_steps decode steps on both sides from decode step `start_step`.  With warm_steps = 0 the retro window
     is empty at start_step; with warm_steps > 0 the ORACLE ALONE first runs decode steps start_step - warm_steps ..
     start_step - 1 (from an empty window), its state (A, output cache) is uploaded to the device, and the
@@ -204,6 +204,8 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
                     assert rel.max() < 1e-12, f"fp64 scores differ: {rel.max()}"
                     errs["scores_rel"] = max(errs["scores_rel"], float(rel.max()))
                     assert np.all(np.isneginf(gs[i, :, npg:]))
+            if exact_select:
+                assert np.array_equal(sub_np(buf.sel_pages), res["sel_pages"]), f"step {s} sel_pages (exact)"
             check_select(sub, desc, res, sub_np(buf.sel_pages), sub_np(buf.sel_prev), sub_np(buf.sel_count), A_before,
                          sub_np(buf.last_loaded) if cfg.window > 0 else None, seq_lens[bs],
                          force_last=desc.force_last_page != 0)

@@ -162,6 +162,33 @@ def test_edge_exact_score_ties_resolve_to_lower_index():
     GH.lockstep(inp, 3)
 
 
+@pytest.mark.parametrize("base", ["f32", "bf16"])
+def test_select_adversarial_near_ties_are_ranked_exactly(base):
+    """Scores crowded around the k-th one: every page has the same keys except one channel that is shifted by a
+    page-dependent amount, so the Eq. 1 scores differ by gaps from far below to far above the fp32 error of the
+    streamed score (fp32: 1e-7 .. 1e-3 relative; bf16: whole ulps on a channel the query weighs lightly, plus
+    exact ties).  The selection must be the fp64 oracle's, index for index: the fp32 pre-selection has to notice
+    that it cannot decide and rank the undecided pages in fp64."""
+    if base == "f32":
+        cfg = wl.shrink(wl.c1(), (3000,), 3, budget_tokens=40 * 16, window=2)
+    else:
+        cfg = wl.shrink(wl.c2(), (3000,), 3, budget_tokens=40 * 16, window=2)
+    inp = wl.make_layer_inputs(cfg)
+    g = torch.Generator().manual_seed(77)
+    npg = inp.k_pages.shape[0]
+    row = inp.k_pages[0, :, 0].clone()                               # [h_k][d]: one key row per KV head
+    k = row[None, :, None, :].repeat(npg, 1, cfg.page_size, 1).float()
+    if base == "f32":
+        shift = 10.0 ** (-7.0 + 4.0 * torch.rand(npg, generator=g)) * torch.randint(0, 3, (npg,), generator=g)
+        k[:, :, :, 0] += (k[:, :, :, 0].abs() + 1.0) * shift[:, None, None]
+    else:
+        ulps = torch.randint(0, 4, (npg,), generator=g).float()      # 0..3 bf16 ulps on channel 0: many exact ties
+        k[:, :, :, 0] = (k[:, :, :, 0].abs() + 1.0) * (1.0 + ulps[:, None, None] * 2.0 ** -7)
+    inp.k_pages[:] = k.to(inp.k_pages.dtype)
+    print("near-tie errs", base, GH.lockstep(inp, 3, exact_select=True))
+    GH.lockstep(inp, 3, use_decode_step=True)
+
+
 def test_c2_full_context_sampled_steps():
     """FULL C2 context (32768-token prompt), the launch configuration bench.py times; first steps + ramp-up."""
     cfg = wl.c2(n_steps=12)
