@@ -33,8 +33,8 @@ DeviceInfo device_info() {
   return di;
 }
 
-int ensure_dynamic_smem(const void* kern, size_t smem_bytes) {
-  if (smem_bytes <= 48 * 1024) return RETRO_OK;
+int ensure_dynamic_smem(const void* kern, size_t smem_bytes, bool max_carveout) {
+  if (smem_bytes <= 48 * 1024 && !max_carveout) return RETRO_OK;
   struct Entry { int dev; const void* kern; size_t granted; };
   constexpr int kEntries = 256;
   static Entry tab[kEntries];
@@ -47,6 +47,9 @@ int ensure_dynamic_smem(const void* kern, size_t smem_bytes) {
     if (tab[i].dev == dev && tab[i].kern == kern) e = &tab[i];
   if (e != nullptr && e->granted >= smem_bytes) return RETRO_OK;
   RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+  if (max_carveout)
+    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                        cudaSharedmemCarveoutMaxShared));
   if (e == nullptr && n_used < kEntries) e = &tab[n_used++];   // table full: the attribute is simply set again
   if (e != nullptr) { e->dev = dev; e->kern = kern; e->granted = smem_bytes; }
   return RETRO_OK;
@@ -108,23 +111,30 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   WorkspaceLayout wl;
   const int units = d->batch * d->num_kv_heads;
   wl.rows = (d->window + 1) * (d->num_q_heads / d->num_kv_heads);
-  // split-KV.  Scalar path: units * nsplit covers the 148 SMs about twice, at least 2 pages per split.  The
-  // tensor-core path (bf16) consumes pages in blocks of 8 and writes a rows x 128 fp32 partial per split: its
-  // splits are whole blocks and the grid (units x row groups x splits) is at most ONE wave of resident CTAs
-  // (one CTA per SM).  More than 128 query rows are handled as ceil(rows / 128) balanced row groups.
+  // split-KV.  Scalar path: units * nsplit covers the SMs about twice, at least 2 pages per split.  The
+  // tensor-core path (bf16) consumes pages in blocks of 8; the splits of a (unit, row group) are the CTAs of one
+  // thread-block cluster (<= 8) that combine their partials through distributed shared memory, and the grid
+  // (units x row groups x splits) is at most ONE wave of resident CTAs (one CTA per SM).  More than 128 query
+  // rows are handled as row groups of whole window ranks (G rows each).
   const bool umma = d->dtype == RETRO_BF16;
+  const int sm_count = device_info().sm_count;
+  const int G = d->num_q_heads / d->num_kv_heads, R = d->window + 1;
   wl.nrg = umma ? ceil_div(wl.rows, 128) : 1;
-  wl.rg_rows = ceil_div(wl.rows, wl.nrg);
-  int nsplit = umma ? 148 / (units * wl.nrg) : ceil_div(2 * 148, units);
+  wl.rg_ranks = ceil_div(R, wl.nrg);
+  while (umma && wl.rg_ranks * G > 128) { ++wl.nrg; wl.rg_ranks = ceil_div(R, wl.nrg); }
+  int nsplit = umma ? sm_count / (units * wl.nrg) : ceil_div(2 * sm_count, units);
+  if (umma && nsplit > 8) nsplit = 8;
   const int min_pages = umma ? 8 : 2;
   const int max_split = d->max_sel_pages >= min_pages ? d->max_sel_pages / min_pages : 1;
   if (nsplit > max_split) nsplit = max_split;
   if (nsplit < 1) nsplit = 1;
   wl.pages_per_split = ceil_div(d->max_sel_pages, nsplit);
   if (umma) wl.pages_per_split = ceil_div(wl.pages_per_split, 8) * 8;
-  // the page list of a split lives in shared memory: very large budgets take more splits (and waves) instead
-  if (umma && wl.pages_per_split > 1024) wl.pages_per_split = 1024;
+  // the page list of a split lives in shared memory (<= 2048 pages x 8 splits = the 16 384-page limit); the
+  // scalar path's list is capped the same way and takes more splits instead
+  if (wl.pages_per_split > 2048) wl.pages_per_split = 2048;
   wl.nsplit = ceil_div(d->max_sel_pages, wl.pages_per_split);
+  if (umma && wl.nsplit > 8) wl.nsplit = 8;   // (unreachable within the limits of validate_desc)
   size_t off = 0;
   wl.scores_off = off;
   off = align_up(off + (size_t)units * d->max_pages_per_seq * sizeof(double), 256);
@@ -335,20 +345,17 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, c
                            st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s, st->k_pages,
                            st->block_table);
   if (rc != RETRO_OK) return rc;
-  // S3; on the tensor-core path with several splits the attend kernel leaves its split partials uncombined and
-  // ONE kernel does the split combine and S4 (the partials and the cache operands ride the same round trip)
-  bool deferred = true;
-  rc = launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
-                            st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s,
-                            &deferred);
-  if (rc != RETRO_OK) return rc;
-  if (deferred) {
-    char* ws = static_cast<char*>(st->workspace);
-    return launch_combine_merge(desc, reinterpret_cast<const float*>(ws + wl.split_o_off),
-                                reinterpret_cast<const float*>(ws + wl.split_lse_off), wl.nsplit, wl.rows, st->part_o,
-                                st->part_lse, q_pos, st->seq_lens, st->cache_o, st->cache_lse, st->cache_pos, out,
-                                out_lse, reinterpret_cast<unsigned int*>(ws + wl.slot_counters_off), s);
+  // S3 (+ S4): on the tensor-core path with one row group the attend kernel also merges the output cache (the
+  // splits of a unit are one cluster: split combine and Eq. 8-9 in its epilogue, TWO launches per layer-step)
+  if (attend_can_fuse_merge(desc, wl)) {
+    const FusedMerge fm{st->cache_o, st->cache_lse, st->cache_pos, out, out_lse};
+    return launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
+                                st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s,
+                                &fm);
   }
+  rc = launch_sparse_attend(desc, wl, q_win, q_pos, st->k_pages, st->v_pages, st->block_table, st->seq_lens,
+                            st->sel_pages, st->sel_prev, st->sel_count, st->part_o, st->part_lse, st->workspace, s);
+  if (rc != RETRO_OK) return rc;
   return launch_merge_output_cache(desc, st->part_o, st->part_lse, q_pos, st->seq_lens, st->cache_o, st->cache_lse,
                                    st->cache_pos, out, out_lse, s);
 }

@@ -10,8 +10,6 @@
 // combines them (LSE merge, Eq. 8 applied to splits) into part_o / part_lse.
 //
 // This is the scalar-ALU path: exact fp32 products (C1's 1e-4 tolerance rules out TF32) and small row blocks.
-#include <cstdlib>
-
 #include "attend_common.cuh"
 
 namespace retro {
@@ -241,12 +239,9 @@ static int launch_simt(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   const size_t smem = (size_t)kStages * 2 * 16 * D * sizeof(T) + (size_t)rows * D * sizeof(T) +
                       (size_t)3 * prm.pages_per_split * sizeof(int32_t) + 8 + kStages * sizeof(uint64_t);
   auto kern = attend_simt_kernel<T, D, RPW>;
-  std::lock_guard<std::mutex> lock(host_mutex());
-  static size_t smem_allowed = 0;   // per instantiation; raised on demand (not a stream operation)
-  if (smem > smem_allowed) {
-    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    smem_allowed = smem;
-  }
+  if (smem > (size_t)device_info().max_smem_optin) return RETRO_ERR_UNSUPPORTED;
+  const int rc = ensure_dynamic_smem((const void*)kern, smem);
+  if (rc != RETRO_OK) return rc;
   RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit, d->num_kv_heads, d->batch), dim3(kAttWarps * 32), smem, s, prm));
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
@@ -265,46 +260,44 @@ static int dispatch_rpw(const retro_desc_t* d, const AttendParams& prm, cudaStre
   return RETRO_ERR_UNSUPPORTED;
 }
 
+bool attend_can_fuse_merge(const retro_desc_t* d, const WorkspaceLayout& wl) {
+  return d->dtype == RETRO_BF16 && wl.nrg == 1;
+}
+
 int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_win, const int32_t* q_pos,
                          const void* k_pages, const void* v_pages, const int32_t* block_table,
                          const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,
                          const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s,
-                         bool* defer_combine) {
+                         const FusedMerge* fused) {
   AttendParams prm;
-  const bool may_defer = defer_combine != nullptr && *defer_combine;
-  if (defer_combine != nullptr) *defer_combine = false;
-  prm.defer_combine = 0;
   char* ws = static_cast<char*>(workspace);
   prm.q_win = q_win; prm.q_pos = q_pos; prm.k_pages = k_pages; prm.v_pages = v_pages;
   prm.block_table = block_table; prm.seq_lens = seq_lens; prm.sel_pages = sel_pages; prm.sel_prev = sel_prev;
   prm.sel_count = sel_count; prm.part_o = part_o; prm.part_lse = part_lse;
   prm.split_o = reinterpret_cast<float*>(ws + wl.split_o_off);
   prm.split_lse = reinterpret_cast<float*>(ws + wl.split_lse_off);
-  prm.counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;   // [units][nrg]
+  prm.counters = reinterpret_cast<unsigned int*>(ws + wl.counters_off) + d->batch * d->num_kv_heads;   // [units]
   prm.B = d->batch; prm.h_q = d->num_q_heads; prm.h_k = d->num_kv_heads; prm.max_pages = d->max_pages_per_seq;
   prm.k_max = d->max_sel_pages; prm.window = d->window; prm.nsplit = wl.nsplit;
   prm.pages_per_split = wl.pages_per_split;
   prm.scale_log2 = d->sm_scale * kLog2e;
-  prm.nrg = 1;
-  prm.rg_rows = wl.rows;
+  prm.nrg = wl.nrg;
+  prm.rg_ranks = wl.rg_ranks;
+  prm.fused = 0;
+  prm.cache_o = nullptr; prm.cache_lse = nullptr; prm.cache_pos = nullptr; prm.out = nullptr; prm.out_lse = nullptr;
+  prm.seq_counters = reinterpret_cast<unsigned int*>(ws + wl.slot_counters_off);   // [B]
   if (d->dtype == RETRO_BF16) {
     // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu; more than 128
-    // rows run as row groups).  The scalar path stays reachable for debugging (RETRO_ATTEND_PATH=simt).
-    static const bool force_simt = [] {
-      const char* e = std::getenv("RETRO_ATTEND_PATH");
-      return e != nullptr && e[0] == 's';
-    }();
-    if (!force_simt) {
-      prm.nrg = wl.nrg;
-      prm.rg_rows = wl.rg_rows;
-      if (may_defer && wl.nsplit > 1) {
-        prm.defer_combine = 1;
-        *defer_combine = true;
-      }
-      return launch_attend_umma(d, prm, s);
+    // rows run as row groups)
+    if (fused != nullptr) {
+      if (!attend_can_fuse_merge(d, wl)) return RETRO_ERR_UNSUPPORTED;
+      prm.fused = 1;
+      prm.cache_o = fused->cache_o; prm.cache_lse = fused->cache_lse; prm.cache_pos = fused->cache_pos;
+      prm.out = fused->out; prm.out_lse = fused->out_lse;
     }
-    return dispatch_rpw<__nv_bfloat16, 128>(d, prm, s);
+    return launch_attend_umma(d, prm, s);
   }
+  if (fused != nullptr) return RETRO_ERR_UNSUPPORTED;
   return dispatch_rpw<float, 64>(d, prm, s);
 }
 

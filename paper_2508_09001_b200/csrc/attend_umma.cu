@@ -125,6 +125,13 @@ __device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t* r) {
                ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3])
                : "memory");
 }
+__device__ __forceinline__ void store_bf16x4(__nv_bfloat16* dst, float4 v) {
+  __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), c = __floats2bfloat162_rn(v.z, v.w);
+  uint2 u;
+  u.x = *reinterpret_cast<uint32_t*>(&a);
+  u.y = *reinterpret_cast<uint32_t*>(&c);
+  *reinterpret_cast<uint2*>(dst) = u;
+}
 __device__ __forceinline__ void softmax_bar() { asm volatile("bar.sync 1, 512;" ::: "memory"); }
 // order-preserving float <-> int image (signed compare), so a column max is one REDUX + one shared atomicMax
 __device__ __forceinline__ int f2o(float f) {
@@ -172,11 +179,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ uint32_t tmem_ptr_s;
   __shared__ int s_flag[3];
   __shared__ unsigned int s_ticket;
+  __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
+  __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
+  __shared__ __align__(16) float s_lse2[NT];     // base-2 log-sum-exp of this split's partial (cluster combine)
   __shared__ __align__(16) int s_colpos[NT];     // position of the row, -1 = none
   __shared__ __align__(16) float s_mref[NT];     // running reference (log2 units)
   __shared__ __align__(16) int s_colmax[NT];     // ordered-int block max (slow path)
   __shared__ __align__(16) float s_alpha[NT];
-  __shared__ __align__(16) int s_coloff[NT];     // output offset (floats) of the row
   __shared__ __align__(16) float s_L[NT];        // row sums (epilogue)
   const int pps = p.pages_per_split;
   const UmmaLayout lay = umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, pps);
@@ -192,9 +201,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
 
   const int split = blockIdx.x % p.nsplit, rg = blockIdx.x / p.nsplit, h = blockIdx.y, b = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int G = p.h_q / p.h_k, R = p.window + 1, rows = R * G;
-  const int row0 = rg * p.rg_rows;                      // this CTA's query rows: [row0, row0 + rows_cta) of the unit
-  const int rows_cta = min(p.rg_rows, rows - row0);
+  const int G = p.h_q / p.h_k, R = p.window + 1;
+  // Query rows are laid out by window RANK (t - position: 0 = the current query, 1 = the newest past query, ...):
+  // local row = (rank - rk0) * G + q head of the group.  This CTA's row group owns the ranks [rk0, rk0 + nrk).
+  const int rk0 = rg * p.rg_ranks;
+  const int nrk = min(p.rg_ranks, R - rk0);
+  const int rows_cta = nrk * G;
   const size_t unit = (size_t)b * p.h_k + h;
 
   // ---- prologue.  Barriers and TMEM do not depend on the previous kernel: set them up before waiting for it.
@@ -210,6 +222,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
                  "r"(cfg.tmem_cols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
+  if (tid <= kMaxWindow) s_rowr[tid] = -1;
+  __syncthreads();
   pdl_wait();
   pdl_trigger();
   // Global loads that depend on nothing are issued first (count, length, Q, q_pos, the list entries of this
@@ -217,24 +231,29 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   // (in program order after it they were issued only once block_table[j], the one dependent load, had returned).
   const int count = p.sel_count[unit];
   const int L = p.seq_lens[b];
-  constexpr int kQIter = (NT * 16 + kUmmaThreads - 1) / kUmmaThreads;
+  // One row group: the unit's R * G rows (<= NT).  Several row groups (R * G > 128): every CTA fetches all of them
+  // and keeps its own ranks (the rank of a row is only known once q_pos and the length are back).
+  constexpr int kQIter = ((NCH >= 5 ? 3 : 1) * NT * 16 + kUmmaThreads - 1) / kUmmaThreads;
   uint4 q_regs[kQIter];
+  int q_rpos[kQIter];
   {
     const uint4* src = reinterpret_cast<const uint4*>(p.q_win);
+    const int n_chunks = R * G * 16;                           // rows of the window x 16 chunks of 16 B
 #pragma unroll
     for (int it = 0; it < kQIter; ++it) {
-      const int i = tid + it * kUmmaThreads;                   // NT rows x 16 chunks of 16 B
-      const int rho = i >> 4, c = i & 15;
+      const int i = tid + it * kUmmaThreads;
       q_regs[it] = make_uint4(0, 0, 0, 0);
-      if (i < NT * 16 && rho < rows_cta) {
-        const int r = (row0 + rho) / G, g = (row0 + rho) - r * G;
+      q_rpos[it] = -1;
+      if (i < n_chunks) {
+        const int rho = i >> 4, c = i & 15;
+        const int r = rho / G, g = rho - r * G;
         q_regs[it] = __ldg(src + (((size_t)b * R + r) * p.h_q + h * G + g) * 16 + c);
+        q_rpos[it] = __ldg(p.q_pos + b * R + r);
       }
     }
   }
-  static_assert(NT <= kUmmaThreads, "one thread per padded row");
   int my_pos_raw = -1;
-  if (tid < rows_cta) my_pos_raw = __ldg(p.q_pos + b * R + (row0 + tid) / G);
+  if (tid < R) my_pos_raw = __ldg(p.q_pos + b * R + tid);
   for (int i = tid; i < pps; i += kUmmaThreads) {
     const int idx = split * pps + i;
     int j = 0, prev = 0;
@@ -248,27 +267,33 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     s_list[pps + i] = prev;
     s_list[2 * pps + i] = phys;
   }
+  const int t = L - 1;
+  // rows of the padded tile that no window row fills must read as zeros for the tensor core
+  for (int i = tid; i < NT * 16; i += kUmmaThreads)
+    *reinterpret_cast<uint4*>(smem + lay.q + (i & 1) * (NT * 128) + (i >> 1) * 16) = make_uint4(0, 0, 0, 0);
+  if (tid < R) {
+    s_posr[tid] = my_pos_raw;
+    const int rank = t - my_pos_raw;
+    if (my_pos_raw >= 0 && rank >= rk0 && rank < rk0 + nrk) s_rowr[rank - rk0] = tid;
+  }
+  if (tid < 3) s_flag[tid] = 0;
+  __syncthreads();
 #pragma unroll
   for (int it = 0; it < kQIter; ++it) {
     const int i = tid + it * kUmmaThreads;
-    if (i < NT * 16) {
-      const int rho = i >> 4, c = i & 15;
+    const int rank = t - q_rpos[it];
+    if (q_rpos[it] >= 0 && rank >= rk0 && rank < rk0 + nrk) {
+      const int g = (i >> 4) % G, c = i & 15;
+      const int rho = (rank - rk0) * G + g;
       const int half = c >> 3, ch = c & 7;
       *reinterpret_cast<uint4*>(smem + lay.q + half * (NT * 128) + rho * 128 + ((ch ^ (rho & 7)) << 4)) = q_regs[it];
     }
   }
-  const int t = L - 1;
-  if (tid < 3) s_flag[tid] = 0;
   for (int c = tid; c < NT; c += kUmmaThreads) {
-    int pos = -1, off = 0;
-    if (c < rows_cta) {
-      const int r = (row0 + c) / G, g = (row0 + c) - r * G;
-      pos = my_pos_raw;
-      if (pos > t || pos < t - p.window) pos = -1;
-      off = p.nsplit > 1 ? (row0 + c) * 128 : (r * p.h_q + h * G + g) * 128;
-    }
+    int pos = -1;
+    if (c < rows_cta && s_rowr[c / G] >= 0) pos = t - (rk0 + c / G);
     s_colpos[c] = pos;
-    s_coloff[c] = off;
+    s_lse2[c] = -INFINITY;
     s_mref[c] = kMrefInit;
     s_colmax[c] = kOrdNegInf;
     s_alpha[c] = 1.f;
@@ -505,17 +530,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
       tc_fence_after();
       softmax_bar();                                       // s_L complete
-      float* o_base;
-      float* lse_base;
-      if (p.nsplit > 1) {
-        o_base = p.split_o + (unit * p.nsplit + split) * rows * 128;
-        lse_base = p.split_lse + (unit * p.nsplit + split) * rows;
-      } else {
-        o_base = p.part_o + (size_t)b * R * p.h_q * 128;
-        lse_base = p.part_lse + (size_t)b * R * p.h_q;
-      }
-      const float lse_scale = p.nsplit > 1 ? 1.f : kLn2;
-      // thread = channel `key`; its NC rows: O = (O_hi + O_lo) / L, 128 B coalesced per warp and row
+      // thread = channel `key`; its NC rows: O = (O_hi + O_lo) / L into the staging tile [row][128 channels] (the
+      // K / V ring is idle: every tensor-core read of it has retired), base-2 lse next to it
+      float* stage = reinterpret_cast<float*>(smem + lay.ring);
 #pragma unroll
       for (int i = 0; i < NCH; ++i) {
         if (cbeg + 4 * i < rows_cta) {                      // warp-uniform
@@ -528,25 +545,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             const int c = cbeg + 4 * i + u;
             if (c < rows_cta) {
               const float l = s_L[c];
-              const float inv = l > 0.f ? rcp_approx(l) : 0.f;
-              const int off = s_coloff[c];
-              o_base[off + key] = (__uint_as_float(oh[u]) + __uint_as_float(ol[u])) * inv;
-              if (key == 0) lse_base[off >> 7] = l > 0.f ? (s_mref[c] + lg2_approx(l)) * lse_scale : -INFINITY;
+              const float inv = rcp_approx(l);
+              stage[c * 128 + key] = l > 0.f ? (__uint_as_float(oh[u]) + __uint_as_float(ol[u])) * inv : 0.f;
+              if (key == 0) s_lse2[c] = l > 0.f ? s_mref[c] + lg2_approx(l) : -INFINITY;
             }
           }
         }
-      }
-    }
-  } else {
-    // no page for this split: empty partial for every row
-    for (int rho = row0 + tid; rho < row0 + rows_cta; rho += kUmmaThreads) {
-      if (p.nsplit > 1) {
-        p.split_lse[(unit * p.nsplit + split) * rows + rho] = -INFINITY;
-      } else {
-        const int r = rho / G, g = rho % G;
-        float* dst = p.part_o + (((size_t)b * R + r) * p.h_q + h * G + g) * 128;
-        for (int c = 0; c < 128; ++c) dst[c] = 0.f;
-        p.part_lse[((size_t)b * R + r) * p.h_q + h * G + g] = -INFINITY;
       }
     }
   }
@@ -556,11 +560,155 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(cfg.tmem_cols));
   }
-  if (p.nsplit == 1 || p.defer_combine) return;
-  combine_splits_last_cta<128>(p, unit, b, h, rows, G, R, &s_ticket, row0, row0 + rows_cta,
-                               &p.counters[unit * p.nrg + rg]);
+  // ---- split combine (+ S4 when fused) over the cluster: the splits of a (unit, row group) are the CTAs of one
+  // cluster; every CTA merges a share of the rows, reading the other splits' partials out of their shared memory.
+  cluster_arrive();
+  cluster_wait();
+  {
+    const float* stage = reinterpret_cast<const float*>(smem + lay.ring);
+    const uint32_t stage_a = smem_u32(stage) + lane * 16, lse_a = smem_u32(s_lse2);
+    const int nsplit = p.nsplit;
+    const int w = p.window;
+    const int nwarps = kUmmaThreads / 32;
+    // Eq. 8 applied to the splits of local row c (weights 2^(lse_s - max)); returns this lane's 4 channels and the
+    // natural-log lse.  An empty split's tile is unspecified: it is never multiplied.
+    auto combine_row = [&](int c, float4& o, float& lse) {
+      float l_mine = -INFINITY;
+      if (lane < nsplit) l_mine = dsmem_ld_f32(dsmem_addr(lse_a + c * 4, lane));
+      float4 v[8];
+#pragma unroll
+      for (int s2 = 0; s2 < 8; ++s2)
+        if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
+      const float mx = warp_max(l_mine);
+      const float w_mine = mx > -INFINITY ? exp2f(l_mine - mx) : 0.f;
+      float wsum = 0.f;
+      o = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int s2 = 0; s2 < 8; ++s2) {
+        const float wg = __shfl_sync(0xffffffffu, w_mine, s2);
+        if (s2 < nsplit && wg > 0.f) {
+          wsum += wg;
+          o.x = fmaf(wg, v[s2].x, o.x); o.y = fmaf(wg, v[s2].y, o.y);
+          o.z = fmaf(wg, v[s2].z, o.z); o.w = fmaf(wg, v[s2].w, o.w);
+        }
+      }
+      const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
+      o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+      lse = wsum > 0.f ? (mx + log2f(wsum)) * kLn2 : -INFINITY;
+    };
+    auto row_elem = [&](int r, int g) { return ((size_t)b * R + r) * p.h_q + h * G + g; };
+    if (!p.fused) {
+      // stand-alone S3: item = local row; part_o / part_lse of the row's place in q_win
+#pragma unroll 1
+      for (int c = split + nsplit * warp; c < rows_cta; c += nsplit * nwarps) {
+        const int r = s_rowr[c / G];
+        if (r < 0) continue;
+        float4 o; float lse;
+        combine_row(c, o, lse);
+        const size_t e = row_elem(r, c % G);
+        *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
+        if (lane == 0) p.part_lse[e] = lse;
+      }
+    } else {
+      // S3 + S4 (one row group): item = (cache slot x, q head g): the slot's past row (position = x mod w, read
+      // and merged with the cache, Eq. 8-9), then the current row if it lands in this slot (pushed): the pop of
+      // position t - w and the push of position t are ordered by the warp.
+      __nv_bfloat16* out = reinterpret_cast<__nv_bfloat16*>(p.out);
+      const int nslot = w > 0 ? w : 1;
+#pragma unroll 1
+      for (int it = split + nsplit * warp; it < nslot * G; it += nsplit * nwarps) {
+        const int x = it / G, g = it - x * G;
+        const int hq = h * G + g;
+        const size_t ce = ((size_t)b * nslot + x) * p.h_q + hq;
+        if (w > 0) {
+          const int p_past = t - 1 - (((t - 1 - x) % w + w) % w);      // the position in [t-w, t-1] with p mod w == x
+          const int rank = t - p_past;
+          const int r = p_past >= 0 ? s_rowr[rank] : -1;
+          if (r >= 0) {
+            const bool cached = p.cache_pos[b * w + x] == p_past;
+            float lc = -INFINITY;
+            float4 vc = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (cached) {
+              lc = p.cache_lse[ce];
+              vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
+            }
+            float4 o; float lp;
+            combine_row(rank * G + g, o, lp);
+            const size_t e = row_elem(r, g);
+            *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
+            if (lane == 0) p.part_lse[e] = lp;
+            float4 res = o;
+            float lse = lp;
+            if (lc > -INFINITY) {
+              if (lp == -INFINITY) { res = vc; lse = lc; }
+              else {
+                const float m2 = fmaxf(lc, lp);
+                const float wc = __expf(lc - m2), wp = __expf(lp - m2);
+                const float iv = 1.f / (wc + wp);
+                res.x = (wc * vc.x + wp * o.x) * iv; res.y = (wc * vc.y + wp * o.y) * iv;
+                res.z = (wc * vc.z + wp * o.z) * iv; res.w = (wc * vc.w + wp * o.w) * iv;
+                lse = m2 + __logf(wc + wp);
+              }
+            }
+            store_bf16x4(out + e * 128 + lane * 4, res);
+            if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lse;
+            if (p_past != t - w) {                                     // not popped: written back
+              *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = res;
+              if (lane == 0) p.cache_lse[ce] = lse;
+            }
+          }
+        }
+        if (w == 0 || t % w == x) {                                    // the current row: out = O_org, pushed
+          const int r = s_rowr[0];
+          if (r >= 0) {
+            float4 o; float lp;
+            combine_row(g, o, lp);
+            const size_t e = row_elem(r, g);
+            *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
+            if (lane == 0) p.part_lse[e] = lp;
+            store_bf16x4(out + e * 128 + lane * 4, o);
+            if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lp;
+            if (w > 0) {
+              *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = o;
+              if (lane == 0) p.cache_lse[ce] = lp;
+            }
+          }
+        }
+      }
+    }
+    // rows of q_win without a position inside the window: zeros / -inf (one CTA of the unit's first row group)
+    if (split == 0 && rg == 0) {
+#pragma unroll 1
+      for (int it = warp; it < R * G; it += nwarps) {
+        const int r = it / G, g = it - r * G;
+        const int pos = s_posr[r];
+        if (pos >= 0 && pos <= t && pos >= t - w) continue;
+        const size_t e = row_elem(r, g);
+        *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (lane == 0) p.part_lse[e] = -INFINITY;
+        if (p.fused) {
+          store_bf16x4(reinterpret_cast<__nv_bfloat16*>(p.out) + e * 128 + lane * 4, make_float4(0.f, 0.f, 0.f, 0.f));
+          if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = -INFINITY;
+        }
+      }
+    }
+  }
+  cluster_arrive();            // nobody leaves while its partial may still be read
+  cluster_wait();
+  if (p.fused && p.window > 0 && split == 0) {
+    // cache_pos is shared by the KV heads of a sequence: the last unit of the sequence to finish reading rewrites it
+    // (Push: slot t mod w <- t; Update: a merged past row keeps its slot; Pop: position t - w is overwritten)
+    if (tid == 0) s_ticket = ticket_acq_rel(&p.seq_counters[b]);
+    __syncthreads();
+    if (s_ticket == (unsigned)(p.h_k - 1)) {
+      const int w = p.window;
+      if (tid == 0) p.seq_counters[b] = 0;
+      if (tid >= 1 && tid <= w && s_rowr[tid] >= 0 && t - tid != t - w) p.cache_pos[b * w + (t - tid) % w] = t - tid;
+      __syncthreads();
+      if (tid == 0 && s_rowr[0] >= 0) p.cache_pos[b * w + t % w] = t;
+    }
+  }
 }
-
 
 // ---- host: tensor maps over the K / V pools viewed as [(phys * h_k + head) * 16 rows][128 channels] ----
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -598,21 +746,20 @@ template <int NCH>
 static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const UmmaCfg& cfg, size_t smem,
                       const CUtensorMap& mk, const CUtensorMap& mv, cudaStream_t s) {
   auto kern = attend_umma_kernel<NCH>;
-  static size_t smem_allowed = 0;   // per instantiation; raised on demand (not a stream operation)
-  if (smem > smem_allowed) {
-    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    RETRO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                        cudaSharedmemCarveoutMaxShared));
-    smem_allowed = smem;
-  }
-  RETRO_CUDA_TRY(launch_kernel(kern, dim3(prm.nsplit * prm.nrg, d->num_kv_heads, d->batch), dim3(kUmmaThreads), smem, s, prm, cfg, mk,
-                               mv));
+  const int rc = ensure_dynamic_smem((const void*)kern, smem, /*max_carveout=*/true);
+  if (rc != RETRO_OK) return rc;
+  // the splits of a (unit, row group) form one cluster (<= 8 CTAs: portable)
+  RETRO_CUDA_TRY(launch_cluster_kernel(kern, dim3(prm.nsplit * prm.nrg, d->num_kv_heads, d->batch), dim3(kUmmaThreads),
+                                       smem, s, prm.nsplit, prm, cfg, mk, mv));
   RETRO_LAUNCH_CHECK();
   return RETRO_OK;
 }
 
 int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStream_t s) {
-  // the encode is pure host work (~1 us); cache the maps per (pool pair, shape)
+  // the encode is pure host work (~1 us); cache the maps per (pool pair, shape).  The cache holds tensor-map
+  // DESCRIPTORS of the caller's pools (addresses, never dereferenced on the host): see retro.h "global state".
+  CUtensorMap map_k, map_v;
+  {
   std::lock_guard<std::mutex> lock(host_mutex());
   struct Cached { const void* k; const void* v; int phys, hk; CUtensorMap mk, mv; };
   constexpr int kCache = 64;
@@ -634,10 +781,14 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
     cache[slot] = c;
     hit = &cache[slot];
   }
-  const int nch = ceil_div(prm.rg_rows, 16), NT = 16 * nch;
+  map_k = hit->mk;
+  map_v = hit->mv;
+  }
+  const int nch = ceil_div(prm.rg_ranks * (d->num_q_heads / d->num_kv_heads), 16), NT = 16 * nch;
+  if (prm.nsplit > 8) return RETRO_ERR_UNSUPPORTED;
   if (NT > kMaxNT) return RETRO_ERR_UNSUPPORTED;
-  // Shared-memory plan.  233472 B per SM, 1 KB reserved per resident CTA, ~2-3 KB static; two CTAs per SM up to
-  // Prefer two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in flight per CTA).
+  // Shared-memory plan (one CTA per SM: 232448 B less the reserved KB and ~5 KB of static shared memory).  Prefer
+  // two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in flight per CTA).
   UmmaCfg cfg;
   cfg.NSB = 2;
   int slots = 0;
@@ -660,14 +811,14 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   cfg.tmem_cols = cols;
   const size_t smem = (size_t)umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, prm.pages_per_split).total;
   switch (nch) {
-    case 1: return launch_nch<1>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 2: return launch_nch<2>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 3: return launch_nch<3>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 4: return launch_nch<4>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 5: return launch_nch<5>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 6: return launch_nch<6>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 7: return launch_nch<7>(d, prm, cfg, smem, hit->mk, hit->mv, s);
-    case 8: return launch_nch<8>(d, prm, cfg, smem, hit->mk, hit->mv, s);
+    case 1: return launch_nch<1>(d, prm, cfg, smem, map_k, map_v, s);
+    case 2: return launch_nch<2>(d, prm, cfg, smem, map_k, map_v, s);
+    case 3: return launch_nch<3>(d, prm, cfg, smem, map_k, map_v, s);
+    case 4: return launch_nch<4>(d, prm, cfg, smem, map_k, map_v, s);
+    case 5: return launch_nch<5>(d, prm, cfg, smem, map_k, map_v, s);
+    case 6: return launch_nch<6>(d, prm, cfg, smem, map_k, map_v, s);
+    case 7: return launch_nch<7>(d, prm, cfg, smem, map_k, map_v, s);
+    case 8: return launch_nch<8>(d, prm, cfg, smem, map_k, map_v, s);
   }
   return RETRO_ERR_UNSUPPORTED;
 }

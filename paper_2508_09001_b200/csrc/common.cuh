@@ -42,7 +42,7 @@ struct DeviceInfo {
 };
 DeviceInfo device_info();
 // cudaFuncAttributeMaxDynamicSharedMemorySize is per device: remembers per (device, kernel) what was granted.
-int ensure_dynamic_smem(const void* kern, size_t smem_bytes);   // RETRO_OK / RETRO_ERR_CUDA
+int ensure_dynamic_smem(const void* kern, size_t smem_bytes, bool max_carveout = false);   // RETRO_OK / RETRO_ERR_CUDA
 // Can `min_clusters` clusters of cluster_x CTAs of this kernel be resident at once on the current device?  Sizes above
 // 8 opt the kernel in to non-portable cluster sizes.  Cached per (device, kernel, shared memory, cluster size).
 bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cluster_x, int min_clusters);
@@ -64,9 +64,15 @@ struct WorkspaceLayout {
   int nsplit;           // split-KV factor of the attend kernel
   int pages_per_split;
   int rows;             // G * (w+1)
-  int nrg, rg_rows;     // query-row groups of the tensor-core attend path (one group unless rows > 128)
+  int nrg, rg_ranks;    // query-row groups of the tensor-core attend path (one group unless rows > 128): window
+                        // ranks per group
 };
 WorkspaceLayout workspace_layout(const retro_desc_t* d);
+
+// S4 operands for the attend kernel that also merges the output cache (retro_decode_step)
+struct FusedMerge {
+  float* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse;
+};
 
 // ---- kernel launchers (one per stage; defined in the matching .cu) ------------------------------
 int launch_update_page_bounds(const retro_desc_t* d, const void* k_pages, const int32_t* block_table,
@@ -81,11 +87,8 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
                          const void* k_pages, const void* v_pages, const int32_t* block_table,
                          const int32_t* seq_lens, const int32_t* sel_pages, const int32_t* sel_prev,
                          const int32_t* sel_count, float* part_o, float* part_lse, void* workspace, cudaStream_t s,
-                         bool* defer_combine = nullptr);   // in: allowed; out: the split partials were left uncombined
-int launch_combine_merge(const retro_desc_t* d, const float* split_o, const float* split_lse, int nsplit, int rows,
-                         float* part_o, float* part_lse, const int32_t* q_pos, const int32_t* seq_lens, float* cache_o,
-                         float* cache_lse, int32_t* cache_pos, void* out, float* out_lse, unsigned int* slot_counters,
-                         cudaStream_t s);
+                         const FusedMerge* fused = nullptr);   // non-null (tensor-core path, one row group): S4 in the same kernel
+bool attend_can_fuse_merge(const retro_desc_t* d, const WorkspaceLayout& wl);
 int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
                               const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);

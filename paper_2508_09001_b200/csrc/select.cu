@@ -303,11 +303,21 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t rank = cluster_ctarank();
   uint32_t* keys = reinterpret_cast<uint32_t*>(smem_raw + kRingBytes);
+  int32_t* s_A = reinterpret_cast<int32_t*>(smem_raw + kRingBytes + (((size_t)p.max_pages * 4 + 15) & ~(size_t)15));
   if (tid == 0) { s_kmin = 0xffffffffu; s_kmax = 0u; s_epsbits = 0u; sh.below = 0u; }
   for (int i = tid; i < kBuckets; i += NT) sh.hist[i] = 0;
   cluster_arrive();            // (#0) the leader's accumulators are initialised before anybody adds to them
   pdl_wait();
   pdl_trigger();
+  // Alg. 2 reads A[p] of the selected pages: the leader prefetches the unit's row of A (it does not depend on
+  // anything this kernel computes), so the selection tail has no global round trip left
+  if (p.last_loaded != nullptr && rank == 0) {
+    const int32_t* a_src = p.last_loaded + ((size_t)blockIdx.z * p.h_k + blockIdx.y) * p.max_pages;
+#pragma unroll 1
+    for (int i = tid; i < p.max_pages; i += NT)
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(s_A + i)), "l"(a_src + i) : "memory");
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
   const T* q_cur = reinterpret_cast<const T*>(p.q_cur);
   const T* bounds = reinterpret_cast<const T*>(p.bounds);
   const int b = blockIdx.z, h = blockIdx.y;
@@ -570,7 +580,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
   for (int i = tid; i < count; i += NT) {
     const int j = sel_s[i];
     int prev = -1;
-    if (A != nullptr) { prev = A[j]; A[j] = t; }
+    if (A != nullptr) { prev = s_A[j]; A[j] = t; }
     out_pages[i] = j;
     out_prev[i] = prev;
   }
@@ -613,7 +623,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   prm.pages_per_cta = 0;
   prm.k_pages = k_pages_refresh; prm.block_table = block_table; prm.bounds_out = const_cast<void*>(bounds);
   const DeviceInfo di = device_info();
-  const size_t smem = (size_t)kRingBytes + (size_t)d->max_pages_per_seq * sizeof(uint32_t);
+  const size_t smem = (size_t)kRingBytes + 2 * ((((size_t)d->max_pages_per_seq * 4) + 15) & ~(size_t)15);
   const size_t smem_static = 32 * 1024;   // s_q (<= 16 KB for GROUP_MAX) + TopkShared (~11 KB): upper bound
   int ctas_per_sm = (int)((size_t)di.max_smem_optin / (smem + smem_static));
   ctas_per_sm = ctas_per_sm > 2 ? 2 : (ctas_per_sm < 1 ? 1 : ctas_per_sm);
