@@ -55,23 +55,26 @@ int ensure_dynamic_smem(const void* kern, size_t smem_bytes, bool max_carveout) 
   return RETRO_OK;
 }
 
-bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cluster_x, int min_clusters) {
+int max_active_clusters(const void* kern, int block_threads, size_t smem_bytes, int cluster_x) {
   struct Entry { int dev; const void* kern; size_t smem; int cluster; int max_active; };
-  constexpr int kEntries = 256;
+  constexpr int kEntries = 512;
   static Entry tab[kEntries];
   static int n_used = 0;
   int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return false; }
-  std::lock_guard<std::mutex> lock(host_mutex());
-  for (int i = 0; i < n_used; ++i)
-    if (tab[i].dev == dev && tab[i].kern == kern && tab[i].smem == smem_bytes && tab[i].cluster == cluster_x)
-      return tab[i].max_active >= min_clusters;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+  {
+    std::lock_guard<std::mutex> lock(host_mutex());
+    for (int i = 0; i < n_used; ++i)
+      if (tab[i].dev == dev && tab[i].kern == kern && tab[i].smem == smem_bytes && tab[i].cluster == cluster_x)
+        return tab[i].max_active;
+  }
   int max_active = 0;
-  bool ok = true;
-  if (cluster_x > 8) ok = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+  bool ok = ensure_dynamic_smem(kern, smem_bytes) == RETRO_OK;   // (only ever raises the kernel's limit)
+  if (ok && cluster_x > 8)
+    ok = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
   if (ok) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(cluster_x * (min_clusters > 0 ? min_clusters : 1), 1, 1);
+    cfg.gridDim = dim3(cluster_x, 1, 1);
     cfg.blockDim = dim3(block_threads);
     cfg.dynamicSmemBytes = smem_bytes;
     cudaLaunchAttribute attr[1];
@@ -84,8 +87,9 @@ bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cl
     ok = cudaOccupancyMaxActiveClusters(&max_active, kern, &cfg) == cudaSuccess;
   }
   if (!ok) { (void)cudaGetLastError(); max_active = 0; }
+  std::lock_guard<std::mutex> lock(host_mutex());
   if (n_used < kEntries) tab[n_used++] = Entry{dev, kern, smem_bytes, cluster_x, max_active};
-  return max_active >= min_clusters;
+  return max_active;
 }
 
 int validate_desc(const retro_desc_t* d) {
@@ -123,7 +127,13 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   wl.rg_ranks = ceil_div(R, wl.nrg);
   while (umma && wl.rg_ranks * G > 128) { ++wl.nrg; wl.rg_ranks = ceil_div(R, wl.nrg); }
   int nsplit = umma ? sm_count / (units * wl.nrg) : ceil_div(2 * sm_count, units);
-  if (umma && nsplit > 8) nsplit = 8;
+  if (umma) {
+    // the largest split count whose clusters (one per unit and row group) are all resident at once: the device
+    // keeps fewer CTAs resident in large clusters (B200, one CTA per SM: 74 x 2, 33 x 4, 22 x 6, 15 x 8)
+    if (nsplit > 8) nsplit = 8;
+    const int nch = ceil_div(wl.rg_ranks * G, 16);
+    while (nsplit > 1 && umma_max_active_clusters(nch, nsplit) < units * wl.nrg) --nsplit;
+  }
   const int min_pages = umma ? 8 : 2;
   const int max_split = d->max_sel_pages >= min_pages ? d->max_sel_pages / min_pages : 1;
   if (nsplit > max_split) nsplit = max_split;

@@ -42,6 +42,7 @@ constexpr int kTileHalfBytes = 16 * 128;      // one (page, head, 64-channel hal
 constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][128 B]
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
 constexpr int kTmemCols = 512;
+constexpr int kUmmaSmemBudget = 232448 - 1024 - 4096;   // dynamic shared memory the launcher plans with (one CTA per SM)
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
 constexpr float kRescaleThreshold = 64.f;     // log2 units: P <= 2^64, sums stay far below the fp32 / bf16 range
 constexpr float kMrefInit = -1.0e30f;         // finite "row not started" reference: -inf - kMrefInit stays -inf
@@ -755,6 +756,28 @@ static int launch_nch(const retro_desc_t* d, const AttendParams& prm, const Umma
   return RETRO_OK;
 }
 
+// Resident clusters of `cluster_x` CTAs of attend_umma_kernel<nch> at the largest shared-memory footprint the
+// launcher plans with.  Without a device (symbol / header tests on a CPU-only box): the B200's measured table.
+int umma_max_active_clusters(int nch, int cluster_x) {
+  const void* kern = nullptr;
+  switch (nch) {
+    case 1: kern = (const void*)attend_umma_kernel<1>; break;
+    case 2: kern = (const void*)attend_umma_kernel<2>; break;
+    case 3: kern = (const void*)attend_umma_kernel<3>; break;
+    case 4: kern = (const void*)attend_umma_kernel<4>; break;
+    case 5: kern = (const void*)attend_umma_kernel<5>; break;
+    case 6: kern = (const void*)attend_umma_kernel<6>; break;
+    case 7: kern = (const void*)attend_umma_kernel<7>; break;
+    case 8: kern = (const void*)attend_umma_kernel<8>; break;
+    default: return 0;
+  }
+  if (device_info().device < 0) {
+    static const int b200[9] = {0, 148, 74, 45, 33, 26, 22, 15, 15};
+    return cluster_x >= 1 && cluster_x <= 8 ? b200[cluster_x] : 0;
+  }
+  return max_active_clusters(kern, kUmmaThreads, (size_t)kUmmaSmemBudget, cluster_x);
+}
+
 int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStream_t s) {
   // the encode is pure host work (~1 us); cache the maps per (pool pair, shape).  The cache holds tensor-map
   // DESCRIPTORS of the caller's pools (addresses, never dereferenced on the host): see retro.h "global state".
@@ -800,7 +823,7 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
       slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
     }
   };
-  plan(232448 - 1024 - 4096);
+  plan(kUmmaSmemBudget);
   if (slots < 2) return RETRO_ERR_UNSUPPORTED;
   if (slots > 6) slots = 6;
   cfg.NK = slots / 2;             // a V block lives longer (it waits for the softmax of its own block)

@@ -43,9 +43,12 @@ struct DeviceInfo {
 DeviceInfo device_info();
 // cudaFuncAttributeMaxDynamicSharedMemorySize is per device: remembers per (device, kernel) what was granted.
 int ensure_dynamic_smem(const void* kern, size_t smem_bytes, bool max_carveout = false);   // RETRO_OK / RETRO_ERR_CUDA
-// Can `min_clusters` clusters of cluster_x CTAs of this kernel be resident at once on the current device?  Sizes above
-// 8 opt the kernel in to non-portable cluster sizes.  Cached per (device, kernel, shared memory, cluster size).
-bool cluster_fits(const void* kern, int block_threads, size_t smem_bytes, int cluster_x, int min_clusters);
+// How many clusters of cluster_x CTAs of this kernel (with this much dynamic shared memory) can be resident at once
+// on the current device (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Sizes above 8 opt the kernel in to
+// non-portable cluster sizes.  Cached per (device, kernel, shared memory, cluster size).
+int max_active_clusters(const void* kern, int block_threads, size_t smem_bytes, int cluster_x);
+// tensor-core attend kernel with NT = 16 * nch padded rows: resident clusters of `cluster_x` splits (attend_umma.cu)
+int umma_max_active_clusters(int nch, int cluster_x);
 
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 inline int ceil_div(int a, int b) { return (a + b - 1) / b; }

@@ -285,6 +285,7 @@ struct SelectParams {
   unsigned long long* amb_keys;  // workspace [units][max_pages]: fp64 keys of the undecided pages (exact refinement)
   int32_t* amb_idx;              // workspace [units][max_pages]
   int h_q, h_k, max_pages, k_max, P, force_last, pages_per_cta;
+  int prefetch_a;                // the leader stages the unit's row of A in shared memory
   // S1 in line (retro_decode_step): the warp that owns the newest page recomputes its digest from the K tile,
   // patches the staged record and writes it back to `bounds`.  k_pages == NULL: digests are up to date.
   const void* k_pages; const int32_t* block_table; void* bounds_out;
@@ -311,7 +312,7 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
   pdl_trigger();
   // Alg. 2 reads A[p] of the selected pages: the leader prefetches the unit's row of A (it does not depend on
   // anything this kernel computes), so the selection tail has no global round trip left
-  if (p.last_loaded != nullptr && rank == 0) {
+  if (p.last_loaded != nullptr && p.prefetch_a && rank == 0) {
     const int32_t* a_src = p.last_loaded + ((size_t)blockIdx.z * p.h_k + blockIdx.y) * p.max_pages;
 #pragma unroll 1
     for (int i = tid; i < p.max_pages; i += NT)
@@ -580,31 +581,12 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
   for (int i = tid; i < count; i += NT) {
     const int j = sel_s[i];
     int prev = -1;
-    if (A != nullptr) { prev = s_A[j]; A[j] = t; }
+    if (A != nullptr) { prev = p.prefetch_a ? s_A[j] : A[j]; A[j] = t; }
     out_pages[i] = j;
     out_prev[i] = prev;
   }
   for (int i = count + tid; i < p.k_max; i += NT) { out_pages[i] = -1; out_prev[i] = -1; }
   if (tid == 0) p.sel_count[unit] = count;
-}
-
-// How many CTAs (= cluster size) stream one unit.  Cost of a plan = pages the busiest SM streams; within 2 % the
-// plan with more CTAs wins (more bytes in flight).  Cluster sizes 1..8 are portable; 16 needs an opt-in and is used
-// when the device can keep one such cluster per unit resident.
-static int plan_chunks(const retro_desc_t* d, int sm_count, int ctas_per_sm, bool allow16) {
-  const int units = d->batch * d->num_kv_heads;
-  const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerWarp);
-  int best = 1;
-  double best_cost = 1e30;
-  for (int n = 1; n <= kMaxSelCluster; ++n) {
-    if (n > 8 && !(n == 16 && allow16)) continue;
-    if (n > max_chunks) break;
-    const int per_sm = ceil_div(units * n, sm_count);
-    if (per_sm > ctas_per_sm && n > 1) continue;
-    const double cost = (double)per_sm * (ceil_div(ceil_div(d->max_pages_per_seq, n), kPagesPerWarp) * kPagesPerWarp);
-    if (cost <= best_cost * 1.02) { best = n; best_cost = cost < best_cost ? cost : best_cost; }
-  }
-  return best;
 }
 
 int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const void* q_cur, const void* bounds,
@@ -621,22 +603,37 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   prm.h_q = d->num_q_heads; prm.h_k = d->num_kv_heads; prm.max_pages = d->max_pages_per_seq;
   prm.k_max = d->max_sel_pages; prm.P = d->page_size; prm.force_last = d->force_last_page;
   prm.pages_per_cta = 0;
+  prm.prefetch_a = 0;
   prm.k_pages = k_pages_refresh; prm.block_table = block_table; prm.bounds_out = const_cast<void*>(bounds);
   const DeviceInfo di = device_info();
-  const size_t smem = (size_t)kRingBytes + 2 * ((((size_t)d->max_pages_per_seq * 4) + 15) & ~(size_t)15);
-  const size_t smem_static = 32 * 1024;   // s_q (<= 16 KB for GROUP_MAX) + TopkShared (~11 KB): upper bound
-  int ctas_per_sm = (int)((size_t)di.max_smem_optin / (smem + smem_static));
-  ctas_per_sm = ctas_per_sm > 2 ? 2 : (ctas_per_sm < 1 ? 1 : ctas_per_sm);
   const int units = d->batch * d->num_kv_heads;
+  const size_t keys_bytes = ((size_t)d->max_pages_per_seq * 4 + 15) & ~(size_t)15;
   auto launch = [&](auto kern) -> int {
+    // How many CTAs (= cluster size) stream one unit, and whether the leader prefetches the unit's row of A.  A
+    // plan's cost = pages the busiest SM streams + a fixed latency (worth ~350 pages) per wave of resident clusters
+    // (cudaOccupancyMaxActiveClusters knows how many clusters of that size and shared-memory footprint the device
+    // keeps resident: e.g. 15 of size 8 at one CTA per SM on a B200); within 2 % the plan with more CTAs wins (more
+    // bytes in flight), then the one that prefetches.
+    int best_n = 1, best_pref = 0;
+    double best_cost = 1e30;
+    const int max_chunks = ceil_div(d->max_pages_per_seq, kPagesPerWarp);
+    for (int pref = 0; pref <= (last_loaded != nullptr ? 1 : 0); ++pref)
+      for (int n = 1; n <= kMaxSelCluster; ++n) {
+        if ((n > 8 && n != 16) || n > max_chunks) continue;
+        const size_t smem = (size_t)kRingBytes + keys_bytes * (1 + pref);
+        const int cap = max_active_clusters((const void*)kern, kSelThreads, smem, n);
+        if (cap <= 0) continue;
+        const int ppc = ceil_div(ceil_div(d->max_pages_per_seq, n), kPagesPerWarp) * kPagesPerWarp;
+        const double cost = (double)ceil_div(units * n, di.sm_count) * ppc + 350.0 * ceil_div(units, cap);
+        if (cost <= best_cost * 1.02) { best_n = n; best_pref = pref; best_cost = cost < best_cost ? cost : best_cost; }
+      }
+    const size_t smem = (size_t)kRingBytes + keys_bytes * (1 + best_pref);
     const int rc = ensure_dynamic_smem((const void*)kern, smem);
     if (rc != RETRO_OK) return rc;
-    const bool allow16 = units * 16 <= di.sm_count * ctas_per_sm &&
-                         cluster_fits((const void*)kern, kSelThreads, smem, 16, units);
-    const int nchunk = plan_chunks(d, di.sm_count, ctas_per_sm, allow16);
-    prm.pages_per_cta = ceil_div(ceil_div(d->max_pages_per_seq, nchunk), kPagesPerWarp) * kPagesPerWarp;
-    RETRO_CUDA_TRY(launch_cluster_kernel(kern, dim3(nchunk, d->num_kv_heads, d->batch), dim3(kSelThreads), smem, s,
-                                         nchunk, prm));
+    prm.prefetch_a = best_pref;
+    prm.pages_per_cta = ceil_div(ceil_div(d->max_pages_per_seq, best_n), kPagesPerWarp) * kPagesPerWarp;
+    RETRO_CUDA_TRY(launch_cluster_kernel(kern, dim3(best_n, d->num_kv_heads, d->batch), dim3(kSelThreads), smem, s,
+                                         best_n, prm));
     return RETRO_OK;
   };
   const bool gmax = d->group_reduce == RETRO_GROUP_MAX;
