@@ -143,8 +143,10 @@ __device__ __forceinline__ float o2f(int i) { return __int_as_float(i >= 0 ? i :
 constexpr int kOrdNegInf = (int)0x807fffff;   // f2o(-inf)
 
 // Dynamic shared memory map (1024 B aligned).  NT = padded rows, NS = ring slots, NP = P buffers.
+constexpr int kPreItems = 16;                 // output-cache operands a CTA prefetches for its merge items
+constexpr int kPreStride = 132;               // floats per prefetched item: o[128], lse, padding (16 B multiple)
 struct UmmaLayout {
-  int q, p, ring, list, total;
+  int q, p, ring, list, pre, total;
   int p_buf_bytes, p_hl_bytes;
 };
 __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
@@ -156,7 +158,8 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
   L.p_buf_bytes = natom * 16384;
   L.ring = L.p + NP * L.p_buf_bytes;
   L.list = L.ring + NS * kSlotBytes;         // int32 [3][pages_per_split]
-  L.total = L.list + 3 * pages_per_split * 4;
+  L.pre = (L.list + 3 * pages_per_split * 4 + 15) & ~15;   // prefetched cache operands [kPreItems][128 o + lse + pad]
+  L.total = L.pre + kPreItems * kPreStride * 4;
   return L;
 }
 
@@ -182,6 +185,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ unsigned int s_ticket;
   __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
   __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
+  __shared__ int s_cpos[kMaxWindow + 1];         // cache_pos of the sequence as this kernel found it
   __shared__ __align__(16) float s_lse2[NT];     // base-2 log-sum-exp of this split's partial (cluster combine)
   __shared__ __align__(16) int s_colpos[NT];     // position of the row, -1 = none
   __shared__ __align__(16) float s_mref[NT];     // running reference (log2 units)
@@ -310,6 +314,42 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_ptr_s;
+
+  if (warp == 3 && p.fused && p.window > 0) {
+    // ---- the idle warp serves S4 while the others attend: (a) the cache operands of this CTA's merge items are
+    // prefetched into shared memory, (b) cache_pos is snapshotted, (c) the CTA reports that it has read cache_pos;
+    // the LAST CTA of the sequence to report rewrites it (the new values depend on q_pos and t only: Push slot
+    // t mod w <- t, Update keeps the slot of a merged past row, Pop: position t - w is overwritten by the push).
+    const int w = p.window;
+    float* pre = reinterpret_cast<float*>(smem + lay.pre);
+#pragma unroll 1
+    for (int k = 0; k < kPreItems; ++k) {
+      const int it = split + p.nsplit * k;
+      if (it >= w * G) break;
+      const int x = it / G, g = it - x * G;
+      const size_t ce = ((size_t)b * w + x) * p.h_q + h * G + g;
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pre + k * kPreStride + lane * 4)),
+                   "l"(p.cache_o + ce * 128 + lane * 4) : "memory");
+      if (lane == 0)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(pre + k * kPreStride + 128)),
+                     "l"(p.cache_lse + ce) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    if (lane < w) s_cpos[lane] = p.cache_pos[b * w + lane];
+    __syncwarp();
+    unsigned int tk = 0;
+    if (lane == 0) tk = ticket_acq_rel(&p.seq_counters[b]);
+    tk = __shfl_sync(0xffffffffu, tk, 0);
+    if (tk == (unsigned)(p.h_k * p.nsplit - 1)) {
+      if (lane == 0) p.seq_counters[b] = 0;              // leave the workspace consistent for the next call
+      for (int r = lane; r < R; r += 32) {
+        const int pos = s_posr[r];
+        if (pos == t) p.cache_pos[b * w + t % w] = t;
+        else if (pos > t - w && pos < t && pos >= 0) p.cache_pos[b * w + pos % w] = pos;
+      }
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+  }
 
   if (nblk > 0) {
     if (warp < 2) {
@@ -617,7 +657,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       __nv_bfloat16* out = reinterpret_cast<__nv_bfloat16*>(p.out);
       const int nslot = w > 0 ? w : 1;
 #pragma unroll 1
-      for (int it = split + nsplit * warp; it < nslot * G; it += nsplit * nwarps) {
+      const float* pre = reinterpret_cast<const float*>(smem + lay.pre);
+      for (int k = warp; split + nsplit * k < nslot * G; k += nwarps) {
+        const int it = split + nsplit * k;
         const int x = it / G, g = it - x * G;
         const int hq = h * G + g;
         const size_t ce = ((size_t)b * nslot + x) * p.h_q + hq;
@@ -626,12 +668,17 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           const int rank = t - p_past;
           const int r = p_past >= 0 ? s_rowr[rank] : -1;
           if (r >= 0) {
-            const bool cached = p.cache_pos[b * w + x] == p_past;
+            const bool cached = s_cpos[x] == p_past;
             float lc = -INFINITY;
             float4 vc = make_float4(0.f, 0.f, 0.f, 0.f);
             if (cached) {
-              lc = p.cache_lse[ce];
-              vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
+              if (k < kPreItems) {
+                lc = pre[k * kPreStride + 128];
+                vc = *reinterpret_cast<const float4*>(pre + k * kPreStride + lane * 4);
+              } else {
+                lc = p.cache_lse[ce];
+                vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
+              }
             }
             float4 o; float lp;
             combine_row(rank * G + g, o, lp);
@@ -694,21 +741,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       }
     }
   }
-  cluster_arrive();            // nobody leaves while its partial may still be read
-  cluster_wait();
-  if (p.fused && p.window > 0 && split == 0) {
-    // cache_pos is shared by the KV heads of a sequence: the last unit of the sequence to finish reading rewrites it
-    // (Push: slot t mod w <- t; Update: a merged past row keeps its slot; Pop: position t - w is overwritten)
-    if (tid == 0) s_ticket = ticket_acq_rel(&p.seq_counters[b]);
-    __syncthreads();
-    if (s_ticket == (unsigned)(p.h_k - 1)) {
-      const int w = p.window;
-      if (tid == 0) p.seq_counters[b] = 0;
-      if (tid >= 1 && tid <= w && s_rowr[tid] >= 0 && t - tid != t - w) p.cache_pos[b * w + (t - tid) % w] = t - tid;
-      __syncthreads();
-      if (tid == 0 && s_rowr[0] >= 0) p.cache_pos[b * w + t % w] = t;
-    }
-  }
+  cluster_arrive_relaxed();    // nobody leaves while its partial may still be read (no data is handed over: no fence)
+  cluster_wait_end();
 }
 
 // ---- host: tensor maps over the K / V pools viewed as [(phys * h_k + head) * 16 rows][128 channels] ----

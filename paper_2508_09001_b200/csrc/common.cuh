@@ -169,6 +169,10 @@ __device__ __forceinline__ uint32_t cluster_nctarank() {
 // every CTA of the cluster after its wait.  Executed by ALL threads of every CTA of the cluster.
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// the same barrier without memory ordering: "every CTA has got this far" (e.g. before a CTA whose shared memory the
+// others read may exit)
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait_end() { asm volatile("barrier.cluster.wait.aligned;" ::: "memory"); }
 // address of `local_smem_addr` (shared::cta window) in CTA `rank`'s shared memory (shared::cluster window)
 __device__ __forceinline__ uint32_t dsmem_addr(uint32_t local_smem_addr, uint32_t rank) {
   uint32_t r;

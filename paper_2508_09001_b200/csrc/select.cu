@@ -364,18 +364,6 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
   };
 #pragma unroll
   for (int it = 0; it < kSelStages - 1; ++it) issue_batch(it);
-  // S1 in line: the warp that will reduce the newest page (j_last) rebuilds its digest while the first batches fly
-  const int j_last = n_pages - 1;
-  const bool own_last = p.k_pages != nullptr && j_last >= cta_page0 && j_last < page_end &&
-                        ((j_last - cta_page0) / kPagesPerWarp) % kScoreWarps == warp;   // warp-uniform
-  uint4 fresh = make_uint4(0, 0, 0, 0);
-  if (own_last) {
-    const int phys = p.block_table[(size_t)b * p.max_pages + j_last];
-    const uint4* tile = reinterpret_cast<const uint4*>(reinterpret_cast<const T*>(p.k_pages) +
-                                                       ((size_t)phys * p.h_k + h) * p.P * D);
-    fresh = warp_page_digest<T, 16>(tile, min(seq_len_b - j_last * p.P, p.P), lane);
-    reinterpret_cast<uint4*>(reinterpret_cast<T*>(p.bounds_out) + (row + j_last) * 2 * D)[lane] = fresh;
-  }
   // q+ / q- in fp64 (exact), summed over the group for GROUP_SUM
   static_assert(NT == 2 * D || NT == 4 * D, "one thread per element of [q+ ; q-]");
   if (tid < 2 * D) {
@@ -392,6 +380,19 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
     if (!kGroupMax) s_q[0][tid] = acc;
   }
   __syncthreads();
+  // S1 in line: the warp that will reduce the newest page (j_last) rebuilds its digest while its batches fly (after
+  // the barrier above: its two dependent round trips must not hold up the other warps of the CTA)
+  const int j_last = n_pages - 1;
+  const bool own_last = p.k_pages != nullptr && j_last >= cta_page0 && j_last < page_end &&
+                        ((j_last - cta_page0) / kPagesPerWarp) % kScoreWarps == warp;   // warp-uniform
+  uint4 fresh = make_uint4(0, 0, 0, 0);
+  if (own_last) {
+    const int phys = p.block_table[(size_t)b * p.max_pages + j_last];
+    const uint4* tile = reinterpret_cast<const uint4*>(reinterpret_cast<const T*>(p.k_pages) +
+                                                       ((size_t)phys * p.h_k + h) * p.P * D);
+    fresh = warp_page_digest<T, 16>(tile, min(seq_len_b - j_last * p.P, p.P), lane);
+    reinterpret_cast<uint4*>(reinterpret_cast<T*>(p.bounds_out) + (row + j_last) * 2 * D)[lane] = fresh;
+  }
   cluster_wait();              // (#0)
   const uint32_t keys_leader = dsmem_addr(smem_u32(keys), 0);
   float qreg[kVals], qabs[kVals];   // fp32 image of [sum q+ ; sum q-] (one rounding, inside eps) and its magnitude
