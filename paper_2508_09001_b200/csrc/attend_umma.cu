@@ -603,124 +603,99 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   // ---- split combine (+ S4 when fused) over the cluster: the splits of a (unit, row group) are the CTAs of one
   // cluster; every CTA merges a share of the rows, reading the other splits' partials out of their shared memory.
+  // This tail runs every instruction once (latency-bound): ONE loop, one combine site, no unrolling.
   cluster_arrive();
   cluster_wait();
   {
-    const float* stage = reinterpret_cast<const float*>(smem + lay.ring);
-    const uint32_t stage_a = smem_u32(stage) + lane * 16, lse_a = smem_u32(s_lse2);
-    const int nsplit = p.nsplit;
-    const int w = p.window;
-    const int nwarps = kUmmaThreads / 32;
-    // Eq. 8 applied to the splits of local row c (weights 2^(lse_s - max)); returns this lane's 4 channels and the
-    // natural-log lse.  An empty split's tile is unspecified: it is never multiplied.
-    auto combine_row = [&](int c, float4& o, float& lse) {
-      float l_mine = -INFINITY;
-      if (lane < nsplit) l_mine = dsmem_ld_f32(dsmem_addr(lse_a + c * 4, lane));
-      float4 v[8];
-#pragma unroll
-      for (int s2 = 0; s2 < 8; ++s2)
-        if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
-      const float mx = warp_max(l_mine);
-      const float w_mine = mx > -INFINITY ? exp2f(l_mine - mx) : 0.f;
-      float wsum = 0.f;
-      o = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-      for (int s2 = 0; s2 < 8; ++s2) {
-        const float wg = __shfl_sync(0xffffffffu, w_mine, s2);
-        if (s2 < nsplit && wg > 0.f) {
-          wsum += wg;
-          o.x = fmaf(wg, v[s2].x, o.x); o.y = fmaf(wg, v[s2].y, o.y);
-          o.z = fmaf(wg, v[s2].z, o.z); o.w = fmaf(wg, v[s2].w, o.w);
-        }
-      }
-      const float inv = wsum > 0.f ? 1.f / wsum : 0.f;
-      o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
-      lse = wsum > 0.f ? (mx + log2f(wsum)) * kLn2 : -INFINITY;
-    };
-    auto row_elem = [&](int r, int g) { return ((size_t)b * R + r) * p.h_q + h * G + g; };
-    if (!p.fused) {
-      // stand-alone S3: item = local row; part_o / part_lse of the row's place in q_win
+    const uint32_t stage_a = smem_u32(smem + lay.ring) + lane * 16, lse_a = smem_u32(s_lse2);
+    const float* pre = reinterpret_cast<const float*>(smem + lay.pre);
+    const int nsplit = p.nsplit, w = p.window, nwarps = kUmmaThreads / 32;
+    const bool fused = p.fused != 0;
+    // Work items.  Stand-alone S3: item = local row.  Fused S3 + S4: item = (cache slot x, q head g) with two
+    // sub-steps, the slot's past row (position = x mod w; merged with the cache, Eq. 8-9) and then the current row if
+    // it lands in this slot (pushed): the pop of position t - w and the push of position t are ordered by the warp.
+    const int nslot = w > 0 ? w : 1;
+    const int n_items = fused ? nslot * G : rows_cta;
 #pragma unroll 1
-      for (int c = split + nsplit * warp; c < rows_cta; c += nsplit * nwarps) {
-        const int r = s_rowr[c / G];
+    for (int k = warp; split + nsplit * k < n_items; k += nwarps) {
+      const int it = split + nsplit * k;
+      const int x = it / G, g = it - x * G;
+#pragma unroll 1
+      for (int sub = 0; sub < (fused ? 2 : 1); ++sub) {
+        int rank, mode;                                  // mode 0: plain partial, 1: merge with the cache, 2: push
+        if (!fused) { rank = x; mode = 0; }
+        else if (sub == 0) {
+          if (w == 0) continue;
+          const int p_past = t - 1 - (((t - 1 - x) % w + w) % w);     // the position in [t-w, t-1] with p mod w == x
+          if (p_past < 0) continue;
+          rank = t - p_past; mode = 1;
+        } else {
+          if (w > 0 && t % w != x) continue;
+          rank = 0; mode = 2;
+        }
+        const int r = s_rowr[rank];
         if (r < 0) continue;
-        float4 o; float lse;
-        combine_row(c, o, lse);
-        const size_t e = row_elem(r, c % G);
+        const int c = rank * G + g;
+        // Eq. 8 applied to the splits of local row c (weights 2^(lse_s - max)).  An empty split's tile is
+        // unspecified: it is never multiplied.
+        float l_mine = -INFINITY;
+        if (lane < nsplit) l_mine = dsmem_ld_f32(dsmem_addr(lse_a + c * 4, lane));
+        const float mx = warp_max(l_mine);
+        const float w_mine = mx > -INFINITY ? ex2_approx(l_mine - mx) : 0.f;
+        float wsum = 0.f;
+        float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 v[8];                                     // (all remote loads in flight before the first use)
+#pragma unroll
+        for (int s2 = 0; s2 < 8; ++s2)
+          if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
+#pragma unroll
+        for (int s2 = 0; s2 < 8; ++s2) {
+          const float wg = __shfl_sync(0xffffffffu, w_mine, s2);
+          if (s2 < nsplit && wg > 0.f) {
+            wsum += wg;
+            o.x = fmaf(wg, v[s2].x, o.x); o.y = fmaf(wg, v[s2].y, o.y);
+            o.z = fmaf(wg, v[s2].z, o.z); o.w = fmaf(wg, v[s2].w, o.w);
+          }
+        }
+        const float inv = wsum > 0.f ? rcp_approx(wsum) : 0.f;
+        o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+        float lse = wsum > 0.f ? (mx + lg2_approx(wsum)) * kLn2 : -INFINITY;
+        const size_t e = ((size_t)b * R + r) * p.h_q + h * G + g;
         *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
         if (lane == 0) p.part_lse[e] = lse;
-      }
-    } else {
-      // S3 + S4 (one row group): item = (cache slot x, q head g): the slot's past row (position = x mod w, read
-      // and merged with the cache, Eq. 8-9), then the current row if it lands in this slot (pushed): the pop of
-      // position t - w and the push of position t are ordered by the warp.
-      __nv_bfloat16* out = reinterpret_cast<__nv_bfloat16*>(p.out);
-      const int nslot = w > 0 ? w : 1;
-#pragma unroll 1
-      const float* pre = reinterpret_cast<const float*>(smem + lay.pre);
-      for (int k = warp; split + nsplit * k < nslot * G; k += nwarps) {
-        const int it = split + nsplit * k;
-        const int x = it / G, g = it - x * G;
-        const int hq = h * G + g;
-        const size_t ce = ((size_t)b * nslot + x) * p.h_q + hq;
-        if (w > 0) {
-          const int p_past = t - 1 - (((t - 1 - x) % w + w) % w);      // the position in [t-w, t-1] with p mod w == x
-          const int rank = t - p_past;
-          const int r = p_past >= 0 ? s_rowr[rank] : -1;
-          if (r >= 0) {
-            const bool cached = s_cpos[x] == p_past;
-            float lc = -INFINITY;
-            float4 vc = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (cached) {
-              if (k < kPreItems) {
-                lc = pre[k * kPreStride + 128];
-                vc = *reinterpret_cast<const float4*>(pre + k * kPreStride + lane * 4);
-              } else {
-                lc = p.cache_lse[ce];
-                vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
-              }
+        if (mode == 0) continue;
+        const size_t ce = ((size_t)b * nslot + x) * p.h_q + h * G + g;
+        bool write_back = w > 0;
+        if (mode == 1) {
+          if (s_cpos[x] == t - rank) {                   // something is cached for this position
+            float lc;
+            float4 vc;
+            if (k < kPreItems) {
+              lc = pre[k * kPreStride + 128];
+              vc = *reinterpret_cast<const float4*>(pre + k * kPreStride + lane * 4);
+            } else {
+              lc = p.cache_lse[ce];
+              vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
             }
-            float4 o; float lp;
-            combine_row(rank * G + g, o, lp);
-            const size_t e = row_elem(r, g);
-            *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
-            if (lane == 0) p.part_lse[e] = lp;
-            float4 res = o;
-            float lse = lp;
             if (lc > -INFINITY) {
-              if (lp == -INFINITY) { res = vc; lse = lc; }
+              if (lse == -INFINITY) { o = vc; lse = lc; }
               else {
-                const float m2 = fmaxf(lc, lp);
-                const float wc = __expf(lc - m2), wp = __expf(lp - m2);
-                const float iv = 1.f / (wc + wp);
-                res.x = (wc * vc.x + wp * o.x) * iv; res.y = (wc * vc.y + wp * o.y) * iv;
-                res.z = (wc * vc.z + wp * o.z) * iv; res.w = (wc * vc.w + wp * o.w) * iv;
-                lse = m2 + __logf(wc + wp);
+                const float m2 = fmaxf(lc, lse);
+                const float wc = ex2_approx((lc - m2) * kLog2e), wp = ex2_approx((lse - m2) * kLog2e);
+                const float iv = rcp_approx(wc + wp);
+                o.x = (wc * vc.x + wp * o.x) * iv; o.y = (wc * vc.y + wp * o.y) * iv;
+                o.z = (wc * vc.z + wp * o.z) * iv; o.w = (wc * vc.w + wp * o.w) * iv;
+                lse = m2 + lg2_approx(wc + wp) * kLn2;
               }
             }
-            store_bf16x4(out + e * 128 + lane * 4, res);
-            if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lse;
-            if (p_past != t - w) {                                     // not popped: written back
-              *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = res;
-              if (lane == 0) p.cache_lse[ce] = lse;
-            }
           }
+          write_back = rank != w;                        // the row at position t - w is popped after its last merge
         }
-        if (w == 0 || t % w == x) {                                    // the current row: out = O_org, pushed
-          const int r = s_rowr[0];
-          if (r >= 0) {
-            float4 o; float lp;
-            combine_row(g, o, lp);
-            const size_t e = row_elem(r, g);
-            *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = o;
-            if (lane == 0) p.part_lse[e] = lp;
-            store_bf16x4(out + e * 128 + lane * 4, o);
-            if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lp;
-            if (w > 0) {
-              *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = o;
-              if (lane == 0) p.cache_lse[ce] = lp;
-            }
-          }
+        store_bf16x4(reinterpret_cast<__nv_bfloat16*>(p.out) + e * 128 + lane * 4, o);
+        if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lse;
+        if (write_back) {
+          *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = o;
+          if (lane == 0) p.cache_lse[ce] = lse;
         }
       }
     }
@@ -731,10 +706,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         const int r = it / G, g = it - r * G;
         const int pos = s_posr[r];
         if (pos >= 0 && pos <= t && pos >= t - w) continue;
-        const size_t e = row_elem(r, g);
+        const size_t e = ((size_t)b * R + r) * p.h_q + h * G + g;
         *reinterpret_cast<float4*>(p.part_o + e * 128 + lane * 4) = make_float4(0.f, 0.f, 0.f, 0.f);
         if (lane == 0) p.part_lse[e] = -INFINITY;
-        if (p.fused) {
+        if (fused) {
           store_bf16x4(reinterpret_cast<__nv_bfloat16*>(p.out) + e * 128 + lane * 4, make_float4(0.f, 0.f, 0.f, 0.f));
           if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = -INFINITY;
         }
