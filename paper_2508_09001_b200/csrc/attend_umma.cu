@@ -146,10 +146,10 @@ constexpr int kOrdNegInf = (int)0x807fffff;   // f2o(-inf)
 constexpr int kPreItems = 16;                 // output-cache operands a CTA prefetches for its merge items
 constexpr int kPreStride = 132;               // floats per prefetched item: o[128], lse, padding (16 B multiple)
 struct UmmaLayout {
-  int q, p, ring, list, pre, total;
+  int q, p, ring, list, pre, bt, total;
   int p_buf_bytes, p_hl_bytes;
 };
-__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split) {
+__host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pages_per_split, int bt_pages) {
   UmmaLayout L;
   const int natom = (2 * NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
@@ -159,7 +159,8 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
   L.ring = L.p + NP * L.p_buf_bytes;
   L.list = L.ring + NS * kSlotBytes;         // int32 [3][pages_per_split]
   L.pre = (L.list + 3 * pages_per_split * 4 + 15) & ~15;   // prefetched cache operands [kPreItems][128 o + lse + pad]
-  L.total = L.pre + kPreItems * kPreStride * 4;
+  L.bt = L.pre + kPreItems * kPreStride * 4;           // int32 [bt_pages] block-table row of the sequence
+  L.total = L.bt + bt_pages * 4;
   return L;
 }
 
@@ -169,6 +170,7 @@ struct UmmaCfg {
   int NP;         // P buffers (1 or 2)
   int NSB;        // S buffers in TMEM (1 or 2)
   int tmem_cols;  // power of two >= (NSB + 2) * NT
+  int bt_pages;   // block-table entries staged in shared memory (0: looked up in global memory)
 };
 
 // NCH = NT / 16; every softmax thread owns one key and NC = 4 * NCH of the padded rows (four column groups).
@@ -193,7 +195,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(16) float s_alpha[NT];
   __shared__ __align__(16) float s_L[NT];        // row sums (epilogue)
   const int pps = p.pages_per_split;
-  const UmmaLayout lay = umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, pps);
+  const UmmaLayout lay = umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, pps, cfg.bt_pages);
   uint64_t* k_full = bars;               // [NK <= 3]
   uint64_t* k_empty = bars + 3;          // [NK <= 3]
   uint64_t* v_full = bars + 6;           // [NV <= 3]
@@ -229,12 +231,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   if (tid <= kMaxWindow) s_rowr[tid] = -1;
   __syncthreads();
-  pdl_wait();
-  pdl_trigger();
-  // Global loads that depend on nothing are issued first (count, length, Q, q_pos, the list entries of this
-  // split): Q and q_pos are held in registers across the list loop so that their round trip overlaps the list's
-  // (in program order after it they were issued only once block_table[j], the one dependent load, had returned).
-  const int count = p.sel_count[unit];
+  // Inside retro_decode_step (fused) the kernel that precedes this one is the select kernel of the same step, and
+  // it releases its dependents only after its own dependency wait: everything older than it is complete when this
+  // CTA starts.  Only the selection (sel_*) needs the wait; the query window, positions, lengths, block table and
+  // output cache do not, so that part of the prologue - and the idle warp's S4 service - overlap the select kernel.
+  // Stand-alone (retro_sparse_attend) nothing is known about the predecessor: wait first.
+  if (!p.fused) { pdl_wait(); pdl_trigger(); }
   const int L = p.seq_lens[b];
   // One row group: the unit's R * G rows (<= NT).  Several row groups (R * G > 128): every CTA fetches all of them
   // and keeps its own ranks (the rank of a row is only known once q_pos and the length are back).
@@ -259,19 +261,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   int my_pos_raw = -1;
   if (tid < R) my_pos_raw = __ldg(p.q_pos + b * R + tid);
-  for (int i = tid; i < pps; i += kUmmaThreads) {
-    const int idx = split * pps + i;
-    int j = 0, prev = 0;
-    if (idx < p.k_max) {
-      j = p.sel_pages[unit * p.k_max + idx];
-      prev = p.sel_prev[unit * p.k_max + idx];
-    }
-    int phys = 0;
-    if (idx < count) phys = p.block_table[(size_t)b * p.max_pages + j];
-    s_list[i] = j;
-    s_list[pps + i] = prev;
-    s_list[2 * pps + i] = phys;
-  }
+  // the sequence's block-table row goes to shared memory when it is small enough (cfg.bt_pages > 0): the logical ->
+  // physical lookup of the selected pages then costs no global round trip after the wait
+  int32_t* s_bt = reinterpret_cast<int32_t*>(smem + lay.bt);
+  for (int i = tid; i < cfg.bt_pages; i += kUmmaThreads)
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(s_bt + i)),
+                 "l"(p.block_table + (size_t)b * p.max_pages + i) : "memory");
+  asm volatile("cp.async.commit_group;" ::: "memory");
   const int t = L - 1;
   // rows of the padded tile that no window row fills must read as zeros for the tensor core
   for (int i = tid; i < NT * 16; i += kUmmaThreads)
@@ -304,18 +300,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     s_alpha[c] = 1.f;
     s_L[c] = 0.f;
   }
-  const int beg = min(split * pps, count);
-  const int end = min(beg + pps, count);
-  const int n_my = end - beg;
-  const int nblk = (n_my + kPB - 1) / kPB;
-  const int colS = 0, colO = cfg.NSB * NT;
-  fence_proxy_async();          // Q written through the generic proxy, read by the tensor core
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = tmem_ptr_s;
-
-  if (warp == 3 && p.fused && p.window > 0) {
+  if (p.fused) {
+    __syncthreads();             // s_posr / s_rowr are complete
+    if (warp == 3 && p.window > 0) {
     // ---- the idle warp serves S4 while the others attend: (a) the cache operands of this CTA's merge items are
     // prefetched into shared memory, (b) cache_pos is snapshotted, (c) the CTA reports that it has read cache_pos;
     // the LAST CTA of the sequence to report rewrites it (the new values depend on q_pos and t only: Push slot
@@ -348,8 +335,36 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         else if (pos > t - w && pos < t && pos >= 0) p.cache_pos[b * w + pos % w] = pos;
       }
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+      }
+    pdl_wait();
+    pdl_trigger();
   }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();               // block-table row (and the S4 prefetch) landed
+  const int count = p.sel_count[unit];
+  for (int i = tid; i < pps; i += kUmmaThreads) {
+    const int idx = split * pps + i;
+    int j = 0, prev = 0;
+    if (idx < p.k_max) {
+      j = p.sel_pages[unit * p.k_max + idx];
+      prev = p.sel_prev[unit * p.k_max + idx];
+    }
+    int phys = 0;
+    if (idx < count) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
+    s_list[i] = j;
+    s_list[pps + i] = prev;
+    s_list[2 * pps + i] = phys;
+  }
+  const int beg = min(split * pps, count);
+  const int end = min(beg + pps, count);
+  const int n_my = end - beg;
+  const int nblk = (n_my + kPB - 1) / kPB;
+  const int colS = 0, colO = cfg.NSB * NT;
+  fence_proxy_async();          // Q written through the generic proxy, read by the tensor core
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_ptr_s;
 
   if (nblk > 0) {
     if (warp < 2) {
@@ -638,16 +653,16 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         const int c = rank * G + g;
         // Eq. 8 applied to the splits of local row c (weights 2^(lse_s - max)).  An empty split's tile is
         // unspecified: it is never multiplied.
+        float4 v[8];                                     // (all remote loads in flight before the first use)
+#pragma unroll
+        for (int s2 = 0; s2 < 8; ++s2)
+          if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
         float l_mine = -INFINITY;
         if (lane < nsplit) l_mine = dsmem_ld_f32(dsmem_addr(lse_a + c * 4, lane));
         const float mx = warp_max(l_mine);
         const float w_mine = mx > -INFINITY ? ex2_approx(l_mine - mx) : 0.f;
         float wsum = 0.f;
         float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-        float4 v[8];                                     // (all remote loads in flight before the first use)
-#pragma unroll
-        for (int s2 = 0; s2 < 8; ++s2)
-          if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
 #pragma unroll
         for (int s2 = 0; s2 < 8; ++s2) {
           const float wg = __shfl_sync(0xffffffffu, w_mine, s2);
@@ -823,13 +838,14 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   // two P buffers; the ring takes what is left (>= 2 slots: K and V of one block in flight per CTA).
   UmmaCfg cfg;
   cfg.NSB = 2;
+  cfg.bt_pages = d->max_pages_per_seq <= 4096 ? d->max_pages_per_seq : 0;   // <= 16 KB of shared memory
   int slots = 0;
   auto plan = [&](int budget) {
     cfg.NP = 2;
-    slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
+    slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split, cfg.bt_pages).total) / kSlotBytes;
     if (slots < 4) {
       cfg.NP = 1;
-      slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split).total) / kSlotBytes;
+      slots = (budget - umma_layout(NT, 0, cfg.NP, prm.pages_per_split, cfg.bt_pages).total) / kSlotBytes;
     }
   };
   plan(kUmmaSmemBudget);
@@ -841,7 +857,7 @@ int launch_attend_umma(const retro_desc_t* d, const AttendParams& prm, cudaStrea
   while (cols < (cfg.NSB + 2) * NT) cols <<= 1;
   if (cols > kTmemCols) return RETRO_ERR_UNSUPPORTED;
   cfg.tmem_cols = cols;
-  const size_t smem = (size_t)umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, prm.pages_per_split).total;
+  const size_t smem = (size_t)umma_layout(NT, cfg.NK + cfg.NV, cfg.NP, prm.pages_per_split, cfg.bt_pages).total;
   switch (nch) {
     case 1: return launch_nch<1>(d, prm, cfg, smem, map_k, map_v, s);
     case 2: return launch_nch<2>(d, prm, cfg, smem, map_k, map_v, s);
