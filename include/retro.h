@@ -133,7 +133,10 @@ int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, cons
                              int32_t* cache_pos, void* out, float* out_lse, void* stream);
 
 /* AppendKV (Alg. 1 line 3).  Writes k_new / v_new [B][h_k][d] T into position seq_lens[b] - 1 of
- * each sequence (seq_lens already counts the new token). */
+ * each sequence (seq_lens already counts the new token).  Capacity: a sequence holds at most
+ * max_pages_per_seq * page_size tokens; positions beyond that are never written (every kernel clamps its page count
+ * to max_pages_per_seq), and the window-advance helpers below leave the length of a full sequence unchanged (it is
+ * not advanced: check seq_lens before appending to it - retro_decode_step_host skips the append itself). */
 int retro_append_kv(const retro_desc_t* desc, const void* k_new, const void* v_new, const int32_t* block_table,
                     const int32_t* seq_lens, void* k_pages, void* v_pages, void* stream);
 
@@ -164,21 +167,38 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st /*
                       const void* q_win, const int32_t* q_pos, const void* q_cur, void* out, float* out_lse,
                       void* stream);
 
-/* End-to-end step with HOST buffers (pinned for async copies): copies this step's inputs host->device
- * (q_new, k_new, v_new: the new token's query [B][h_q][d] and key/value [B][h_k][d]), advances seq_lens and the
- * query window ring on the device, appends the token to the KV pool, runs retro_decode_step, and copies
- * out [B][w+1][h_q][d] device->host.  dev_io holds caller-owned device staging buffers. */
+/* Measurement helpers.  retro_decode_step_part enqueues ONE of the step's kernels exactly as retro_decode_step
+ * does: part 0 = S1 + S2 (select kernel, newest page's digest rebuilt in line), part 1 = S3 + S4 (attend kernel
+ * with the split combine and the cache merge in its epilogue; S3 then S4 as two launches where the fusion does not
+ * apply: fp32, or more than 128 query rows per KV head).  retro_launches_per_step: kernels retro_decode_step
+ * enqueues for this descriptor (2 or 3). */
+int retro_decode_step_part(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
+                           const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, int32_t part /*HOST*/,
+                           void* stream);
+int retro_launches_per_step(const retro_desc_t* desc /*HOST*/, int32_t* launches /*HOST out*/);
+
+/* End-to-end step with HOST buffers (pinned for async copies): ONE host->device copy of this step's packed
+ * inputs host_qkv_new = [q_new [B][h_q][d] | k_new [B][h_k][d] | v_new [B][h_k][d]] (T), one launch that advances
+ * seq_lens and the query window ring and appends the token to the KV pool, retro_decode_step, and ONE device->host
+ * copy of out [B][w+1][h_q][d].  Five stream operations, CUDA-graph capturable (the host addresses are baked into a
+ * captured graph: refill the same pinned buffers before every replay).  dev_io holds caller-owned device staging
+ * buffers; batch <= 64. */
 typedef struct retro_step_io {
-  void* q_new;      /* device [B][h_q][d] T            */
-  void* k_new;      /* device [B][h_k][d] T            */
-  void* v_new;      /* device [B][h_k][d] T            */
-  void* q_win;      /* device [B][w+1][h_q][d] T ring  */
-  int32_t* q_pos;   /* device [B][w+1]                 */
-  void* out;        /* device [B][w+1][h_q][d] T       */
+  void* qkv_new;    /* device [q_new | k_new | v_new] T, packed as above */
+  void* q_win;      /* device [B][w+1][h_q][d] T ring                   */
+  int32_t* q_pos;   /* device [B][w+1]                                  */
+  void* out;        /* device [B][w+1][h_q][d] T                        */
 } retro_step_io_t;
 int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* dev_io,
-                           const void* host_q_new, const void* host_k_new, const void* host_v_new,
-                           void* host_out, void* stream);
+                           const void* host_qkv_new /*HOST*/, void* host_out /*HOST*/, void* stream);
+
+/* The same for n_layers layers of one decode step with ONE copy in and ONE copy out: host_qkv_new
+ * [n_layers][q | k | v], host_out [n_layers][B][w+1][h_q][d].  states / dev_ios: HOST arrays of n_layers records;
+ * the records' qkv_new (and out) device buffers must be consecutive slices of one device buffer
+ * (dev_ios[l].qkv_new == dev_ios[0].qkv_new + l * token bytes; likewise out), else RETRO_ERR_ARG. */
+int retro_decode_steps_host(const retro_desc_t* desc, const retro_layer_state_t* states /*HOST*/,
+                            const retro_step_io_t* dev_ios /*HOST*/, int32_t n_layers /*HOST*/,
+                            const void* host_qkv_new /*HOST*/, void* host_out /*HOST*/, void* stream);
 
 /* NEXT-1: UpdateKV of Alg. 1 line 2 (Sec. 2.4): overwrite the K
  * and V rows of up to n_upd past tokens per sequence with the caller's re-embedded K^, V^.

@@ -24,7 +24,8 @@ EXPORTED = [
     "retro_version", "retro_update_page_bounds", "retro_select_pages", "retro_sparse_attend",
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
     "retro_window_advance", "retro_window_advance_layers", "retro_update_kv",
-    "retro_budget_policy", "retro_build_mask", "retro_step_diagnostics",
+    "retro_budget_policy", "retro_build_mask", "retro_step_diagnostics", "retro_decode_step_part",
+    "retro_launches_per_step", "retro_decode_steps_host",
 ]
 
 
@@ -50,7 +51,7 @@ class RetroLayerState(C.Structure):
 
 
 class RetroStepIO(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("q_new", "k_new", "v_new", "q_win", "q_pos", "out")]
+    _fields_ = [(n, C.c_void_p) for n in ("qkv_new", "q_win", "q_pos", "out")]
 
 
 class RetroError(RuntimeError):
@@ -215,10 +216,32 @@ def retro_decode_step(desc, state: RetroLayerState, q_win, q_pos, q_cur, out, ou
                                     _p(out_lse), _stream(stream)), "retro_decode_step")
 
 
-def retro_decode_step_host(desc, state: RetroLayerState, io: RetroStepIO, host_q_new, host_k_new, host_v_new,
-                           host_out, stream=None):
-    _check(_lib().retro_decode_step_host(C.byref(desc), C.byref(state), C.byref(io), _p(host_q_new), _p(host_k_new),
-                                         _p(host_v_new), _p(host_out), _stream(stream)), "retro_decode_step_host")
+def retro_decode_step_part(desc, state: RetroLayerState, q_win, q_pos, q_cur, out, part, out_lse=None, stream=None):
+    """One kernel of retro_decode_step: part 0 = S1 + S2, part 1 = S3 + S4 (measurement helper)."""
+    _check(_lib().retro_decode_step_part(C.byref(desc), C.byref(state), _p(q_win), _p(q_pos), _p(q_cur), _p(out),
+                                         _p(out_lse), C.c_int32(part), _stream(stream)), "retro_decode_step_part")
+
+
+def retro_launches_per_step(desc) -> int:
+    n = C.c_int32(0)
+    _check(_lib().retro_launches_per_step(C.byref(desc), C.byref(n)), "retro_launches_per_step")
+    return n.value
+
+
+def retro_decode_step_host(desc, state: RetroLayerState, io: RetroStepIO, host_qkv_new, host_out, stream=None):
+    """host_qkv_new: pinned host tensor holding [q_new | k_new | v_new] back to back."""
+    _check(_lib().retro_decode_step_host(C.byref(desc), C.byref(state), C.byref(io), _p(host_qkv_new), _p(host_out),
+                                         _stream(stream)), "retro_decode_step_host")
+
+
+def retro_decode_steps_host(desc, states, ios, host_qkv_new, host_out, stream=None):
+    """All layers of one decode step with one copy in and one copy out (states / ios: lists of the C structs; the
+    ios' qkv_new / out buffers must be consecutive slices of one device buffer each)."""
+    n = len(states)
+    st_arr = (RetroLayerState * n)(*states)
+    io_arr = (RetroStepIO * n)(*ios)
+    _check(_lib().retro_decode_steps_host(C.byref(desc), st_arr, io_arr, C.c_int32(n), _p(host_qkv_new), _p(host_out),
+                                          _stream(stream)), "retro_decode_steps_host")
 
 
 class LayerBuffers:

@@ -340,8 +340,10 @@ static int check_state(const retro_desc_t* desc, const retro_layer_state_t* st) 
   return RETRO_OK;
 }
 
-int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
-                      const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, void* stream) {
+// parts: bit 0 = S1 + S2 (the select kernel, newest digest rebuilt in line), bit 1 = S3 + S4
+static int decode_step_parts(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
+                             const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, int parts,
+                             void* stream) {
   RETRO_CHECK_DESC(desc);
   int rc = check_state(desc, st);
   if (rc != RETRO_OK) return rc;
@@ -349,12 +351,15 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, c
   const WorkspaceLayout wl = workspace_layout(desc);
   if (st->workspace_bytes < wl.total) return RETRO_ERR_WORKSPACE;
   cudaStream_t s = (cudaStream_t)stream;
-  // S1 + S2: the digest of the newest token's page is rebuilt inside the select kernel (by the warp that scores
-  // that page) and written back, so the step needs no separate digest launch.
-  rc = launch_select_pages(desc, wl, q_cur, st->bounds, st->seq_lens, st->budget_pages, st->last_loaded,
-                           st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s, st->k_pages,
-                           st->block_table);
-  if (rc != RETRO_OK) return rc;
+  if (parts & 1) {
+    // S1 + S2: the digest of the newest token's page is rebuilt inside the select kernel (by the warp that scores
+    // that page) and written back, so the step needs no separate digest launch.
+    rc = launch_select_pages(desc, wl, q_cur, st->bounds, st->seq_lens, st->budget_pages, st->last_loaded,
+                             st->sel_pages, st->sel_prev, st->sel_count, nullptr, st->workspace, s, st->k_pages,
+                             st->block_table);
+    if (rc != RETRO_OK) return rc;
+  }
+  if (!(parts & 2)) return RETRO_OK;
   // S3 (+ S4): on the tensor-core path with one row group the attend kernel also merges the output cache (the
   // splits of a unit are one cluster: split combine and Eq. 8-9 in its epilogue, TWO launches per layer-step)
   if (attend_can_fuse_merge(desc, wl)) {
@@ -370,31 +375,76 @@ int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, c
                                    st->cache_pos, out, out_lse, s);
 }
 
-int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* io,
-                           const void* host_q_new, const void* host_k_new, const void* host_v_new, void* host_out,
+int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
+                      const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, void* stream) {
+  return decode_step_parts(desc, st, q_win, q_pos, q_cur, out, out_lse, 3, stream);
+}
+
+int retro_decode_step_part(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
+                           const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, int32_t part,
                            void* stream) {
+  if (part != 0 && part != 1) return RETRO_ERR_ARG;
+  return decode_step_parts(desc, st, q_win, q_pos, q_cur, out, out_lse, 1 << part, stream);
+}
+
+int retro_launches_per_step(const retro_desc_t* desc, int32_t* launches) {
+  RETRO_CHECK_DESC(desc);
+  if (launches == nullptr) return RETRO_ERR_ARG;
+  *launches = attend_can_fuse_merge(desc, workspace_layout(desc)) ? 2 : 3;
+  return RETRO_OK;
+}
+
+int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* io,
+                           const void* host_qkv_new, void* host_out, void* stream) {
   RETRO_CHECK_DESC(desc);
   int rc = check_state(desc, st);
   if (rc != RETRO_OK) return rc;
-  if (io == nullptr || host_q_new == nullptr || host_k_new == nullptr || host_v_new == nullptr ||
-      host_out == nullptr)
-    return RETRO_ERR_ARG;
-  RETRO_CHECK_PTR(io->q_new); RETRO_CHECK_PTR(io->k_new); RETRO_CHECK_PTR(io->v_new); RETRO_CHECK_PTR(io->q_win);
-  RETRO_CHECK_PTR(io->q_pos); RETRO_CHECK_PTR(io->out);
+  if (io == nullptr || host_qkv_new == nullptr || host_out == nullptr) return RETRO_ERR_ARG;
+  RETRO_CHECK_PTR(io->qkv_new); RETRO_CHECK_PTR(io->q_win); RETRO_CHECK_PTR(io->q_pos); RETRO_CHECK_PTR(io->out);
   cudaStream_t s = (cudaStream_t)stream;
   const size_t esz = desc->dtype == RETRO_BF16 ? 2 : 4;
   const size_t q_bytes = (size_t)desc->batch * desc->num_q_heads * desc->head_dim * esz;
   const size_t kv_bytes = (size_t)desc->batch * desc->num_kv_heads * desc->head_dim * esz;
-  RETRO_CUDA_TRY(cudaMemcpyAsync(io->q_new, host_q_new, q_bytes, cudaMemcpyHostToDevice, s));
-  RETRO_CUDA_TRY(cudaMemcpyAsync(io->k_new, host_k_new, kv_bytes, cudaMemcpyHostToDevice, s));
-  RETRO_CUDA_TRY(cudaMemcpyAsync(io->v_new, host_v_new, kv_bytes, cudaMemcpyHostToDevice, s));
-  rc = launch_window_advance(desc, io->q_new, nullptr, 1, st->seq_lens, io->q_win, io->q_pos, nullptr, s);
+  // ONE host->device copy (the packed token), one launch for the window ring + AppendKV, the step's two (three)
+  // kernels, ONE device->host copy: five stream operations, all CUDA-graph capturable
+  RETRO_CUDA_TRY(cudaMemcpyAsync(io->qkv_new, host_qkv_new, q_bytes + 2 * kv_bytes, cudaMemcpyHostToDevice, s));
+  rc = launch_ingest_token(desc, io->qkv_new, st->block_table, st->seq_lens, io->q_win, io->q_pos, st->k_pages,
+                           st->v_pages, s);
   if (rc != RETRO_OK) return rc;
-  rc = launch_append_kv(desc, io->k_new, io->v_new, st->block_table, st->seq_lens, st->k_pages, st->v_pages, s);
-  if (rc != RETRO_OK) return rc;
-  rc = retro_decode_step(desc, st, io->q_win, io->q_pos, io->q_new, io->out, nullptr, stream);
+  rc = retro_decode_step(desc, st, io->q_win, io->q_pos, io->qkv_new, io->out, nullptr, stream);
   if (rc != RETRO_OK) return rc;
   RETRO_CUDA_TRY(cudaMemcpyAsync(host_out, io->out, q_bytes * (desc->window + 1), cudaMemcpyDeviceToHost, s));
+  return RETRO_OK;
+}
+
+int retro_decode_steps_host(const retro_desc_t* desc, const retro_layer_state_t* states, const retro_step_io_t* ios,
+                            int32_t n_layers, const void* host_qkv_new, void* host_out, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  if (states == nullptr || ios == nullptr || n_layers < 1 || host_qkv_new == nullptr || host_out == nullptr)
+    return RETRO_ERR_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t esz = desc->dtype == RETRO_BF16 ? 2 : 4;
+  const size_t q_bytes = (size_t)desc->batch * desc->num_q_heads * desc->head_dim * esz;
+  const size_t kv_bytes = (size_t)desc->batch * desc->num_kv_heads * desc->head_dim * esz;
+  const size_t tok_bytes = q_bytes + 2 * kv_bytes, out_bytes = q_bytes * (desc->window + 1);
+  for (int l = 0; l < n_layers; ++l) {
+    int rc = check_state(desc, &states[l]);
+    if (rc != RETRO_OK) return rc;
+    RETRO_CHECK_PTR(ios[l].qkv_new); RETRO_CHECK_PTR(ios[l].q_win); RETRO_CHECK_PTR(ios[l].q_pos); RETRO_CHECK_PTR(ios[l].out);
+    // the layers' staging buffers are slices of ONE device buffer each, so that one copy serves them all
+    if (static_cast<char*>(ios[l].qkv_new) != static_cast<char*>(ios[0].qkv_new) + l * tok_bytes ||
+        static_cast<char*>(ios[l].out) != static_cast<char*>(ios[0].out) + l * out_bytes)
+      return RETRO_ERR_ARG;
+  }
+  RETRO_CUDA_TRY(cudaMemcpyAsync(ios[0].qkv_new, host_qkv_new, tok_bytes * n_layers, cudaMemcpyHostToDevice, s));
+  for (int l = 0; l < n_layers; ++l) {
+    int rc = launch_ingest_token(desc, ios[l].qkv_new, states[l].block_table, states[l].seq_lens, ios[l].q_win,
+                                 ios[l].q_pos, states[l].k_pages, states[l].v_pages, s);
+    if (rc != RETRO_OK) return rc;
+    rc = retro_decode_step(desc, &states[l], ios[l].q_win, ios[l].q_pos, ios[l].qkv_new, ios[l].out, nullptr, stream);
+    if (rc != RETRO_OK) return rc;
+  }
+  RETRO_CUDA_TRY(cudaMemcpyAsync(host_out, ios[0].out, out_bytes * n_layers, cudaMemcpyDeviceToHost, s));
   return RETRO_OK;
 }
 

@@ -28,6 +28,7 @@
 //   warps 4..19 softmax: TMEM lane quadrant = warp % 4 (32 keys), column group = (warp - 4) / 4 (a quarter of the rows).
 // Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
 #include <cuda.h>
+#include <cuda_fp16.h>
 
 #include <cstdlib>
 
@@ -587,8 +588,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       tc_fence_after();
       softmax_bar();                                       // s_L complete
       // thread = channel `key`; its NC rows: O = (O_hi + O_lo) / L into the staging tile [row][128 channels] (the
-      // K / V ring is idle: every tensor-core read of it has retired), base-2 lse next to it
-      float* stage = reinterpret_cast<float*>(smem + lay.ring);
+      // K / V ring is idle: every tensor-core read of it has retired), base-2 lse next to it.  The tile is fp16
+      // (|o| <= max |v|, 11 significant bits: far inside the bf16 tolerance): distributed shared memory serves
+      // ~19 B/clk per SM, and the combine below is bound by exactly that.
+      __half* stage = reinterpret_cast<__half*>(smem + lay.ring);
 #pragma unroll
       for (int i = 0; i < NCH; ++i) {
         if (cbeg + 4 * i < rows_cta) {                      // warp-uniform
@@ -602,7 +605,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
             if (c < rows_cta) {
               const float l = s_L[c];
               const float inv = rcp_approx(l);
-              stage[c * 128 + key] = l > 0.f ? (__uint_as_float(oh[u]) + __uint_as_float(ol[u])) * inv : 0.f;
+              stage[c * 128 + key] = __float2half_rn(l > 0.f ? (__uint_as_float(oh[u]) + __uint_as_float(ol[u])) * inv : 0.f);
               if (key == 0) s_lse2[c] = l > 0.f ? s_mref[c] + lg2_approx(l) : -INFINITY;
             }
           }
@@ -622,7 +625,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   cluster_arrive();
   cluster_wait();
   {
-    const uint32_t stage_a = smem_u32(smem + lay.ring) + lane * 16, lse_a = smem_u32(s_lse2);
+    const uint32_t stage_a = smem_u32(smem + lay.ring) + lane * 8, lse_a = smem_u32(s_lse2);
     const float* pre = reinterpret_cast<const float*>(smem + lay.pre);
     const int nsplit = p.nsplit, w = p.window, nwarps = kUmmaThreads / 32;
     const bool fused = p.fused != 0;
@@ -653,10 +656,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         const int c = rank * G + g;
         // Eq. 8 applied to the splits of local row c (weights 2^(lse_s - max)).  An empty split's tile is
         // unspecified: it is never multiplied.
-        float4 v[8];                                     // (all remote loads in flight before the first use)
+        uint2 v[8];                                      // 4 halves per lane; all remote loads in flight before the first use
 #pragma unroll
         for (int s2 = 0; s2 < 8; ++s2)
-          if (s2 < nsplit) v[s2] = dsmem_ld_v4(dsmem_addr(stage_a + c * 512, s2));
+          if (s2 < nsplit) v[s2] = dsmem_ld_v2(dsmem_addr(stage_a + c * 256, s2));
         float l_mine = -INFINITY;
         if (lane < nsplit) l_mine = dsmem_ld_f32(dsmem_addr(lse_a + c * 4, lane));
         const float mx = warp_max(l_mine);
@@ -668,8 +671,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           const float wg = __shfl_sync(0xffffffffu, w_mine, s2);
           if (s2 < nsplit && wg > 0.f) {
             wsum += wg;
-            o.x = fmaf(wg, v[s2].x, o.x); o.y = fmaf(wg, v[s2].y, o.y);
-            o.z = fmaf(wg, v[s2].z, o.z); o.w = fmaf(wg, v[s2].w, o.w);
+            const float2 f01 = __half22float2(*reinterpret_cast<const __half2*>(&v[s2].x));
+            const float2 f23 = __half22float2(*reinterpret_cast<const __half2*>(&v[s2].y));
+            o.x = fmaf(wg, f01.x, o.x); o.y = fmaf(wg, f01.y, o.y);
+            o.z = fmaf(wg, f23.x, o.z); o.w = fmaf(wg, f23.y, o.w);
           }
         }
         const float inv = wsum > 0.f ? rcp_approx(wsum) : 0.f;

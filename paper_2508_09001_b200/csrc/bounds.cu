@@ -71,7 +71,7 @@ __global__ void append_kv_kernel(const T* __restrict__ k_new, const T* __restric
   if (idx >= B * h_k * 32) return;
   const int col = idx & 15, kv = (idx >> 4) & 1, h = (idx >> 5) % h_k, b = idx / (32 * h_k);
   const int pos = seq_lens[b] - 1;
-  if (pos < 0) return;
+  if (pos < 0 || pos / P >= max_pages) return;   // a sequence never outgrows its block-table row
   const int phys = block_table[(size_t)b * max_pages + pos / P];
   const T* src = (kv ? v_new : k_new) + ((size_t)b * h_k + h) * D;
   T* dst = (kv ? v_pages : k_pages) + (((size_t)phys * h_k + h) * P + pos % P) * D;
@@ -134,9 +134,10 @@ int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat
 
 // ---- window ring bookkeeping: seq_lens++, q_win[slot] <- q_new, q_pos[slot] <- new position -----------
 // Single CTA (the payload is B*h_q*256 bytes).  All threads read the step counter before thread 0 bumps it.
+// A sequence whose block-table row is full (seq_len == capacity) is NOT advanced: nothing is written for it.
 __device__ __forceinline__ void window_advance_cta(const uint4* __restrict__ q_src, int32_t* step_counter,
                                                    int pool_steps, int32_t* seq_lens, uint4* q_win, int32_t* q_pos,
-                                                   uint4* q_cur_out, int B, int h_q, int rows) {
+                                                   uint4* q_cur_out, int B, int h_q, int rows, int capacity) {
   __shared__ int s_pos[64];
   const int row_chunks = h_q * 16;   // uint4 per [h_q][d] block (a q row is 256 B)
   size_t src_off = 0;
@@ -150,14 +151,16 @@ __device__ __forceinline__ void window_advance_cta(const uint4* __restrict__ q_s
     const int b = i / row_chunks, c = i % row_chunks;
     const int pos = s_pos[b];
     const uint4 v = q_src[src_off + i];
-    q_win[((size_t)b * rows + pos % rows) * row_chunks + c] = v;
+    if (pos < capacity) q_win[((size_t)b * rows + pos % rows) * row_chunks + c] = v;
     if (q_cur_out != nullptr) q_cur_out[i] = v;
   }
   __syncthreads();
   for (int b = threadIdx.x; b < B; b += blockDim.x) {
     const int pos = s_pos[b];
-    q_pos[b * rows + pos % rows] = pos;
-    seq_lens[b] = pos + 1;
+    if (pos < capacity) {
+      q_pos[b * rows + pos % rows] = pos;
+      seq_lens[b] = pos + 1;
+    }
   }
   if (threadIdx.x == 0 && step_counter != nullptr) *step_counter += 1;
 }
@@ -165,20 +168,62 @@ __device__ __forceinline__ void window_advance_cta(const uint4* __restrict__ q_s
 __global__ void __launch_bounds__(1024) window_advance_kernel(const uint4* __restrict__ q_src, int32_t* step_counter,
                                                                int pool_steps, int32_t* seq_lens, uint4* q_win,
                                                                int32_t* q_pos, uint4* q_cur_out, int B, int h_q,
-                                                               int rows) {
+                                                               int rows, int capacity) {
   pdl_wait();
   pdl_trigger();
-  window_advance_cta(q_src, step_counter, pool_steps, seq_lens, q_win, q_pos, q_cur_out, B, h_q, rows);
+  window_advance_cta(q_src, step_counter, pool_steps, seq_lens, q_win, q_pos, q_cur_out, B, h_q, rows, capacity);
 }
 
 // one CTA per layer record
 __global__ void __launch_bounds__(1024) window_advance_layers_kernel(const retro_advance_rec_t* __restrict__ table,
-                                                                      int pool_steps, int B, int h_q, int rows) {
+                                                                      int pool_steps, int B, int h_q, int rows,
+                                                                      int capacity) {
   pdl_wait();
   pdl_trigger();
   const retro_advance_rec_t rec = table[blockIdx.x];
   window_advance_cta((const uint4*)rec.q_pool, rec.step_counter, pool_steps, rec.seq_lens, (uint4*)rec.q_win,
-                     rec.q_pos, (uint4*)rec.q_cur_out, B, h_q, rows);
+                     rec.q_pos, (uint4*)rec.q_cur_out, B, h_q, rows, capacity);
+}
+
+// ---- host-buffer step: window advance + AppendKV of the packed new token [q | k | v] in one launch ----------------
+template <typename T, int D, int P>
+__global__ void __launch_bounds__(1024) ingest_token_kernel(const uint4* __restrict__ qkv_new, int32_t* seq_lens,
+                                                            uint4* q_win, int32_t* q_pos,
+                                                            const int32_t* __restrict__ block_table, T* k_pages,
+                                                            T* v_pages, int B, int h_q, int h_k, int rows,
+                                                            int max_pages) {
+  __shared__ int s_full[64];
+  pdl_wait();
+  pdl_trigger();
+  for (int b = threadIdx.x; b < B; b += blockDim.x) s_full[b] = seq_lens[b] >= max_pages * P;
+  __syncthreads();
+  window_advance_cta(qkv_new, nullptr, 1, seq_lens, q_win, q_pos, nullptr, B, h_q, rows, max_pages * P);
+  __syncthreads();               // seq_lens[b] now counts the new token (unless the sequence is full: no append)
+  const uint4* k_new = qkv_new + (size_t)B * h_q * 16;
+  const uint4* v_new = k_new + (size_t)B * h_k * 16;
+  for (int idx = threadIdx.x; idx < B * h_k * 32; idx += blockDim.x) {   // one 16 B chunk each: [B][h_k][2][16]
+    const int col = idx & 15, kv = (idx >> 4) & 1, h = (idx >> 5) % h_k, b = idx / (32 * h_k);
+    const int pos = seq_lens[b] - 1;
+    if (pos < 0 || pos / P >= max_pages || s_full[b]) continue;
+    const int phys = block_table[(size_t)b * max_pages + pos / P];
+    T* dst = (kv ? v_pages : k_pages) + (((size_t)phys * h_k + h) * P + pos % P) * D;
+    reinterpret_cast<uint4*>(dst)[col] = (kv ? v_new : k_new)[((size_t)b * h_k + h) * 16 + col];
+  }
+}
+
+int launch_ingest_token(const retro_desc_t* d, const void* qkv_new, const int32_t* block_table, int32_t* seq_lens,
+                        void* q_win, int32_t* q_pos, void* k_pages, void* v_pages, cudaStream_t s) {
+  if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
+  if (d->dtype == RETRO_BF16)
+    RETRO_CUDA_TRY(launch_kernel(ingest_token_kernel<__nv_bfloat16, 128, 16>, dim3(1), dim3(1024), 0, s,
+                                 (const uint4*)qkv_new, seq_lens, (uint4*)q_win, q_pos, block_table,
+                                 (__nv_bfloat16*)k_pages, (__nv_bfloat16*)v_pages, d->batch, d->num_q_heads,
+                                 d->num_kv_heads, d->window + 1, d->max_pages_per_seq));
+  else
+    RETRO_CUDA_TRY(launch_kernel(ingest_token_kernel<float, 64, 16>, dim3(1), dim3(1024), 0, s, (const uint4*)qkv_new,
+                                 seq_lens, (uint4*)q_win, q_pos, block_table, (float*)k_pages, (float*)v_pages,
+                                 d->batch, d->num_q_heads, d->num_kv_heads, d->window + 1, d->max_pages_per_seq));
+  return RETRO_OK;
 }
 
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
@@ -186,7 +231,7 @@ int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int3
   if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
   RETRO_CUDA_TRY(launch_kernel(window_advance_kernel, dim3(1), dim3(1024), 0, s, (const uint4*)q_new_or_pool,
                                step_counter, pool_steps, seq_lens, (uint4*)q_win, q_pos, (uint4*)q_cur_out, d->batch,
-                               d->num_q_heads, d->window + 1));
+                               d->num_q_heads, d->window + 1, d->max_pages_per_seq * d->page_size));
   return RETRO_OK;
 }
 
@@ -194,7 +239,7 @@ int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_
                                  int pool_steps, cudaStream_t s) {
   if (d->batch > 64) return RETRO_ERR_UNSUPPORTED;
   RETRO_CUDA_TRY(launch_kernel(window_advance_layers_kernel, dim3(n_layers), dim3(1024), 0, s, table, pool_steps,
-                               d->batch, d->num_q_heads, d->window + 1));
+                               d->batch, d->num_q_heads, d->window + 1, d->max_pages_per_seq * d->page_size));
   return RETRO_OK;
 }
 

@@ -108,6 +108,8 @@ int launch_step_diagnostics(const retro_desc_t* d, const int32_t* sel_pages, con
 int launch_update_kv(const retro_desc_t* d, const void* k_hat, const void* v_hat, const int32_t* positions, int n_upd,
                      const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                      cudaStream_t s);
+int launch_ingest_token(const retro_desc_t* d, const void* qkv_new, const int32_t* block_table, int32_t* seq_lens,
+                        void* q_win, int32_t* q_pos, void* k_pages, void* v_pages, cudaStream_t s);
 int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_t* table, int n_layers,
                                  int pool_steps, cudaStream_t s);
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
@@ -193,6 +195,11 @@ __device__ __forceinline__ float4 dsmem_ld_v4(uint32_t addr) {
   float4 v;
   asm volatile("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr)
                : "memory");
+  return v;
+}
+__device__ __forceinline__ uint2 dsmem_ld_v2(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared::cluster.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
   return v;
 }
 __device__ __forceinline__ float dsmem_ld_f32(uint32_t addr) {

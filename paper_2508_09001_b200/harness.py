@@ -14,7 +14,6 @@ import torch
 from . import binding as rb
 from . import workload as wl
 
-KERNELS_PER_LAYER_STEP = 3   # select_pages (newest digest + score + top-k + mask), attend, merge
 KERNELS_PER_STEP = 1         # window_advance_layers: every layer's query stream advances in one launch
 
 
@@ -47,8 +46,12 @@ def stage_bytes(cfg: wl.RetroConfig, seq_lens: List[int]) -> Dict[str, float]:
     q = B * (w + 1) * hq * d * e
     part = B * (w + 1) * hq * (d + 1) * 4
     cache = B * (2 * w * hq * (d + 1) * 4 + (hq * (d + 1) * 4 if w > 0 else 0))
+    bounds = B * hk * (P * d * e + 2 * d * e)
     return {
-        "bounds": B * hk * (P * d * e + 2 * d * e),                  # newest page in, one record out
+        # the two kernels of retro_decode_step: select (S1 of the newest page + S2a-c), attend (S3 + S4)
+        "select_step": digests + B * hq * d * e + mask + bounds,
+        "attend_step": kv + q + part + mask / 2 + cache + q,
+        "bounds": bounds,                                            # newest page in, one record out
         "score": digests + B * hq * d * e + B * hk * (-(-max(seq_lens) // P)) * 8,
         "topk": mask + B * hk * (-(-max(seq_lens) // P)) * 8,
         "attend": kv + q + part + mask / 2,
@@ -142,6 +145,18 @@ class DecodeStack:
               buf.q_cur.data_ptr()] for buf, pool, ctr in zip(self.layers, self.q_pools, self.counters)],
             dtype=torch.int64, device=self.device)
         torch.cuda.synchronize(self.device)
+
+    def launches_per_layer_step(self) -> int:
+        """Kernels retro_decode_step enqueues per layer: select (S1 + S2) and attend (S3 + S4), or three where the
+        cache merge is its own launch (fp32 / more than 128 query rows per KV head)."""
+        return rb.retro_launches_per_step(self.desc)
+
+    def enqueue_step_part(self, part: int, stream=None):
+        """ONE of the step's kernels for every layer back to back (part 0: select, part 1: attend + merge), exactly
+        as retro_decode_step launches them (per-kernel timing of the real step; state stays valid for timing)."""
+        d = self.desc
+        for buf in self.layers:
+            rb.retro_decode_step_part(d, buf.state, buf.q_win, buf.q_pos, buf.q_cur, buf.out, part, None, stream)
 
     def enqueue_step(self, stream=None):
         """One decode step: advance every layer's synthetic query stream (one launch: the stand-in for the QKV

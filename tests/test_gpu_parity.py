@@ -397,29 +397,98 @@ def test_decode_step_host_end_to_end_matches_oracle():
     buf.seq_lens.copy_(torch.from_numpy(prompt.astype(np.int32)))
     buf.rebuild_bounds()
     dt = torch.bfloat16
-    dq = torch.empty((B, cfg.num_q_heads, cfg.head_dim), dtype=dt, device="cuda")
-    dk = torch.empty((B, cfg.num_kv_heads, cfg.head_dim), dtype=dt, device="cuda")
-    dv = torch.empty_like(dk)
-    io = rb.RetroStepIO(dq.data_ptr(), dk.data_ptr(), dv.data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(),
-                        buf.out.data_ptr())
-    hout = torch.empty((B, w + 1, cfg.num_q_heads, cfg.head_dim), dtype=dt).pin_memory()
+    hq_n, hk_n, D = cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim
+    n_q, n_kv = B * hq_n * D, B * hk_n * D
+    dqkv = torch.empty(n_q + 2 * n_kv, dtype=dt, device="cuda")
+    io = rb.RetroStepIO(dqkv.data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(), buf.out.data_ptr())
+    hqkv = torch.empty(n_q + 2 * n_kv, dtype=dt).pin_memory()       # [q_new | k_new | v_new], refilled every step
+    hout = torch.empty((B, w + 1, hq_n, D), dtype=dt).pin_memory()
     atol, rtol = GH.TOL[cfg.dtype]
     for s in range(12):
-        hq = inp.q_all[s].cpu().contiguous().pin_memory()
-        hk = torch.empty((B, cfg.num_kv_heads, cfg.head_dim), dtype=dt)
+        hqkv[:n_q] = inp.q_all[s].cpu().reshape(-1)
+        hk = torch.empty((B, hk_n, D), dtype=dt)
         hv = torch.empty_like(hk)
         for b in range(B):
             pos = cfg.prompt_lens[b] + s
             phys = int(inp.block_table[b, pos // P])
             hk[b], hv[b] = inp.k_pages[phys, :, pos % P].cpu(), inp.v_pages[phys, :, pos % P].cpu()
-        hk, hv = hk.pin_memory(), hv.pin_memory()
-        rb.retro_decode_step_host(desc, buf.state, io, hq, hk, hv, hout)
+        hqkv[n_q:n_q + n_kv] = hk.reshape(-1)
+        hqkv[n_q + n_kv:] = hv.reshape(-1)
+        rb.retro_decode_step_host(desc, buf.state, io, hqkv, hout)
         torch.cuda.synchronize()
         q_win, q_pos = wl.make_q_window(inp, s)
         res = layer.step(H.np64(q_win), q_pos.numpy(), H.np64(inp.q_all[s].cpu()), inp.seq_lens_at(s).cpu().numpy(),
                          np.full(B, cfg.budget_pages, dtype=np.int32))
         assert np.array_equal(buf.sel_pages.cpu().numpy(), res["sel_pages"])
         GH.close(hout.float().numpy(), res["out"], atol, rtol, f"e2e step {s} out")
+
+
+def test_decode_steps_host_two_layers_one_copy_each_way():
+    """retro_decode_steps_host: two layers (two independent device states of the same inputs) stepped with ONE
+    host->device and ONE device->host copy per step; both layers' outputs against the oracle, every step."""
+    cfg = wl.shrink(wl.c5(8, 512), (700, 655), 11, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    layers = [GH.make_device_layer(inp) for _ in range(2)]
+    desc = layers[0][0]
+    layer = H.oracle_layer(inp)
+    B, w, P = cfg.batch, cfg.window, cfg.page_size
+    hq_n, hk_n, D = cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim
+    prompt = np.asarray(cfg.prompt_lens)
+    layer.prefill_bounds(prompt)
+    for _, buf in layers:
+        buf.seq_lens.copy_(torch.from_numpy(prompt.astype(np.int32)))
+        buf.rebuild_bounds()
+    dt = torch.bfloat16
+    n_q, n_kv = B * hq_n * D, B * hk_n * D
+    tok = n_q + 2 * n_kv
+    d_in = torch.empty((2, tok), dtype=dt, device="cuda")
+    d_out = torch.empty((2, B, w + 1, hq_n, D), dtype=dt, device="cuda")
+    ios = [rb.RetroStepIO(d_in[l].data_ptr(), buf.q_win.data_ptr(), buf.q_pos.data_ptr(), d_out[l].data_ptr())
+           for l, (_, buf) in enumerate(layers)]
+    h_in = torch.empty((2, tok), dtype=dt).pin_memory()
+    h_out = torch.empty((2, B, w + 1, hq_n, D), dtype=dt).pin_memory()
+    atol, rtol = GH.TOL[cfg.dtype]
+    for s in range(11):
+        for l in range(2):
+            h_in[l, :n_q] = inp.q_all[s].reshape(-1)
+            for b in range(B):
+                pos = cfg.prompt_lens[b] + s
+                phys = int(inp.block_table[b, pos // P])
+                h_in[l, n_q + b * hk_n * D:n_q + (b + 1) * hk_n * D] = inp.k_pages[phys, :, pos % P].reshape(-1)
+                h_in[l, n_q + n_kv + b * hk_n * D:n_q + n_kv + (b + 1) * hk_n * D] = inp.v_pages[phys, :, pos % P].reshape(-1)
+        rb.retro_decode_steps_host(desc, [buf.state for _, buf in layers], ios, h_in, h_out)
+        torch.cuda.synchronize()
+        q_win, q_pos = wl.make_q_window(inp, s)
+        res = layer.step(H.np64(q_win), q_pos.numpy(), H.np64(inp.q_all[s]), inp.seq_lens_at(s).numpy(),
+                         np.full(B, cfg.budget_pages, dtype=np.int32))
+        for l in range(2):
+            assert np.array_equal(layers[l][1].sel_pages.cpu().numpy(), res["sel_pages"])
+            GH.close(h_out[l].float().numpy(), res["out"], atol, rtol, f"layers-host step {s} layer {l} out")
+
+
+def test_sequence_at_capacity_is_not_advanced():
+    """A sequence whose block-table row is full is left alone by the window-advance / append helpers (no write
+    past its last page, seq_len unchanged); the other sequences of the batch advance normally."""
+    cfg = wl.shrink(wl.c2(), (32, 20), 1, window=3, budget_tokens=32, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    cap = desc.max_pages_per_seq * cfg.page_size
+    buf.seq_lens.copy_(torch.tensor([cap, 21], dtype=torch.int32))
+    k_ref, v_ref = buf.k_pages.clone(), buf.v_pages.clone()
+    qpos_ref = buf.q_pos.clone()
+    q_new = inp.q_all[0].cuda().contiguous()
+    rb.retro_window_advance(desc, q_new, None, 1, buf.seq_lens, buf.q_win, buf.q_pos, buf.q_cur)
+    kn = torch.ones((2, cfg.num_kv_heads, cfg.head_dim), dtype=torch.bfloat16, device="cuda")
+    rb.retro_append_kv(desc, kn, kn, buf.block_table, buf.seq_lens, buf.k_pages, buf.v_pages)
+    torch.cuda.synchronize()
+    assert buf.seq_lens.cpu().tolist() == [cap, 22]
+    assert torch.equal(buf.q_pos[0], qpos_ref[0])
+    # sequence 0: (seq_len - 1) is its last valid slot and append rewrites it in place - nothing else moves
+    phys1 = int(inp.block_table[1, 21 // 16])
+    k_chk = buf.k_pages.clone(); k_chk[phys1, :, 21 % 16] = k_ref[phys1, :, 21 % 16]
+    phys0 = int(inp.block_table[0, (cap - 1) // 16])
+    k_chk[phys0, :, (cap - 1) % 16] = k_ref[phys0, :, (cap - 1) % 16]
+    assert torch.equal(k_chk, k_ref)
 
 
 def _to_cpu(inp):
