@@ -159,6 +159,8 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
     for (int l = 0; l < P; ++l) {
       kraw[l] = *reinterpret_cast<const Raw*>(kt + l * D + lane * kCh);
       vraw[l] = *reinterpret_cast<const Raw*>(vt + l * D + lane * kCh);
+      // slots past the sequence's last token are unwritten memory: their weight is 0, and 0 x NaN must not happen
+      if (j * P + l >= L) vraw[l] = Raw{};
     }
 #pragma unroll
     for (int i = 0; i < RPW; ++i) {

@@ -185,6 +185,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(8) uint64_t bars[24];
   __shared__ uint32_t tmem_ptr_s;
   __shared__ int s_flag[3];
+  __shared__ int s_fix[2];                       // (block, page slot) of the newest page if its tail is unwritten, else -1
   __shared__ unsigned int s_ticket;
   __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
   __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
@@ -203,6 +204,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   uint64_t* v_empty = bars + 9;          // [NV <= 3]
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
+  uint64_t* v_clean = bars + 18;         // [1] the unwritten tail rows of the newest page's V tile are zeroed
   uint64_t* o_full = bars + 16;          // [2] PV of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
@@ -223,6 +225,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
     mbar_init(&p_ready[0], kSoftmaxThreads / 32); mbar_init(&p_ready[1], kSoftmaxThreads / 32);
     mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
+    mbar_init(v_clean, 1);
     fence_mbar_init();
   }
   if (warp == 2) {
@@ -279,6 +282,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     if (my_pos_raw >= 0 && rank >= rk0 && rank < rk0 + nrk) s_rowr[rank - rk0] = tid;
   }
   if (tid < 3) s_flag[tid] = 0;
+  if (tid == 0) s_fix[0] = -1;
   __syncthreads();
 #pragma unroll
   for (int it = 0; it < kQIter; ++it) {
@@ -343,6 +347,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncthreads();               // block-table row (and the S4 prefetch) landed
   const int count = p.sel_count[unit];
+  const int beg0 = min(split * pps, count);
   for (int i = tid; i < pps; i += kUmmaThreads) {
     const int idx = split * pps + i;
     int j = 0, prev = 0;
@@ -355,6 +360,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     s_list[i] = j;
     s_list[pps + i] = prev;
     s_list[2 * pps + i] = phys;
+    // slots of the newest page past the sequence's last token are unwritten memory (possibly NaN / Inf): P is 0
+    // there, but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (below)
+    if (idx < count && j == (L - 1) / 16 && (L & 15) != 0) { s_fix[0] = (idx - beg0) / kPB; s_fix[1] = (idx - beg0) % kPB; }
   }
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
@@ -425,6 +433,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
         if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
         mbar_wait(&v_full[slot], n & 1);
+        if (blk == s_fix[0]) mbar_wait(v_clean, 0);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t v_addr = smem_u32(smem + lay.ring + (cfg.NK + slot) * kSlotBytes);
@@ -438,6 +447,21 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           tc_commit(&o_full[blk & 1]);
         }
         __syncwarp();
+      }
+    } else if (warp == 3) {
+      // ===== idle warp: zero the unwritten tail rows of the newest page's V tile (both 64-channel halves) =====
+      const int fb = s_fix[0];
+      if (fb >= 0) {
+        const int slot = fb % cfg.NV, pg = s_fix[1], nv = L & 15;
+        mbar_wait(&v_full[slot], (fb / cfg.NV) & 1);
+        unsigned char* vt = smem + lay.ring + (cfg.NK + slot) * kSlotBytes + pg * kTileHalfBytes;
+        for (int i = lane; i < (16 - nv) * 8; i += 32) {             // 16-byte chunks of rows nv..15 (a row is 128 B per half)
+          *reinterpret_cast<uint4*>(vt + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
+          *reinterpret_cast<uint4*>(vt + kHalfStride + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(v_clean);
       }
     } else if (warp >= 4) {
       // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NC = NT / 4 columns (rows) each =====

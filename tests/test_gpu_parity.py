@@ -189,6 +189,28 @@ def test_select_adversarial_near_ties_are_ranked_exactly(base):
     GH.lockstep(inp, 3, use_decode_step=True)
 
 
+@pytest.mark.parametrize("base", ["f32", "bf16"])
+def test_unwritten_tail_of_newest_page_may_hold_nan_and_inf(base):
+    """Slots of the newest page past the last token are unwritten memory in a real paged cache: K there is NaN, V is
+    +-Inf / NaN.  Nothing of it may reach a result (the masked weights are 0, and 0 x NaN must never be formed)."""
+    if base == "f32":
+        cfg = wl.shrink(wl.c1(), (505,), 3)
+    else:
+        cfg = wl.shrink(wl.c2(), (1003, 771), 3, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    P = cfg.page_size
+    for b in range(cfg.batch):
+        total = cfg.prompt_lens[b] + cfg.n_steps
+        assert total % P != 0
+        phys = int(inp.block_table[b, total // P])
+        inp.k_pages[phys, :, total % P:] = float("nan")
+        inp.v_pages[phys, :, total % P:] = float("inf")
+        inp.v_pages[phys, :, total % P:, ::2] = float("nan")
+        inp.v_pages[phys, :, total % P + 1:, 1::4] = float("-inf")
+    print("nan tail errs", base, GH.lockstep(inp, 3))
+    GH.lockstep(inp, 3, use_decode_step=True)
+
+
 def test_c2_full_context_sampled_steps():
     """FULL C2 context (32768-token prompt), the launch configuration bench.py times; first steps + ramp-up."""
     cfg = wl.c2(n_steps=12)
