@@ -178,6 +178,17 @@ int retro_decode_step_part(const retro_desc_t* desc, const retro_layer_state_t* 
                            void* stream);
 int retro_launches_per_step(const retro_desc_t* desc /*HOST*/, int32_t* launches /*HOST out*/);
 
+/* Debug build.  Compiled with -DRETRO_DEBUG_CHECKS (paper_2508_09001_b200/lib/libretro_dbg.so) the kernels validate
+ * the caller-supplied indices on the device - sel_pages entries against the sequence's page count, block_table entries
+ * against num_phys_pages, sel_count, seq_lens, budget_pages, q_pos - count the violations in the workspace, and
+ * neutralise the offending entry (an invalid page is treated as already seen by every row) instead of reading out
+ * of bounds.  retro_debug_status reports enabled (0 in the release build, where the counts read 0 and nothing is
+ * synchronised), the violations since retro_workspace_init and the code of the last one (1 sel_pages, 2 block_table,
+ * 3 q_pos, 4 seq_lens, 5 budget_pages, 6 sel_count).  enabled / violations / last_code: HOST out.  In the debug build
+ * this call SYNCHRONISES `stream` (the one exception to the conventions above). */
+int retro_debug_status(const retro_desc_t* desc, const void* workspace, size_t ws_bytes, int32_t* enabled /*HOST*/,
+                       uint32_t* violations /*HOST*/, uint32_t* last_code /*HOST*/, void* stream);
+
 /* End-to-end step with HOST buffers (pinned for async copies): ONE host->device copy of this step's packed
  * inputs host_qkv_new = [q_new [B][h_q][d] | k_new [B][h_k][d] | v_new [B][h_k][d]] (T), one launch that advances
  * seq_lens and the query window ring and appends the token to the KV pool, retro_decode_step, and ONE device->host

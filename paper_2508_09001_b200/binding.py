@@ -25,7 +25,7 @@ EXPORTED = [
     "retro_merge_output_cache", "retro_append_kv", "retro_decode_step", "retro_decode_step_host",
     "retro_window_advance", "retro_window_advance_layers", "retro_update_kv",
     "retro_budget_policy", "retro_build_mask", "retro_step_diagnostics", "retro_decode_step_part",
-    "retro_launches_per_step", "retro_decode_steps_host",
+    "retro_launches_per_step", "retro_decode_steps_host", "retro_debug_status",
 ]
 
 
@@ -63,12 +63,15 @@ class RetroError(RuntimeError):
 
 
 _LIB = None
+_LIB_PATH = None     # None: the release build (paper_2508_09001_b200/lib/libretro.so)
 
 
 def _lib():
     global _LIB
     if _LIB is None:
-        path = _build.build()          # no-op when up to date; raises if nvcc fails
+        global _LIB_PATH
+        path = _LIB_PATH if _LIB_PATH is not None else _build.build()   # no-op when up to date; raises if nvcc fails
+        _LIB_PATH = path
         lib = C.CDLL(path)
         lib.retro_error_string.restype = C.c_char_p
         lib.retro_error_string.argtypes = [C.c_int]
@@ -80,7 +83,23 @@ def _lib():
 
 def library_path() -> str:
     _lib()
-    return _build.LIB_PATH
+    return _LIB_PATH
+
+
+def use_library(path: Optional[str] = None):
+    """Load another build of the library (e.g. build.build_debug(): device-side index validation); None = the
+    release build.  Affects every later call of this module."""
+    global _LIB, _LIB_PATH
+    _LIB, _LIB_PATH = None, path
+    _lib()
+
+
+def retro_debug_status(desc, workspace, stream=None):
+    """(enabled, violations, last_code) of a -DRETRO_DEBUG_CHECKS build; (0, 0, 0) in the release build."""
+    en, n, code = C.c_int32(0), C.c_uint32(0), C.c_uint32(0)
+    _check(_lib().retro_debug_status(C.byref(desc), _p(workspace), C.c_size_t(workspace.numel()), C.byref(en),
+                                     C.byref(n), C.byref(code), _stream(stream)), "retro_debug_status")
+    return en.value, n.value, code.value
 
 
 def _p(t: Optional[torch.Tensor]):

@@ -13,6 +13,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB_DIR = os.path.join(PKG, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libretro.so")
+DBG_LIB_PATH = os.path.join(LIB_DIR, "libretro_dbg.so")
 INCLUDE = os.path.join(os.path.dirname(PKG), "include")
 
 
@@ -21,29 +22,37 @@ def sources():
     return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cu"))
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB_PATH):
+def _stale(lib_path: str = None) -> bool:
+    lib_path = lib_path or LIB_PATH
+    if not os.path.exists(lib_path):
         return True
-    t = os.path.getmtime(LIB_PATH)
+    t = os.path.getmtime(lib_path)
     deps = sources() + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")]
     deps.append(os.path.join(INCLUDE, "retro.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return LIB_PATH
+def build_debug(force: bool = False) -> str:
+    """The same library with -DRETRO_DEBUG_CHECKS (device-side index validation) -> lib/libretro_dbg.so."""
+    return build(force=force, lib_path=DBG_LIB_PATH, extra_flags=["-DRETRO_DEBUG_CHECKS"], obj_suffix=".dbg.o")
+
+
+def build(force: bool = False, verbose: bool = False, lib_path: str = LIB_PATH, extra_flags=(),
+          obj_suffix: str = ".o") -> str:
+    if not force and not _stale(lib_path):
+        return lib_path
     os.makedirs(LIB_DIR, exist_ok=True)
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
     for src in sources():
-        obj = os.path.join(LIB_DIR, os.path.basename(src)[:-3] + ".o")
+        obj = os.path.join(LIB_DIR, os.path.basename(src)[:-3] + obj_suffix)
         cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
                "-Xcompiler", "-fPIC", "-I", INCLUDE, "-c", src, "-o", obj]
         if verbose:
             cmd += ["-Xptxas", "-v"]
-        cmd += os.environ.get("RETRO_NVCC_FLAGS", "").split()     # e.g. -DRETRO_STAMPS (debug timestamps)
+        cmd += list(extra_flags)
+        cmd += os.environ.get("RETRO_NVCC_FLAGS", "").split()     # extra nvcc flags for experiments
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     failed = False
@@ -54,13 +63,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
         failed |= pr.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed building libretro.so")
-    link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB_PATH] + objs
+    link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib_path] + objs
     r = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:
         sys.stderr.write(r.stdout)
         raise RuntimeError("nvcc link failed for libretro.so")
-    return LIB_PATH
+    return lib_path
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--debug" in sys.argv:
+        print(build_debug(force="--force" in sys.argv))

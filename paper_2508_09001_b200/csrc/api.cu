@@ -154,6 +154,8 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d) {
   off = align_up(off + (size_t)units * wl.nsplit * wl.rows * d->head_dim * sizeof(float), 256);
   wl.split_lse_off = off;
   off = align_up(off + (size_t)units * wl.nsplit * wl.rows * sizeof(float), 256);
+  wl.debug_off = off;     // (zeroed by retro_workspace_init together with the counters after it)
+  off = align_up(off + 2 * sizeof(unsigned int), 256);
   wl.counters_off = off;
   off = align_up(off + (size_t)4 * units * sizeof(unsigned int), 256);
   wl.slot_counters_off = off;   // (zeroed by retro_workspace_init together with the counters before it)
@@ -203,7 +205,7 @@ int retro_workspace_init(const retro_desc_t* desc, void* workspace, size_t ws_by
   RETRO_CHECK_PTR(workspace);
   const WorkspaceLayout wl = workspace_layout(desc);
   if (ws_bytes < wl.total) return RETRO_ERR_WORKSPACE;
-  RETRO_CUDA_TRY(cudaMemsetAsync(static_cast<char*>(workspace) + wl.counters_off, 0, wl.total - wl.counters_off,
+  RETRO_CUDA_TRY(cudaMemsetAsync(static_cast<char*>(workspace) + wl.debug_off, 0, wl.total - wl.debug_off,
                                  (cudaStream_t)stream));
   return RETRO_OK;
 }
@@ -385,6 +387,28 @@ int retro_decode_step_part(const retro_desc_t* desc, const retro_layer_state_t* 
                            void* stream) {
   if (part != 0 && part != 1) return RETRO_ERR_ARG;
   return decode_step_parts(desc, st, q_win, q_pos, q_cur, out, out_lse, 1 << part, stream);
+}
+
+int retro_debug_status(const retro_desc_t* desc, const void* workspace, size_t ws_bytes, int32_t* enabled,
+                       uint32_t* violations, uint32_t* last_code, void* stream) {
+  RETRO_CHECK_DESC(desc);
+  RETRO_CHECK_PTR(workspace);
+  if (enabled == nullptr || violations == nullptr || last_code == nullptr) return RETRO_ERR_ARG;
+  const WorkspaceLayout wl = workspace_layout(desc);
+  if (ws_bytes < wl.total) return RETRO_ERR_WORKSPACE;
+  *violations = 0; *last_code = 0;
+#ifdef RETRO_DEBUG_CHECKS
+  *enabled = 1;
+  unsigned int host[2] = {0, 0};
+  RETRO_CUDA_TRY(cudaMemcpyAsync(host, static_cast<const char*>(workspace) + wl.debug_off, sizeof(host),
+                                 cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  RETRO_CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+  *violations = host[0]; *last_code = host[1];
+#else
+  *enabled = 0;
+  (void)stream;
+#endif
+  return RETRO_OK;
 }
 
 int retro_launches_per_step(const retro_desc_t* desc, int32_t* launches) {

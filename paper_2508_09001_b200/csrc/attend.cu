@@ -91,7 +91,9 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
   const int L = p.seq_lens[b];
   const int t = L - 1;
   const size_t unit = (size_t)b * p.h_k + h;
-  const int count = p.sel_count[unit];
+  int count = p.sel_count[unit];
+  RETRO_DBG_ONLY(if (count < 0 || count > p.k_max) { if (tid == 0) dbg_violation(p.dbg, kDbgSelCount); count = 0; })
+  RETRO_DBG_ONLY(if (L < 0 || L > p.max_pages * P) { if (tid == 0) dbg_violation(p.dbg, kDbgSeqLen); count = 0; })
   const int beg = min(split * p.pages_per_split, count);
   const int end = min(beg + p.pages_per_split, count);
   const int n_my = end - beg;
@@ -101,10 +103,14 @@ __global__ void __launch_bounds__(kAttWarps * 32) attend_simt_kernel(const Atten
     fence_mbar_init();
   }
   for (int i = tid; i < n_my; i += blockDim.x) {
-    const int j = p.sel_pages[unit * p.k_max + beg + i];
+    int j = p.sel_pages[unit * p.k_max + beg + i];
+    int prev = p.sel_prev[unit * p.k_max + beg + i];
+    RETRO_DBG_ONLY(if (j < 0 || j >= min((L + P - 1) / P, p.max_pages)) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
+    int phys = p.block_table[(size_t)b * p.max_pages + j];
+    RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
     s_list[i] = j;
-    s_list[p.pages_per_split + i] = p.sel_prev[unit * p.k_max + beg + i];
-    s_list[2 * p.pages_per_split + i] = p.block_table[(size_t)b * p.max_pages + j];
+    s_list[p.pages_per_split + i] = prev;
+    s_list[2 * p.pages_per_split + i] = phys;
   }
   // q rows of this KV head: row rho = r*G + g  <-  q_win[b][r][h*G+g][:]
   {
@@ -288,6 +294,8 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
   prm.fused = 0;
   prm.cache_o = nullptr; prm.cache_lse = nullptr; prm.cache_pos = nullptr; prm.out = nullptr; prm.out_lse = nullptr;
   prm.seq_counters = reinterpret_cast<unsigned int*>(ws + wl.slot_counters_off);   // [B]
+  prm.dbg = reinterpret_cast<unsigned int*>(ws + wl.debug_off);
+  prm.num_phys = d->num_phys_pages;
   if (d->dtype == RETRO_BF16) {
     // bf16: the rows x keys block is a dense contraction -> tcgen05 tensor cores (attend_umma.cu; more than 128
     // rows run as row groups)

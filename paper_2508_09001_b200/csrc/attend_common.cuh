@@ -19,6 +19,7 @@ struct AttendParams {
   // tensor-core path inside retro_decode_step (fused = 1, nrg == 1): S4 runs in the same kernel
   int fused;
   float* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse; unsigned int* seq_counters;
+  unsigned int* dbg; int num_phys;   // -DRETRO_DEBUG_CHECKS: violation counter in the workspace, pool size
 };
 
 #ifdef __CUDACC__

@@ -186,7 +186,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ uint32_t tmem_ptr_s;
   __shared__ int s_flag[3];
   __shared__ int s_fix[2];                       // (block, page slot) of the newest page if its tail is unwritten, else -1
-  __shared__ unsigned int s_ticket;
   __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
   __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
   __shared__ int s_cpos[kMaxWindow + 1];         // cache_pos of the sequence as this kernel found it
@@ -346,7 +345,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   }
   asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncthreads();               // block-table row (and the S4 prefetch) landed
-  const int count = p.sel_count[unit];
+  int count = p.sel_count[unit];
+  RETRO_DBG_ONLY(if (count < 0 || count > p.k_max) { if (tid == 0) dbg_violation(p.dbg, kDbgSelCount); count = 0; })
+  RETRO_DBG_ONLY(if (L < 0 || L > p.max_pages * 16) { if (tid == 0) dbg_violation(p.dbg, kDbgSeqLen); count = 0; })
+  RETRO_DBG_ONLY(if (tid < R && my_pos_raw > L - 1) dbg_violation(p.dbg, kDbgQPos);)
   const int beg0 = min(split * pps, count);
   for (int i = tid; i < pps; i += kUmmaThreads) {
     const int idx = split * pps + i;
@@ -355,8 +357,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       j = p.sel_pages[unit * p.k_max + idx];
       prev = p.sel_prev[unit * p.k_max + idx];
     }
+    RETRO_DBG_ONLY(if (idx < count && (j < 0 || j >= min((L + 15) / 16, p.max_pages))) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
     int phys = 0;
     if (idx < count) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
+    RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
     s_list[i] = j;
     s_list[pps + i] = prev;
     s_list[2 * pps + i] = phys;

@@ -62,6 +62,7 @@ struct WorkspaceLayout {
   size_t split_o_off;   // float  [B][h_k][nsplit][rows][d]
   size_t split_lse_off; // float  [B][h_k][nsplit][rows]
   size_t slot_counters_off;  // uint32 [B][w+1]: arrivals per (sequence, cache slot) of the combine + merge kernel
+  size_t debug_off;     // uint32 [2]: violations counted by a -DRETRO_DEBUG_CHECKS build, code of the last one
   size_t counters_off;  // uint32 [4][B][h_k]: score-chunk counters first, then split arrival counters per row group
   size_t total;
   int nsplit;           // split-KV factor of the attend kernel
@@ -115,7 +116,26 @@ int launch_window_advance_layers(const retro_desc_t* d, const retro_advance_rec_
 int launch_window_advance(const retro_desc_t* d, const void* q_new_or_pool, int32_t* step_counter, int pool_steps,
                           int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out, cudaStream_t s);
 
+// Codes a -DRETRO_DEBUG_CHECKS build records next to its violation count (retro_debug_status)
+enum : unsigned int {
+  kDbgSelPage = 1,      // sel_pages entry outside [0, #pages of the sequence)
+  kDbgPhysPage = 2,     // block_table entry outside [0, num_phys_pages)
+  kDbgQPos = 3,         // q_pos entry above the current position
+  kDbgSeqLen = 4,       // seq_lens entry outside [0, max_pages_per_seq * page_size]
+  kDbgBudget = 5,       // negative budget_pages entry
+  kDbgSelCount = 6,     // sel_count entry outside [0, max_sel_pages]
+};
+
 #ifdef __CUDACC__
+#ifdef RETRO_DEBUG_CHECKS
+#define RETRO_DBG_ONLY(...) __VA_ARGS__
+__device__ __forceinline__ void dbg_violation(unsigned int* dbg, unsigned int code) {
+  atomicAdd(dbg, 1u);
+  dbg[1] = code;
+}
+#else
+#define RETRO_DBG_ONLY(...)
+#endif
 // ---- programmatic dependent launch ---------------------------------------------------------------
 // Every libretro kernel is launched with the programmatic-stream-serialization attribute, waits for the
 // COMPLETION of its predecessor (pdl_wait) before it touches global memory and then lets its own dependent

@@ -284,6 +284,7 @@ struct SelectParams {
   double* scores_out;            // optional fp64 scores (tests)
   unsigned long long* amb_keys;  // workspace [units][max_pages]: fp64 keys of the undecided pages (exact refinement)
   int32_t* amb_idx;              // workspace [units][max_pages]
+  unsigned int* dbg;             // -DRETRO_DEBUG_CHECKS: violation counter in the workspace
   int h_q, h_k, max_pages, k_max, P, force_last, pages_per_cta;
   int prefetch_a;                // the leader stages the unit's row of A in shared memory
   // S1 in line (retro_decode_step): the warp that owns the newest page recomputes its digest from the K tile,
@@ -331,8 +332,10 @@ __global__ void __launch_bounds__(kSelThreads, 2) select_pages_kernel(const Sele
     for (int g = 0; g < kMaxGroup; ++g)
       if (g < G) q_raw[g] = q_cur[((size_t)b * p.h_q + h * G + g) * D + c];
   }
-  const int budget_b = p.budget_pages[b];     // only the leader needs it: fetched with the first round trip
-  const int seq_len_b = p.seq_lens[b];
+  int budget_b = p.budget_pages[b];           // only the leader needs it: fetched with the first round trip
+  int seq_len_b = p.seq_lens[b];
+  RETRO_DBG_ONLY(if (seq_len_b < 0 || seq_len_b > p.max_pages * p.P) { if (tid == 0 && rank == 0) dbg_violation(p.dbg, kDbgSeqLen); seq_len_b = 0; })
+  RETRO_DBG_ONLY(if (budget_b < 0) { if (tid == 0 && rank == 0) dbg_violation(p.dbg, kDbgBudget); budget_b = 0; })
   const int n_pages = min((seq_len_b + p.P - 1) / p.P, p.max_pages);   // a sequence never outgrows its block-table row
   const int cta_page0 = (int)rank * p.pages_per_cta;
   const int page_end = min(cta_page0 + p.pages_per_cta, n_pages);
@@ -605,6 +608,7 @@ int launch_select_pages(const retro_desc_t* d, const WorkspaceLayout& wl, const 
   prm.k_max = d->max_sel_pages; prm.P = d->page_size; prm.force_last = d->force_last_page;
   prm.pages_per_cta = 0;
   prm.prefetch_a = 0;
+  prm.dbg = reinterpret_cast<unsigned int*>(ws + wl.debug_off);
   prm.k_pages = k_pages_refresh; prm.block_table = block_table; prm.bounds_out = const_cast<void*>(bounds);
   const DeviceInfo di = device_info();
   const int units = d->batch * d->num_kv_heads;
