@@ -44,6 +44,7 @@ constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][1
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
 constexpr int kTmemCols = 512;
 constexpr int kUmmaSmemBudget = 232448 - 1024 - 4096;   // dynamic shared memory the launcher plans with (one CTA per SM)
+constexpr int kMaxBlocks = 256;                // key blocks per CTA (2048 pages per split)
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
 constexpr float kRescaleThreshold = 64.f;     // log2 units: P <= 2^64, sums stay far below the fp32 / bf16 range
 constexpr float kMrefInit = -1.0e30f;         // finite "row not started" reference: -inf - kMrefInit stays -inf
@@ -154,7 +155,8 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
   UmmaLayout L;
   const int natom = (2 * NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
-  L.p = L.q + 2 * NT * 128;                  // [buf][atom][128 keys][128 B = 64 columns]; columns = hi rows | lo rows
+  L.p = L.q + 2 * NT * 128;                  // [buf][atom][128 keys][128 B = 64 columns]; columns: per 16-row chunk
+                                             // its 16 hi values then its 16 lo values
   L.p_hl_bytes = 0;
   L.p_buf_bytes = natom * 16384;
   L.ring = L.p + NP * L.p_buf_bytes;
@@ -185,6 +187,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(8) uint64_t bars[24];
   __shared__ uint32_t tmem_ptr_s;
   __shared__ int s_flag[3];
+  __shared__ int s_nlive[kMaxBlocks];            // live 16-row chunks of every key block of this CTA (non-increasing)
   __shared__ int s_fix[2];                       // (block, page slot) of the newest page if its tail is unwritten, else -1
   __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
   __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
@@ -368,6 +371,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     // there, but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (below)
     if (idx < count && j == (L - 1) / 16 && (L & 15) != 0) { s_fix[0] = (idx - beg0) / kPB; s_fix[1] = (idx - beg0) % kPB; }
   }
+  for (int i = tid; i < kMaxBlocks; i += kUmmaThreads) s_nlive[i] = NCH;
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
   const int n_my = end - beg;
@@ -405,8 +409,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     } else if (warp == 2) {
       // ===== MMA issuer: the whole warp walks the loop (waits), one elected lane issues =====
       const uint32_t q_addr = smem_u32(smem + lay.q);
-      const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
-      const uint32_t idesc_o = idesc_bf16_ab(2 * NT, true, true);
+      // N follows the block's live 16-row chunks: rows are rank-major (newest first) and a page is visible to a
+      // PREFIX of the ranks, so the rows a block can contribute to are the first 16 * nl (S) / 32 * nl (P, O) columns
       auto issue_s = [&](int blk) {
         const int slot = blk % cfg.NK, n = blk / cfg.NK;
         mbar_wait(&k_full[slot], n & 1);
@@ -418,7 +422,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           for (int ks = 0; ks < 8; ++ks) {    // K = 128 channels = 8 steps of 16; 4 steps per 64-channel half
             const uint32_t koff = (ks >> 2) * kHalfStride + (ks & 3) * 32;
             const uint32_t qoff = (ks >> 2) * (NT * 128) + (ks & 3) * 32;
-            umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff), idesc_s, ks > 0);
+            umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff),
+                      idesc_bf16_ab(16 * s_nlive[blk], false, false), ks > 0);
           }
           tc_commit(&k_empty[slot]);
           tc_commit(&s_full[blk % cfg.NSB]);
@@ -445,7 +450,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
             const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
             const uint64_t pdesc = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
-            umma_bf16(tmem_base + colO, vdesc, pdesc, idesc_o, (blk > 0 || ks > 0) ? 1u : 0u);
+            umma_bf16(tmem_base + colO, vdesc, pdesc, idesc_bf16_ab(32 * s_nlive[blk], true, true),
+                      (blk > 0 || ks > 0) ? 1u : 0u);
           }
           tc_commit(&v_empty[slot]);
           tc_commit(&o_full[blk & 1]);
@@ -473,9 +479,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       const int quadrant = warp & 3;                      // TMEM lanes a warp may touch: 32*(warp%4)..+31
       const int cg = sw >> 2;                             // column group
       const int key = quadrant * 32 + lane;
-      const int cbeg = cg * NC;
+      const int c4 = 4 * cg;                              // the thread's columns of 16-row chunk i: 16 i + c4 .. + 3
       const int st = tid - 128;                           // 0..511
       const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
+      const int nl0 = s_nlive[0];                         // the first block has the most live chunks
       float l_acc[NC];                                    // this key-thread's share of the row sums
 #pragma unroll
       for (int j = 0; j < NC; ++j) l_acc[j] = 0.f;
@@ -490,26 +497,30 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         if (st == 0) s_flag[(blk + 1) % 3] = 0;
         mbar_wait(&s_full[blk % cfg.NSB], (blk / cfg.NSB) & 1);
         tc_fence_after();
-        const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
+        const int nl = s_nlive[blk];                        // live 16-row chunks of this block (block-uniform)
+        const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + c4;
         // d = s * scale - m_ref (log2 units), -inf where masked; the common block needs nothing else
         float d[NC];
         float tmax = -INFINITY;
         {
           uint32_t raw[NC];
 #pragma unroll
-          for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
+          for (int i = 0; i < NCH; ++i)
+            if (i < nl) tmem_ld4(s_addr + 16 * i, raw + 4 * i);
           tmem_wait_ld();
 #pragma unroll
           for (int i = 0; i < NCH; ++i) {
-            const int4 ps = *reinterpret_cast<const int4*>(s_colpos + cbeg + 4 * i);
-            const float4 mr = *reinterpret_cast<const float4*>(s_mref + cbeg + 4 * i);
-            const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
-            const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
+            if (i < nl) {
+              const int4 ps = *reinterpret_cast<const int4*>(s_colpos + 16 * i + c4);
+              const float4 mr = *reinterpret_cast<const float4*>(s_mref + 16 * i + c4);
+              const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
+              const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-              const float v = fmaf(__uint_as_float(raw[4 * i + u]), p.scale_log2, -mv[u]);
-              d[4 * i + u] = pv[u] > thr ? v : -INFINITY;
-              tmax = fmaxf(tmax, d[4 * i + u]);
+              for (int u = 0; u < 4; ++u) {
+                const float v = fmaf(__uint_as_float(raw[4 * i + u]), p.scale_log2, -mv[u]);
+                d[4 * i + u] = pv[u] > thr ? v : -INFINITY;
+                tmax = fmaxf(tmax, d[4 * i + u]);
+              }
             }
           }
         }
@@ -521,16 +532,20 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           {
             uint32_t raw[NC];
 #pragma unroll
-            for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
+            for (int i = 0; i < NCH; ++i)
+              if (i < nl) tmem_ld4(s_addr + 16 * i, raw + 4 * i);
             tmem_wait_ld();
 #pragma unroll
             for (int j = 0; j < NC; ++j)
-              xs[j] = s_colpos[cbeg + j] > thr ? __uint_as_float(raw[j]) * p.scale_log2 : -INFINITY;
+              if ((j >> 2) < nl)
+                xs[j] = s_colpos[16 * (j >> 2) + c4 + (j & 3)] > thr ? __uint_as_float(raw[j]) * p.scale_log2 : -INFINITY;
           }
 #pragma unroll
           for (int j = 0; j < NC; ++j) {
-            const int r = __reduce_max_sync(0xffffffffu, f2o(xs[j]));
-            if (lane == 0) atomicMax(&s_colmax[cbeg + j], r);
+            if ((j >> 2) < nl) {
+              const int r = __reduce_max_sync(0xffffffffu, f2o(xs[j]));
+              if (lane == 0) atomicMax(&s_colmax[16 * (j >> 2) + c4 + (j & 3)], r);
+            }
           }
           softmax_bar();
           if (st < NT) {
@@ -542,28 +557,30 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           }
           softmax_bar();
 #pragma unroll
-          for (int j = 0; j < NC; ++j) {
-            l_acc[j] *= s_alpha[cbeg + j];
-            d[j] = xs[j] - s_mref[cbeg + j];
+          for (int j = 0; j < NC; ++j) {                   // (alpha is 1 for the rows of dead chunks)
+            const int c = 16 * (j >> 2) + c4 + (j & 3);
+            l_acc[j] *= s_alpha[c];
+            if ((j >> 2) < nl) d[j] = xs[j] - s_mref[c];
           }
           if (blk > 0) {
             mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O is ours
             tc_fence_after();
 #pragma unroll
             for (int i = 0; i < NCH; ++i) {                  // this thread's columns of O_hi and O_lo
-              const float4 al4 = *reinterpret_cast<const float4*>(s_alpha + cbeg + 4 * i);
+              if (i >= nl0) continue;                        // chunks no block has touched yet hold nothing
+              const float4 al4 = *reinterpret_cast<const float4*>(s_alpha + 16 * i + c4);
               const float al[4] = {al4.x, al4.y, al4.z, al4.w};
               uint32_t oh[4], ol[4];
-              tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
-              tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
+              tmem_ld4(lane_addr + colO + 32 * i + c4, oh);
+              tmem_ld4(lane_addr + colO + 32 * i + 16 + c4, ol);
               tmem_wait_ld();
 #pragma unroll
               for (int u = 0; u < 4; ++u) {
                 oh[u] = __float_as_uint(__uint_as_float(oh[u]) * al[u]);
                 ol[u] = __float_as_uint(__uint_as_float(ol[u]) * al[u]);
               }
-              tmem_st4(lane_addr + colO + cbeg + 4 * i, oh);
-              tmem_st4(lane_addr + colO + NT + cbeg + 4 * i, ol);
+              tmem_st4(lane_addr + colO + 32 * i + c4, oh);
+              tmem_st4(lane_addr + colO + 32 * i + 16 + c4, ol);
             }
             tmem_wait_st();
           }
@@ -573,13 +590,14 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
+          if (i >= nl) continue;
           float e[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             e[u] = ex2_approx(d[4 * i + u]);
             l_acc[4 * i + u] += e[u];
           }
-          const int c_hi = cbeg + 4 * i, c_lo = NT + c_hi;
+          const int c_hi = 32 * i + c4, c_lo = c_hi + 16;   // operand columns: chunk i = [16 hi rows | 16 lo rows]
           uint2 hi, lo;
           split_bf16x2(e[0], e[1], hi.x, lo.x);
           split_bf16x2(e[2], e[3], hi.y, lo.y);
@@ -609,7 +627,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           v += __shfl_xor_sync(0xffffffffu, v, 4);
           v += __shfl_xor_sync(0xffffffffu, v, 2);
           v += __shfl_xor_sync(0xffffffffu, v, 1);
-          if ((lane & 7) == 0) atomicAdd(&s_L[cbeg + ((lane >> 3) & 3) * NCH + i], v);
+          const int k = ((lane >> 3) & 3) * NCH + i;        // index into l_acc = 4 * chunk + u
+          if ((lane & 7) == 0) atomicAdd(&s_L[16 * (k >> 2) + c4 + (k & 3)], v);
         }
       }
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
@@ -622,14 +641,16 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       __half* stage = reinterpret_cast<__half*>(smem + lay.ring);
 #pragma unroll
       for (int i = 0; i < NCH; ++i) {
-        if (cbeg + 4 * i < rows_cta) {                      // warp-uniform
-          uint32_t oh[4], ol[4];
-          tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
-          tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
-          tmem_wait_ld();
+        if (16 * i + c4 < rows_cta) {                       // warp-uniform
+          uint32_t oh[4] = {0u, 0u, 0u, 0u}, ol[4] = {0u, 0u, 0u, 0u};
+          if (i < nl0) {                                    // (chunks no block touched: L is 0, the row reads empty)
+            tmem_ld4(lane_addr + colO + 32 * i + c4, oh);
+            tmem_ld4(lane_addr + colO + 32 * i + 16 + c4, ol);
+            tmem_wait_ld();
+          }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int c = cbeg + 4 * i + u;
+            const int c = 16 * i + c4 + u;
             if (c < rows_cta) {
               const float l = s_L[c];
               const float inv = rcp_approx(l);
