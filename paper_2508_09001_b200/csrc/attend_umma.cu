@@ -207,6 +207,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
   uint64_t* v_clean = bars + 18;         // [1] the unwritten tail rows of the newest page's V tile are zeroed
+  uint64_t* v_landed = bars + 19;        // [1] the V block that holds that tile has landed (single use: a parity
+                                         // wait on the ring's own barrier would alias with earlier fills of the slot)
   uint64_t* o_full = bars + 16;          // [2] PV of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
@@ -227,7 +229,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
     mbar_init(&p_ready[0], kSoftmaxThreads / 32); mbar_init(&p_ready[1], kSoftmaxThreads / 32);
     mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
-    mbar_init(v_clean, 1);
+    mbar_init(v_clean, 1); mbar_init(v_landed, 1);
     fence_mbar_init();
   }
   if (warp == 2) {
@@ -352,30 +354,96 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   RETRO_DBG_ONLY(if (count < 0 || count > p.k_max) { if (tid == 0) dbg_violation(p.dbg, kDbgSelCount); count = 0; })
   RETRO_DBG_ONLY(if (L < 0 || L > p.max_pages * 16) { if (tid == 0) dbg_violation(p.dbg, kDbgSeqLen); count = 0; })
   RETRO_DBG_ONLY(if (tid < R && my_pos_raw > L - 1) dbg_violation(p.dbg, kDbgQPos);)
-  const int beg0 = min(split * pps, count);
-  for (int i = tid; i < pps; i += kUmmaThreads) {
-    const int idx = split * pps + i;
-    int j = 0, prev = 0;
-    if (idx < p.k_max) {
-      j = p.sel_pages[unit * p.k_max + idx];
-      prev = p.sel_prev[unit * p.k_max + idx];
-    }
-    RETRO_DBG_ONLY(if (idx < count && (j < 0 || j >= min((L + 15) / 16, p.max_pages))) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
-    int phys = 0;
-    if (idx < count) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
-    RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
-    s_list[i] = j;
-    s_list[pps + i] = prev;
-    s_list[2 * pps + i] = phys;
-    // slots of the newest page past the sequence's last token are unwritten memory (possibly NaN / Inf): P is 0
-    // there, but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (below)
-    if (idx < count && j == (L - 1) / 16 && (L & 15) != 0) { s_fix[0] = (idx - beg0) / kPB; s_fix[1] = (idx - beg0) % kPB; }
-  }
-  for (int i = tid; i < kMaxBlocks; i += kUmmaThreads) s_nlive[i] = NCH;
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
-  const int n_my = end - beg;
-  const int nblk = (n_my + kPB - 1) / kPB;
+  const int n_all = end - beg;                   // selected pages of this split
+  // Mask-aware order.  A page with previous load position `prev` is visible to the window ranks r < t - prev only
+  // (Eq. 2: a past query attends the pages it has NOT seen), i.e. to a PREFIX of the rank-major rows; cls = how
+  // many of this CTA's ranks see it.  The split's pages are sorted by cls, most first (stable counting sort), so
+  // that a key block needs only its first 16 * nl rows and whole trailing blocks nobody of this row group sees
+  // (cls 0) are never loaded.  Pages seen by every live past query (the ~83 % that repeat from the previous step,
+  // PAPER.md:349) cost the current query's rows only.
+  auto cls_of = [&](int prev) { return max(0, min(t - prev - rk0, nrk)); };
+  {
+    int32_t* tmp = reinterpret_cast<int32_t*>(smem + lay.ring);   // the K / V ring is idle until the producers start
+    int32_t* cnt = tmp + 3 * pps;                                  // [chunks of 32 entries + 1][classes 0 .. w + 1] counts
+    constexpr int kCls = kMaxWindow + 2;
+    const bool sorted = n_all > kPB;
+    const int nchunk = (n_all + 31) / 32;
+    if (sorted)
+      for (int i = tid; i < nchunk * kCls; i += kUmmaThreads) cnt[i] = 0;
+#pragma unroll 1
+    for (int i = tid; i < pps; i += kUmmaThreads) {
+      const int idx = beg + i;
+      int j = 0, prev = 0;
+      if (i < n_all) {
+        j = p.sel_pages[unit * p.k_max + idx];
+        prev = p.sel_prev[unit * p.k_max + idx];
+      }
+      RETRO_DBG_ONLY(if (i < n_all && (j < 0 || j >= min((L + 15) / 16, p.max_pages))) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
+      int phys = 0;
+      if (i < n_all) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
+      RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
+      int32_t* dst = sorted ? tmp : s_list;
+      dst[i] = j;
+      dst[pps + i] = prev;
+      dst[2 * pps + i] = phys;
+    }
+    if (sorted) {
+      __syncthreads();
+      // per 32-entry chunk (one warp each): how many entries of every class, and each entry's rank among its equals
+#pragma unroll 1
+      for (int ch = warp; ch < nchunk; ch += kUmmaThreads / 32) {
+        const int i = ch * 32 + lane;
+        const int v = i < n_all ? cls_of(tmp[pps + i]) : 1000;          // (padding lanes: a class of their own)
+        const unsigned int m = __match_any_sync(0xffffffffu, v);
+        if (i < n_all && (m & ((1u << lane) - 1u)) == 0) cnt[ch * kCls + v] = __popc(m);
+      }
+      __syncthreads();
+      if (tid < kCls) {                            // class tid: exclusive prefix of its counts over the chunks
+        int run = 0;
+#pragma unroll 1
+        for (int ch = 0; ch < nchunk; ++ch) { const int c = cnt[ch * kCls + tid]; cnt[ch * kCls + tid] = run; run += c; }
+        cnt[nchunk * kCls + tid] = run;            // class total
+      }
+      __syncthreads();
+      if (tid == 0) {                              // class bases, most visible class first
+        int off = 0;
+#pragma unroll 1
+        for (int v = kCls - 1; v >= 0; --v) { const int c = cnt[nchunk * kCls + v]; cnt[nchunk * kCls + v] = off; off += c; }
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int ch = warp; ch < nchunk; ch += kUmmaThreads / 32) {
+        const int i = ch * 32 + lane;
+        const int v = i < n_all ? cls_of(tmp[pps + i]) : 1000;
+        const unsigned int m = __match_any_sync(0xffffffffu, v);
+        if (i < n_all) {
+          const int dst = cnt[nchunk * kCls + v] + cnt[ch * kCls + v] + __popc(m & ((1u << lane) - 1u));
+          s_list[dst] = tmp[i];
+          s_list[pps + dst] = tmp[pps + i];
+          s_list[2 * pps + dst] = tmp[2 * pps + i];
+        }
+      }
+      for (int i = n_all + tid; i < pps; i += kUmmaThreads) { s_list[i] = 0; s_list[pps + i] = 0; s_list[2 * pps + i] = 0; }
+    }
+    __syncthreads();
+  }
+  // live 16-row chunks per key block (non-increasing: the list is sorted; a single unsorted block takes its maximum)
+  int my_nl = 0;
+  if (tid < kMaxBlocks && tid * kPB < n_all) {
+    int cmax = 0;
+    for (int e = tid * kPB; e < min(n_all, tid * kPB + kPB); ++e) cmax = max(cmax, cls_of(s_list[pps + e]));
+    my_nl = min(NCH, (cmax * G + 15) / 16);
+    s_nlive[tid] = my_nl;
+  }
+  // slots of the newest page past the sequence's last token are unwritten memory (possibly NaN / Inf): P is 0 there,
+  // but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (idle warp, below)
+  if ((L & 15) != 0)
+    for (int e = tid; e < n_all; e += kUmmaThreads)
+      if (s_list[e] == (L - 1) / 16) { s_fix[0] = e / kPB; s_fix[1] = e % kPB; }
+  const int nblk = __syncthreads_count(my_nl > 0);   // blocks that somebody of this row group sees (a prefix)
+  const int n_my = min(n_all, nblk * kPB);
   const int colS = 0, colO = cfg.NSB * NT;
   fence_proxy_async();          // Q written through the generic proxy, read by the tensor core
   tc_fence_before();
@@ -442,7 +510,10 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
         if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
         mbar_wait(&v_full[slot], n & 1);
-        if (blk == s_fix[0]) mbar_wait(v_clean, 0);
+        if (blk == s_fix[0]) {
+          if (lane == 0) mbar_arrive(v_landed);
+          mbar_wait(v_clean, 0);
+        }
         tc_fence_after();
         if (elect_one()) {
           const uint32_t v_addr = smem_u32(smem + lay.ring + (cfg.NK + slot) * kSlotBytes);
@@ -461,9 +532,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     } else if (warp == 3) {
       // ===== idle warp: zero the unwritten tail rows of the newest page's V tile (both 64-channel halves) =====
       const int fb = s_fix[0];
-      if (fb >= 0) {
+      if (fb >= 0 && fb < nblk) {
         const int slot = fb % cfg.NV, pg = s_fix[1], nv = L & 15;
-        mbar_wait(&v_full[slot], (fb / cfg.NV) & 1);
+        mbar_wait(v_landed, 0);
         unsigned char* vt = smem + lay.ring + (cfg.NK + slot) * kSlotBytes + pg * kTileHalfBytes;
         for (int i = lane; i < (16 - nv) * 8; i += 32) {             // 16-byte chunks of rows nv..15 (a row is 128 B per half)
           *reinterpret_cast<uint4*>(vt + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);

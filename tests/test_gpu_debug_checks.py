@@ -87,8 +87,9 @@ def test_corrupted_selector_output_is_counted_and_neutralised(debug_library, dty
         if j in buf.sel_pages[0, h].tolist():                             # the page whose block-table entry was hit
             continue
         for hq in range(h * G, (h + 1) * G):
-            assert torch.equal(buf.part_o[0, cur, hq], good_o[0, cur, hq])
-            assert torch.equal(buf.part_lse[0, cur, hq], good_l[0, cur, hq])
+            # (row sums are accumulated with shared-memory float atomics: equal up to the order of the additions)
+            assert torch.allclose(buf.part_o[0, cur, hq], good_o[0, cur, hq], atol=1e-5, rtol=1e-5)
+            assert torch.allclose(buf.part_lse[0, cur, hq], good_l[0, cur, hq], atol=1e-5, rtol=1e-5)
     if cfg.batch > 1:                                                     # the other sequence is untouched
-        assert torch.equal(buf.part_o[1], good_o[1])
+        assert torch.allclose(buf.part_o[1], good_o[1], atol=1e-5, rtol=1e-5)
     assert torch.isfinite(buf.part_o).all()

@@ -259,10 +259,11 @@ def test_c5_full_sweep_points_whole_step(w, budget):
 @pytest.mark.parametrize("use_step", [False, True])
 def test_multi_block_wide_rows_window_full(use_step):
     """C3 shape shrunk: 128 units (one split each), 128 selected pages = 16 key blocks per CTA, 68 rows (NT = 80,
-    a single P buffer), window full on the last two steps."""
+    a single P buffer), every step from the empty window to the full one (few live row chunks early on); the last
+    sequence is shorter than the budget (dense, 100 pages, a 4-page last block with the partly written newest page)."""
     cfg = wl.shrink(wl.c3(), tuple(2500 - 61 * b for b in range(16)), 18)
     inp = wl.make_layer_inputs(cfg)
-    print("multi-block wide errs", GH.lockstep(inp, 18, oracle_batch=(0, 9), use_decode_step=use_step, check_from=8))
+    print("multi-block wide errs", GH.lockstep(inp, 18, oracle_batch=(0, 15), use_decode_step=use_step))
 
 
 def test_multi_block_wide_rows_gqa7_window_full():
