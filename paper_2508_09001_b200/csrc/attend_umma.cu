@@ -44,7 +44,6 @@ constexpr int kHalfStride = kPB * kTileHalfBytes;   // 16 KB: [half][page][16][1
 constexpr int kSlotBytes = 2 * kHalfStride;   // 32 KB: one K block or one V block
 constexpr int kTmemCols = 512;
 constexpr int kUmmaSmemBudget = 232448 - 1024 - 4096;   // dynamic shared memory the launcher plans with (one CTA per SM)
-constexpr int kMaxBlocks = 256;                // key blocks per CTA (2048 pages per split)
 constexpr int kMaxNT = 128;                   // rows padded to 16; larger row blocks take the scalar path
 constexpr float kRescaleThreshold = 64.f;     // log2 units: P <= 2^64, sums stay far below the fp32 / bf16 range
 constexpr float kMrefInit = -1.0e30f;         // finite "row not started" reference: -inf - kMrefInit stays -inf
@@ -155,8 +154,7 @@ __host__ __device__ inline UmmaLayout umma_layout(int NT, int NS, int NP, int pa
   UmmaLayout L;
   const int natom = (2 * NT + 63) / 64;
   L.q = 0;                                   // [half][NT rows][128 B]
-  L.p = L.q + 2 * NT * 128;                  // [buf][atom][128 keys][128 B = 64 columns]; columns: per 16-row chunk
-                                             // its 16 hi values then its 16 lo values
+  L.p = L.q + 2 * NT * 128;                  // [buf][atom][128 keys][128 B = 64 columns]; columns = hi rows | lo rows
   L.p_hl_bytes = 0;
   L.p_buf_bytes = natom * 16384;
   L.ring = L.p + NP * L.p_buf_bytes;
@@ -187,7 +185,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   __shared__ __align__(8) uint64_t bars[24];
   __shared__ uint32_t tmem_ptr_s;
   __shared__ int s_flag[3];
-  __shared__ int s_nlive[kMaxBlocks];            // live 16-row chunks of every key block of this CTA (non-increasing)
   __shared__ int s_fix[2];                       // (block, page slot) of the newest page if its tail is unwritten, else -1
   __shared__ int s_rowr[kMaxWindow + 1];         // window rank (t - position) -> row of q_win / out, -1 = none
   __shared__ int s_posr[kMaxWindow + 1];         // q_pos of every row of q_win
@@ -206,9 +203,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   uint64_t* v_empty = bars + 9;          // [NV <= 3]
   uint64_t* s_full = bars + 12;          // [2]
   uint64_t* p_ready = bars + 14;         // [2]
-  uint64_t* v_clean = bars + 18;         // [1] the unwritten tail rows of the newest page's V tile are zeroed
-  uint64_t* v_landed = bars + 19;        // [1] the V block that holds that tile has landed (single use: a parity
-                                         // wait on the ring's own barrier would alias with earlier fills of the slot)
   uint64_t* o_full = bars + 16;          // [2] PV of block blk retired -> o_full[blk & 1], phase blk >> 1 (the
                                          // softmax warps run up to two blocks ahead: one barrier would alias)
   int32_t* s_list = reinterpret_cast<int32_t*>(smem + lay.list);       // [3][pps] logical, prev, physical
@@ -229,7 +223,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     mbar_init(&s_full[0], 1); mbar_init(&s_full[1], 1);
     mbar_init(&p_ready[0], kSoftmaxThreads / 32); mbar_init(&p_ready[1], kSoftmaxThreads / 32);
     mbar_init(&o_full[0], 1); mbar_init(&o_full[1], 1);
-    mbar_init(v_clean, 1); mbar_init(v_landed, 1);
     fence_mbar_init();
   }
   if (warp == 2) {
@@ -354,96 +347,29 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
   RETRO_DBG_ONLY(if (count < 0 || count > p.k_max) { if (tid == 0) dbg_violation(p.dbg, kDbgSelCount); count = 0; })
   RETRO_DBG_ONLY(if (L < 0 || L > p.max_pages * 16) { if (tid == 0) dbg_violation(p.dbg, kDbgSeqLen); count = 0; })
   RETRO_DBG_ONLY(if (tid < R && my_pos_raw > L - 1) dbg_violation(p.dbg, kDbgQPos);)
+  const int beg0 = min(split * pps, count);
+  for (int i = tid; i < pps; i += kUmmaThreads) {
+    const int idx = split * pps + i;
+    int j = 0, prev = 0;
+    if (idx < p.k_max) {
+      j = p.sel_pages[unit * p.k_max + idx];
+      prev = p.sel_prev[unit * p.k_max + idx];
+    }
+    RETRO_DBG_ONLY(if (idx < count && (j < 0 || j >= min((L + 15) / 16, p.max_pages))) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
+    int phys = 0;
+    if (idx < count) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
+    RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
+    s_list[i] = j;
+    s_list[pps + i] = prev;
+    s_list[2 * pps + i] = phys;
+    // slots of the newest page past the sequence's last token are unwritten memory (possibly NaN / Inf): P is 0
+    // there, but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (below)
+    if (idx < count && j == (L - 1) / 16 && (L & 15) != 0) { s_fix[0] = (idx - beg0) / kPB; s_fix[1] = (idx - beg0) % kPB; }
+  }
   const int beg = min(split * pps, count);
   const int end = min(beg + pps, count);
-  const int n_all = end - beg;                   // selected pages of this split
-  // Mask-aware order.  A page with previous load position `prev` is visible to the window ranks r < t - prev only
-  // (Eq. 2: a past query attends the pages it has NOT seen), i.e. to a PREFIX of the rank-major rows; cls = how
-  // many of this CTA's ranks see it.  The split's pages are sorted by cls, most first (stable counting sort), so
-  // that a key block needs only its first 16 * nl rows and whole trailing blocks nobody of this row group sees
-  // (cls 0) are never loaded.  Pages seen by every live past query (the ~83 % that repeat from the previous step,
-  // PAPER.md:349) cost the current query's rows only.
-  auto cls_of = [&](int prev) { return max(0, min(t - prev - rk0, nrk)); };
-  {
-    int32_t* tmp = reinterpret_cast<int32_t*>(smem + lay.ring);   // the K / V ring is idle until the producers start
-    int32_t* cnt = tmp + 3 * pps;                                  // [chunks of 32 entries + 1][classes 0 .. w + 1] counts
-    constexpr int kCls = kMaxWindow + 2;
-    const bool sorted = n_all > kPB;
-    const int nchunk = (n_all + 31) / 32;
-    if (sorted)
-      for (int i = tid; i < nchunk * kCls; i += kUmmaThreads) cnt[i] = 0;
-#pragma unroll 1
-    for (int i = tid; i < pps; i += kUmmaThreads) {
-      const int idx = beg + i;
-      int j = 0, prev = 0;
-      if (i < n_all) {
-        j = p.sel_pages[unit * p.k_max + idx];
-        prev = p.sel_prev[unit * p.k_max + idx];
-      }
-      RETRO_DBG_ONLY(if (i < n_all && (j < 0 || j >= min((L + 15) / 16, p.max_pages))) { dbg_violation(p.dbg, kDbgSelPage); j = 0; prev = 0x7fffffff; })
-      int phys = 0;
-      if (i < n_all) phys = j < cfg.bt_pages ? s_bt[j] : p.block_table[(size_t)b * p.max_pages + j];
-      RETRO_DBG_ONLY(if (phys < 0 || phys >= p.num_phys) { dbg_violation(p.dbg, kDbgPhysPage); phys = 0; prev = 0x7fffffff; })
-      int32_t* dst = sorted ? tmp : s_list;
-      dst[i] = j;
-      dst[pps + i] = prev;
-      dst[2 * pps + i] = phys;
-    }
-    if (sorted) {
-      __syncthreads();
-      // per 32-entry chunk (one warp each): how many entries of every class, and each entry's rank among its equals
-#pragma unroll 1
-      for (int ch = warp; ch < nchunk; ch += kUmmaThreads / 32) {
-        const int i = ch * 32 + lane;
-        const int v = i < n_all ? cls_of(tmp[pps + i]) : 1000;          // (padding lanes: a class of their own)
-        const unsigned int m = __match_any_sync(0xffffffffu, v);
-        if (i < n_all && (m & ((1u << lane) - 1u)) == 0) cnt[ch * kCls + v] = __popc(m);
-      }
-      __syncthreads();
-      if (tid < kCls) {                            // class tid: exclusive prefix of its counts over the chunks
-        int run = 0;
-#pragma unroll 1
-        for (int ch = 0; ch < nchunk; ++ch) { const int c = cnt[ch * kCls + tid]; cnt[ch * kCls + tid] = run; run += c; }
-        cnt[nchunk * kCls + tid] = run;            // class total
-      }
-      __syncthreads();
-      if (tid == 0) {                              // class bases, most visible class first
-        int off = 0;
-#pragma unroll 1
-        for (int v = kCls - 1; v >= 0; --v) { const int c = cnt[nchunk * kCls + v]; cnt[nchunk * kCls + v] = off; off += c; }
-      }
-      __syncthreads();
-#pragma unroll 1
-      for (int ch = warp; ch < nchunk; ch += kUmmaThreads / 32) {
-        const int i = ch * 32 + lane;
-        const int v = i < n_all ? cls_of(tmp[pps + i]) : 1000;
-        const unsigned int m = __match_any_sync(0xffffffffu, v);
-        if (i < n_all) {
-          const int dst = cnt[nchunk * kCls + v] + cnt[ch * kCls + v] + __popc(m & ((1u << lane) - 1u));
-          s_list[dst] = tmp[i];
-          s_list[pps + dst] = tmp[pps + i];
-          s_list[2 * pps + dst] = tmp[2 * pps + i];
-        }
-      }
-      for (int i = n_all + tid; i < pps; i += kUmmaThreads) { s_list[i] = 0; s_list[pps + i] = 0; s_list[2 * pps + i] = 0; }
-    }
-    __syncthreads();
-  }
-  // live 16-row chunks per key block (non-increasing: the list is sorted; a single unsorted block takes its maximum)
-  int my_nl = 0;
-  if (tid < kMaxBlocks && tid * kPB < n_all) {
-    int cmax = 0;
-    for (int e = tid * kPB; e < min(n_all, tid * kPB + kPB); ++e) cmax = max(cmax, cls_of(s_list[pps + e]));
-    my_nl = min(NCH, (cmax * G + 15) / 16);
-    s_nlive[tid] = my_nl;
-  }
-  // slots of the newest page past the sequence's last token are unwritten memory (possibly NaN / Inf): P is 0 there,
-  // but 0 x NaN would poison the PV product, so those V rows are zeroed in shared memory (idle warp, below)
-  if ((L & 15) != 0)
-    for (int e = tid; e < n_all; e += kUmmaThreads)
-      if (s_list[e] == (L - 1) / 16) { s_fix[0] = e / kPB; s_fix[1] = e % kPB; }
-  const int nblk = __syncthreads_count(my_nl > 0);   // blocks that somebody of this row group sees (a prefix)
-  const int n_my = min(n_all, nblk * kPB);
+  const int n_my = end - beg;
+  const int nblk = (n_my + kPB - 1) / kPB;
   const int colS = 0, colO = cfg.NSB * NT;
   fence_proxy_async();          // Q written through the generic proxy, read by the tensor core
   tc_fence_before();
@@ -477,8 +403,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
     } else if (warp == 2) {
       // ===== MMA issuer: the whole warp walks the loop (waits), one elected lane issues =====
       const uint32_t q_addr = smem_u32(smem + lay.q);
-      // N follows the block's live 16-row chunks: rows are rank-major (newest first) and a page is visible to a
-      // PREFIX of the ranks, so the rows a block can contribute to are the first 16 * nl (S) / 32 * nl (P, O) columns
+      const uint32_t idesc_s = idesc_bf16_ab(NT, false, false);
+      const uint32_t idesc_o = idesc_bf16_ab(2 * NT, true, true);
       auto issue_s = [&](int blk) {
         const int slot = blk % cfg.NK, n = blk / cfg.NK;
         mbar_wait(&k_full[slot], n & 1);
@@ -490,8 +416,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           for (int ks = 0; ks < 8; ++ks) {    // K = 128 channels = 8 steps of 16; 4 steps per 64-channel half
             const uint32_t koff = (ks >> 2) * kHalfStride + (ks & 3) * 32;
             const uint32_t qoff = (ks >> 2) * (NT * 128) + (ks & 3) * 32;
-            umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff),
-                      idesc_bf16_ab(16 * s_nlive[blk], false, false), ks > 0);
+            umma_bf16(d_tmem, desc_kmajor_sw128(k_addr + koff), desc_kmajor_sw128(q_addr + qoff), idesc_s, ks > 0);
           }
           tc_commit(&k_empty[slot]);
           tc_commit(&s_full[blk % cfg.NSB]);
@@ -510,10 +435,6 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         mbar_wait(&p_ready[blk % cfg.NP], (blk / cfg.NP) & 1);
         if (cfg.NSB == 1 && blk + 1 < nblk) issue_s(blk + 1);   // S is free once P(blk) is written
         mbar_wait(&v_full[slot], n & 1);
-        if (blk == s_fix[0]) {
-          if (lane == 0) mbar_arrive(v_landed);
-          mbar_wait(v_clean, 0);
-        }
         tc_fence_after();
         if (elect_one()) {
           const uint32_t v_addr = smem_u32(smem + lay.ring + (cfg.NK + slot) * kSlotBytes);
@@ -521,28 +442,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           for (int ks = 0; ks < np; ++ks) {   // K = 16 keys (one page) per step
             const uint64_t vdesc = desc_mnmajor_sw128(v_addr + ks * kTileHalfBytes, kHalfStride);
             const uint64_t pdesc = desc_mnmajor_sw128(p_addr + ks * 2048, 16384);
-            umma_bf16(tmem_base + colO, vdesc, pdesc, idesc_bf16_ab(32 * s_nlive[blk], true, true),
-                      (blk > 0 || ks > 0) ? 1u : 0u);
+            umma_bf16(tmem_base + colO, vdesc, pdesc, idesc_o, (blk > 0 || ks > 0) ? 1u : 0u);
           }
           tc_commit(&v_empty[slot]);
           tc_commit(&o_full[blk & 1]);
         }
         __syncwarp();
-      }
-    } else if (warp == 3) {
-      // ===== idle warp: zero the unwritten tail rows of the newest page's V tile (both 64-channel halves) =====
-      const int fb = s_fix[0];
-      if (fb >= 0 && fb < nblk) {
-        const int slot = fb % cfg.NV, pg = s_fix[1], nv = L & 15;
-        mbar_wait(v_landed, 0);
-        unsigned char* vt = smem + lay.ring + (cfg.NK + slot) * kSlotBytes + pg * kTileHalfBytes;
-        for (int i = lane; i < (16 - nv) * 8; i += 32) {             // 16-byte chunks of rows nv..15 (a row is 128 B per half)
-          *reinterpret_cast<uint4*>(vt + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
-          *reinterpret_cast<uint4*>(vt + kHalfStride + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
-        }
-        fence_proxy_async();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(v_clean);
       }
     } else if (warp >= 4) {
       // ===== softmax warps: thread <-> TMEM lane <-> key of the block; NC = NT / 4 columns (rows) each =====
@@ -550,10 +455,9 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       const int quadrant = warp & 3;                      // TMEM lanes a warp may touch: 32*(warp%4)..+31
       const int cg = sw >> 2;                             // column group
       const int key = quadrant * 32 + lane;
-      const int c4 = 4 * cg;                              // the thread's columns of 16-row chunk i: 16 i + c4 .. + 3
+      const int cbeg = cg * NC;
       const int st = tid - 128;                           // 0..511
       const uint32_t lane_addr = tmem_base + ((uint32_t)(quadrant * 32) << 16);
-      const int nl0 = s_nlive[0];                         // the first block has the most live chunks
       float l_acc[NC];                                    // this key-thread's share of the row sums
 #pragma unroll
       for (int j = 0; j < NC; ++j) l_acc[j] = 0.f;
@@ -568,30 +472,26 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         if (st == 0) s_flag[(blk + 1) % 3] = 0;
         mbar_wait(&s_full[blk % cfg.NSB], (blk / cfg.NSB) & 1);
         tc_fence_after();
-        const int nl = s_nlive[blk];                        // live 16-row chunks of this block (block-uniform)
-        const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + c4;
+        const uint32_t s_addr = lane_addr + colS + (blk % cfg.NSB) * NT + cbeg;
         // d = s * scale - m_ref (log2 units), -inf where masked; the common block needs nothing else
         float d[NC];
         float tmax = -INFINITY;
         {
           uint32_t raw[NC];
 #pragma unroll
-          for (int i = 0; i < NCH; ++i)
-            if (i < nl) tmem_ld4(s_addr + 16 * i, raw + 4 * i);
+          for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
           tmem_wait_ld();
 #pragma unroll
           for (int i = 0; i < NCH; ++i) {
-            if (i < nl) {
-              const int4 ps = *reinterpret_cast<const int4*>(s_colpos + 16 * i + c4);
-              const float4 mr = *reinterpret_cast<const float4*>(s_mref + 16 * i + c4);
-              const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
-              const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
+            const int4 ps = *reinterpret_cast<const int4*>(s_colpos + cbeg + 4 * i);
+            const float4 mr = *reinterpret_cast<const float4*>(s_mref + cbeg + 4 * i);
+            const int pv[4] = {ps.x, ps.y, ps.z, ps.w};
+            const float mv[4] = {mr.x, mr.y, mr.z, mr.w};
 #pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const float v = fmaf(__uint_as_float(raw[4 * i + u]), p.scale_log2, -mv[u]);
-                d[4 * i + u] = pv[u] > thr ? v : -INFINITY;
-                tmax = fmaxf(tmax, d[4 * i + u]);
-              }
+            for (int u = 0; u < 4; ++u) {
+              const float v = fmaf(__uint_as_float(raw[4 * i + u]), p.scale_log2, -mv[u]);
+              d[4 * i + u] = pv[u] > thr ? v : -INFINITY;
+              tmax = fmaxf(tmax, d[4 * i + u]);
             }
           }
         }
@@ -603,20 +503,16 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           {
             uint32_t raw[NC];
 #pragma unroll
-            for (int i = 0; i < NCH; ++i)
-              if (i < nl) tmem_ld4(s_addr + 16 * i, raw + 4 * i);
+            for (int i = 0; i < NCH; ++i) tmem_ld4(s_addr + 4 * i, raw + 4 * i);
             tmem_wait_ld();
 #pragma unroll
             for (int j = 0; j < NC; ++j)
-              if ((j >> 2) < nl)
-                xs[j] = s_colpos[16 * (j >> 2) + c4 + (j & 3)] > thr ? __uint_as_float(raw[j]) * p.scale_log2 : -INFINITY;
+              xs[j] = s_colpos[cbeg + j] > thr ? __uint_as_float(raw[j]) * p.scale_log2 : -INFINITY;
           }
 #pragma unroll
           for (int j = 0; j < NC; ++j) {
-            if ((j >> 2) < nl) {
-              const int r = __reduce_max_sync(0xffffffffu, f2o(xs[j]));
-              if (lane == 0) atomicMax(&s_colmax[16 * (j >> 2) + c4 + (j & 3)], r);
-            }
+            const int r = __reduce_max_sync(0xffffffffu, f2o(xs[j]));
+            if (lane == 0) atomicMax(&s_colmax[cbeg + j], r);
           }
           softmax_bar();
           if (st < NT) {
@@ -628,30 +524,28 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           }
           softmax_bar();
 #pragma unroll
-          for (int j = 0; j < NC; ++j) {                   // (alpha is 1 for the rows of dead chunks)
-            const int c = 16 * (j >> 2) + c4 + (j & 3);
-            l_acc[j] *= s_alpha[c];
-            if ((j >> 2) < nl) d[j] = xs[j] - s_mref[c];
+          for (int j = 0; j < NC; ++j) {
+            l_acc[j] *= s_alpha[cbeg + j];
+            d[j] = xs[j] - s_mref[cbeg + j];
           }
           if (blk > 0) {
             mbar_wait(&o_full[(blk - 1) & 1], ((blk - 1) >> 1) & 1);   // PV(blk-1) retired: O is ours
             tc_fence_after();
 #pragma unroll
             for (int i = 0; i < NCH; ++i) {                  // this thread's columns of O_hi and O_lo
-              if (i >= nl0) continue;                        // chunks no block has touched yet hold nothing
-              const float4 al4 = *reinterpret_cast<const float4*>(s_alpha + 16 * i + c4);
+              const float4 al4 = *reinterpret_cast<const float4*>(s_alpha + cbeg + 4 * i);
               const float al[4] = {al4.x, al4.y, al4.z, al4.w};
               uint32_t oh[4], ol[4];
-              tmem_ld4(lane_addr + colO + 32 * i + c4, oh);
-              tmem_ld4(lane_addr + colO + 32 * i + 16 + c4, ol);
+              tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
+              tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
               tmem_wait_ld();
 #pragma unroll
               for (int u = 0; u < 4; ++u) {
                 oh[u] = __float_as_uint(__uint_as_float(oh[u]) * al[u]);
                 ol[u] = __float_as_uint(__uint_as_float(ol[u]) * al[u]);
               }
-              tmem_st4(lane_addr + colO + 32 * i + c4, oh);
-              tmem_st4(lane_addr + colO + 32 * i + 16 + c4, ol);
+              tmem_st4(lane_addr + colO + cbeg + 4 * i, oh);
+              tmem_st4(lane_addr + colO + NT + cbeg + 4 * i, ol);
             }
             tmem_wait_st();
           }
@@ -661,14 +555,13 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         unsigned char* p_row = smem + lay.p + (blk % cfg.NP) * lay.p_buf_bytes + key * 128;
 #pragma unroll
         for (int i = 0; i < NCH; ++i) {
-          if (i >= nl) continue;
           float e[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             e[u] = ex2_approx(d[4 * i + u]);
             l_acc[4 * i + u] += e[u];
           }
-          const int c_hi = 32 * i + c4, c_lo = c_hi + 16;   // operand columns: chunk i = [16 hi rows | 16 lo rows]
+          const int c_hi = cbeg + 4 * i, c_lo = NT + c_hi;
           uint2 hi, lo;
           split_bf16x2(e[0], e[1], hi.x, lo.x);
           split_bf16x2(e[2], e[3], hi.y, lo.y);
@@ -676,6 +569,19 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
                                     ((c_hi & 4) << 1)) = hi;
           *reinterpret_cast<uint2*>(p_row + (c_lo >> 6) * 16384 + ((((c_lo & 63) >> 3) ^ (key & 7)) << 4) +
                                     ((c_lo & 4) << 1)) = lo;
+        }
+        if (blk == s_fix[0] && sw == 0) {
+          // the unwritten tail rows of the newest page's V tile (both 64-channel halves) are zeroed before this
+          // block's PV product can start (it needs every softmax warp's arrival below).  The V slot of block blk
+          // cannot be refilled before that product, so its barrier is in phase blk / NV or one later: the parity
+          // wait cannot alias with another fill of the slot.
+          const int slot = blk % cfg.NV, pg = s_fix[1], nv = L & 15;
+          mbar_wait(&v_full[slot], (blk / cfg.NV) & 1);
+          unsigned char* vt = smem + lay.ring + (cfg.NK + slot) * kSlotBytes + pg * kTileHalfBytes;
+          for (int i = lane; i < (16 - nv) * 8; i += 32) {           // 16-byte chunks of rows nv..15 (128 B per row and half)
+            *reinterpret_cast<uint4*>(vt + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
+            *reinterpret_cast<uint4*>(vt + kHalfStride + nv * 128 + i * 16) = make_uint4(0, 0, 0, 0);
+          }
         }
         fence_proxy_async();
         tc_fence_before();
@@ -698,8 +604,7 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           v += __shfl_xor_sync(0xffffffffu, v, 4);
           v += __shfl_xor_sync(0xffffffffu, v, 2);
           v += __shfl_xor_sync(0xffffffffu, v, 1);
-          const int k = ((lane >> 3) & 3) * NCH + i;        // index into l_acc = 4 * chunk + u
-          if ((lane & 7) == 0) atomicAdd(&s_L[16 * (k >> 2) + c4 + (k & 3)], v);
+          if ((lane & 7) == 0) atomicAdd(&s_L[cbeg + ((lane >> 3) & 3) * NCH + i], v);
         }
       }
       mbar_wait(&o_full[(nblk - 1) & 1], ((nblk - 1) >> 1) & 1);
@@ -712,16 +617,14 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       __half* stage = reinterpret_cast<__half*>(smem + lay.ring);
 #pragma unroll
       for (int i = 0; i < NCH; ++i) {
-        if (16 * i + c4 < rows_cta) {                       // warp-uniform
-          uint32_t oh[4] = {0u, 0u, 0u, 0u}, ol[4] = {0u, 0u, 0u, 0u};
-          if (i < nl0) {                                    // (chunks no block touched: L is 0, the row reads empty)
-            tmem_ld4(lane_addr + colO + 32 * i + c4, oh);
-            tmem_ld4(lane_addr + colO + 32 * i + 16 + c4, ol);
-            tmem_wait_ld();
-          }
+        if (cbeg + 4 * i < rows_cta) {                      // warp-uniform
+          uint32_t oh[4], ol[4];
+          tmem_ld4(lane_addr + colO + cbeg + 4 * i, oh);
+          tmem_ld4(lane_addr + colO + NT + cbeg + 4 * i, ol);
+          tmem_wait_ld();
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int c = 16 * i + c4 + u;
+            const int c = cbeg + 4 * i + u;
             if (c < rows_cta) {
               const float l = s_L[c];
               const float inv = rcp_approx(l);

@@ -87,9 +87,10 @@ def test_corrupted_selector_output_is_counted_and_neutralised(debug_library, dty
         if j in buf.sel_pages[0, h].tolist():                             # the page whose block-table entry was hit
             continue
         for hq in range(h * G, (h + 1) * G):
-            # (row sums are accumulated with shared-memory float atomics: equal up to the order of the additions)
-            assert torch.allclose(buf.part_o[0, cur, hq], good_o[0, cur, hq], atol=1e-5, rtol=1e-5)
-            assert torch.allclose(buf.part_lse[0, cur, hq], good_l[0, cur, hq], atol=1e-5, rtol=1e-5)
+            # (row sums are accumulated with shared-memory float atomics, the split partials pass through fp16:
+            # equal up to the order of the additions amplified to an fp16 ulp)
+            assert torch.allclose(buf.part_o[0, cur, hq], good_o[0, cur, hq], atol=2e-3, rtol=2e-3)
+            assert torch.allclose(buf.part_lse[0, cur, hq], good_l[0, cur, hq], atol=1e-4, rtol=1e-4)
     if cfg.batch > 1:                                                     # the other sequence is untouched
-        assert torch.allclose(buf.part_o[1], good_o[1], atol=1e-5, rtol=1e-5)
+        assert torch.allclose(buf.part_o[1], good_o[1], atol=2e-3, rtol=2e-3)
     assert torch.isfinite(buf.part_o).all()
