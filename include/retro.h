@@ -37,7 +37,10 @@
  *                                                   [t-w, t] are treated as empty
  *   part_o           [B][w+1][h_q][d] float         normalised partial output of each row over its unseen pages
  *   part_lse         [B][w+1][h_q] float            natural-log sum-exp of the same; empty set -> o = 0, lse = -inf
- *   cache_o          [B][w][h_q][d] float           output cache ring, slot = position mod w
+ *   cache_o          [B][w][h_q][d] float           output cache ring, slot = position mod w; bf16 instead of float
+ *                                                   with desc->cache_dtype == RETRO_BF16 (needs dtype RETRO_BF16):
+ *                                                   the paper's footprint, 16-bit O + fp32 LSE (Eq. 12,
+ *                                                   PAPER.md:502-507); merges run in fp32, the STORED row is rounded
  *   cache_lse        [B][w][h_q] float
  *   cache_pos        [B][w] int32                   position held by each slot, -1 = empty
  *   out              [B][w+1][h_q][d] T             merged outputs, row r belongs to q_pos[b][r]; empty rows = 0
@@ -81,6 +84,7 @@ typedef struct retro_desc {
   int32_t group_reduce;      /* RETRO_GROUP_SUM | RETRO_GROUP_MAX                              */
   int32_t force_last_page;   /* 1: newest page always selected and counted in k (reading Q3)   */
   float sm_scale;            /* softmax scale, 1/sqrt(head_dim)                  */
+  int32_t cache_dtype;       /* RETRO_F32 (0, default) | RETRO_BF16: element type of cache_o   */
 } retro_desc_t;
 
 /* Bytes of scratch the S2/S3 entry points need for this descriptor (page scores, split-KV partials,
@@ -130,7 +134,7 @@ int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32
  * `out`; written back to its slot unless p = t-w (popped after its last merge).  Current row: out = part, pushed
  * into slot t mod w.  window == 0: out = part, cache_* may be NULL. */
 int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, const float* part_lse,
-                             const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                             const int32_t* q_pos, const int32_t* seq_lens, void* cache_o, float* cache_lse,
                              int32_t* cache_pos, void* out, float* out_lse, void* stream);
 
 /* AppendKV (Alg. 1 line 3).  Writes k_new / v_new [B][h_k][d] T into position seq_lens[b] - 1 of
@@ -155,7 +159,7 @@ typedef struct retro_layer_state {
   int32_t* sel_count;
   float* part_o;
   float* part_lse;
-  float* cache_o;
+  void* cache_o;         /* float or bf16, see cache_dtype */
   float* cache_lse;
   int32_t* cache_pos;
   void* workspace;

@@ -71,6 +71,8 @@ class OracleDesc:
     sm_scale: float
     group_reduce: str = "sum"   # "sum" | "max"   (reading Q2)
     force_last_page: bool = True  # reading Q3
+    cache_round: str = "none"     # "none": the cached O keeps full precision (reading Q13); "bf16": it is stored in 16 bits
+                                  # next to an fp32 LSE, the paper's footprint (Eq. 12) with bf16 for FP16
 
     @property
     def group(self) -> int:
@@ -318,6 +320,15 @@ def merge_partials(o_a, lse_a, o_b, lse_b):
     return (wa * o_a + wb * o_b) / (wa + wb), m + math.log(wa + wb)
 
 
+def round_bf16(x):
+    """Round-to-nearest-even to bfloat16 (8 significant bits), returned as float64: what a 16-bit output cache stores
+    (Eq. 12).  Bit arithmetic on the float32 image; values are finite."""
+    f = np.asarray(x, dtype=np.float64).astype(np.float32)
+    u = f.view(np.uint32).astype(np.uint64)
+    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32).astype(np.float64)
+
+
 def merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_lse, cache_pos):
     """Update: merge each past row's new partial into its cached (o, lse); Push: store the current
     row; Pop: the row at position t-w is returned after its last merge and its slot is reused.
@@ -344,7 +355,7 @@ def merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_l
                 out[b, r, hh] = o
                 out_lse[b, r, hh] = lse
                 if p != t - w:                           # the oldest row is popped, not written back
-                    cache_o[b, slot, hh] = o
+                    cache_o[b, slot, hh] = round_bf16(o) if desc.cache_round == "bf16" else o
                     cache_lse[b, slot, hh] = lse
             if p != t - w:
                 new_pos[slot] = p
@@ -355,7 +366,7 @@ def merge_output_cache(desc, part_o, part_lse, q_pos, seq_lens, cache_o, cache_l
             out[b, r] = part_o[b, r]
             out_lse[b, r] = part_lse[b, r]
             if w > 0:
-                cache_o[b, t % w] = part_o[b, r]
+                cache_o[b, t % w] = round_bf16(part_o[b, r]) if desc.cache_round == "bf16" else part_o[b, r]
                 cache_lse[b, t % w] = part_lse[b, r]
                 new_pos[t % w] = t
         if w > 0:

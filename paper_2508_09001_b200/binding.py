@@ -32,7 +32,8 @@ EXPORTED = [
 class RetroDesc(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size", "max_pages_per_seq", "max_sel_pages",
-        "num_phys_pages", "window", "dtype", "group_reduce", "force_last_page")] + [("sm_scale", C.c_float)]
+        "num_phys_pages", "window", "dtype", "group_reduce", "force_last_page")] + [("sm_scale", C.c_float),
+                                                                                      ("cache_dtype", C.c_int32)]
 
     @property
     def group(self):
@@ -122,14 +123,14 @@ def _check(rc: int, where: str):
 
 def make_desc(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_pages_per_seq, max_sel_pages,
               num_phys_pages, window, dtype, group_reduce=RETRO_GROUP_SUM, force_last_page=1,
-              sm_scale=None) -> RetroDesc:
+              sm_scale=None, cache_dtype=RETRO_F32) -> RetroDesc:
     if isinstance(dtype, torch.dtype):
         dtype = RETRO_BF16 if dtype == torch.bfloat16 else RETRO_F32
     elif isinstance(dtype, str):
         dtype = RETRO_BF16 if dtype == "bf16" else RETRO_F32
     return RetroDesc(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_pages_per_seq, max_sel_pages,
                      num_phys_pages, window, dtype, group_reduce, int(force_last_page),
-                     1.0 / math.sqrt(head_dim) if sm_scale is None else sm_scale)
+                     1.0 / math.sqrt(head_dim) if sm_scale is None else sm_scale, int(cache_dtype))
 
 
 def retro_version() -> int:
@@ -281,7 +282,8 @@ class LayerBuffers:
         self.sel_count = torch.zeros((B, hk), dtype=torch.int32, device=dev)
         self.part_o = torch.zeros((B, w + 1, hq, D), dtype=torch.float32, device=dev)
         self.part_lse = torch.full((B, w + 1, hq), -math.inf, dtype=torch.float32, device=dev)
-        self.cache_o = torch.zeros((B, max(w, 1), hq, D), dtype=torch.float32, device=dev)
+        cache_dt = torch.bfloat16 if d.cache_dtype == RETRO_BF16 else torch.float32
+        self.cache_o = torch.zeros((B, max(w, 1), hq, D), dtype=cache_dt, device=dev)
         self.cache_lse = torch.full((B, max(w, 1), hq), -math.inf, dtype=torch.float32, device=dev)
         self.cache_pos = torch.full((B, max(w, 1)), -1, dtype=torch.int32, device=dev)
         self.out = torch.zeros((B, w + 1, hq, D), dtype=dt, device=dev)

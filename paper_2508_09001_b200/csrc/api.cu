@@ -99,6 +99,8 @@ int validate_desc(const retro_desc_t* d) {
     return RETRO_ERR_ARG;
   if (d->num_q_heads % d->num_kv_heads != 0) return RETRO_ERR_ARG;
   if (d->group_reduce != RETRO_GROUP_SUM && d->group_reduce != RETRO_GROUP_MAX) return RETRO_ERR_ARG;
+  if (d->cache_dtype != RETRO_F32 && d->cache_dtype != RETRO_BF16) return RETRO_ERR_ARG;
+  if (d->cache_dtype == RETRO_BF16 && d->dtype != RETRO_BF16) return RETRO_ERR_UNSUPPORTED;
   if (!(d->sm_scale > 0.f)) return RETRO_ERR_ARG;
   const bool f32 = d->dtype == RETRO_F32 && d->head_dim == 64 && d->page_size == 16;
   const bool bf16 = d->dtype == RETRO_BF16 && d->head_dim == 128 && d->page_size == 16;
@@ -251,7 +253,7 @@ int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32
 }
 
 int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, const float* part_lse,
-                             const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                             const int32_t* q_pos, const int32_t* seq_lens, void* cache_o, float* cache_lse,
                              int32_t* cache_pos, void* out, float* out_lse, void* stream) {
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(part_o); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(seq_lens);

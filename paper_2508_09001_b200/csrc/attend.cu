@@ -292,6 +292,7 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
   prm.nrg = wl.nrg;
   prm.rg_ranks = wl.rg_ranks;
   prm.fused = 0;
+  prm.cache_bf16 = 0;
   prm.cache_o = nullptr; prm.cache_lse = nullptr; prm.cache_pos = nullptr; prm.out = nullptr; prm.out_lse = nullptr;
   prm.seq_counters = reinterpret_cast<unsigned int*>(ws + wl.slot_counters_off);   // [B]
   prm.dbg = reinterpret_cast<unsigned int*>(ws + wl.debug_off);
@@ -303,6 +304,7 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
       if (!attend_can_fuse_merge(d, wl)) return RETRO_ERR_UNSUPPORTED;
       prm.fused = 1;
       prm.cache_o = fused->cache_o; prm.cache_lse = fused->cache_lse; prm.cache_pos = fused->cache_pos;
+      prm.cache_bf16 = d->cache_dtype == RETRO_BF16;
       prm.out = fused->out; prm.out_lse = fused->out_lse;
     }
     return launch_attend_umma(d, prm, s);

@@ -18,7 +18,8 @@ struct AttendParams {
   float scale_log2;   // sm_scale * log2(e)
   // tensor-core path inside retro_decode_step (fused = 1, nrg == 1): S4 runs in the same kernel
   int fused;
-  float* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse; unsigned int* seq_counters;
+  void* cache_o; int cache_bf16;     // output cache rows: float, or bf16 (Eq. 12's 16-bit O) when cache_bf16
+  float* cache_lse; int32_t* cache_pos; void* out; float* out_lse; unsigned int* seq_counters;
   unsigned int* dbg; int num_phys;   // -DRETRO_DEBUG_CHECKS: violation counter in the workspace, pool size
 };
 

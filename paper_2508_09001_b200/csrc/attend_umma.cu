@@ -317,8 +317,12 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
       if (it >= w * G) break;
       const int x = it / G, g = it - x * G;
       const size_t ce = ((size_t)b * w + x) * p.h_q + h * G + g;
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pre + k * kPreStride + lane * 4)),
-                   "l"(p.cache_o + ce * 128 + lane * 4) : "memory");
+      if (!p.cache_bf16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pre + k * kPreStride + lane * 4)),
+                     "l"(static_cast<const float*>(p.cache_o) + ce * 128 + lane * 4) : "memory");
+      else if (lane < 16)                          // a bf16 row is 256 B
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pre + k * kPreStride + lane * 4)),
+                     "l"(static_cast<const __nv_bfloat16*>(p.cache_o) + ce * 128 + lane * 8) : "memory");
       if (lane == 0)
         asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(pre + k * kPreStride + 128)),
                      "l"(p.cache_lse + ce) : "memory");
@@ -713,12 +717,16 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
           if (s_cpos[x] == t - rank) {                   // something is cached for this position
             float lc;
             float4 vc;
-            if (k < kPreItems) {
-              lc = pre[k * kPreStride + 128];
-              vc = *reinterpret_cast<const float4*>(pre + k * kPreStride + lane * 4);
-            } else {
-              lc = p.cache_lse[ce];
-              vc = *reinterpret_cast<const float4*>(p.cache_o + ce * 128 + lane * 4);
+            if (k < kPreItems) lc = pre[k * kPreStride + 128];
+            else lc = p.cache_lse[ce];
+            if (!p.cache_bf16) {
+              vc = k < kPreItems ? *reinterpret_cast<const float4*>(pre + k * kPreStride + lane * 4)
+                                 : *reinterpret_cast<const float4*>(static_cast<const float*>(p.cache_o) + ce * 128 + lane * 4);
+            } else {                                     // 16-bit cache rows (Eq. 12): 4 bf16 per lane
+              const uint2 u = k < kPreItems
+                  ? *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(pre + k * kPreStride) + lane * 8)
+                  : *reinterpret_cast<const uint2*>(static_cast<const __nv_bfloat16*>(p.cache_o) + ce * 128 + lane * 4);
+              vc = make_float4(bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y));
             }
             if (lc > -INFINITY) {
               if (lse == -INFINITY) { o = vc; lse = lc; }
@@ -737,7 +745,8 @@ attend_umma_kernel(const AttendParams p, const UmmaCfg cfg, const __grid_constan
         store_bf16x4(reinterpret_cast<__nv_bfloat16*>(p.out) + e * 128 + lane * 4, o);
         if (lane == 0 && p.out_lse != nullptr) p.out_lse[e] = lse;
         if (write_back) {
-          *reinterpret_cast<float4*>(p.cache_o + ce * 128 + lane * 4) = o;
+          if (!p.cache_bf16) *reinterpret_cast<float4*>(static_cast<float*>(p.cache_o) + ce * 128 + lane * 4) = o;
+          else store_bf16x4(static_cast<__nv_bfloat16*>(p.cache_o) + ce * 128 + lane * 4, o);
           if (lane == 0) p.cache_lse[ce] = lse;
         }
       }

@@ -75,7 +75,7 @@ WorkspaceLayout workspace_layout(const retro_desc_t* d);
 
 // S4 operands for the attend kernel that also merges the output cache (retro_decode_step)
 struct FusedMerge {
-  float* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse;
+  void* cache_o; float* cache_lse; int32_t* cache_pos; void* out; float* out_lse;
 };
 
 // ---- kernel launchers (one per stage; defined in the matching .cu) ------------------------------
@@ -94,7 +94,7 @@ int launch_sparse_attend(const retro_desc_t* d, const WorkspaceLayout& wl, const
                          const FusedMerge* fused = nullptr);   // non-null (tensor-core path, one row group): S4 in the same kernel
 bool attend_can_fuse_merge(const retro_desc_t* d, const WorkspaceLayout& wl);
 int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
-                              const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                              const int32_t* q_pos, const int32_t* seq_lens, void* cache_o, float* cache_lse,
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s);
 int launch_append_kv(const retro_desc_t* d, const void* k_new, const void* v_new, const int32_t* block_table,
                      const int32_t* seq_lens, void* k_pages, void* v_pages, cudaStream_t s);

@@ -23,11 +23,24 @@ template <> struct OutVec<__nv_bfloat16> {
   }
 };
 
-template <typename T>
+template <typename C> struct CacheVec;   // 4 consecutive cache values as a float4
+template <> struct CacheVec<float> {
+  __device__ static __forceinline__ float4 load(const float* p) { return *reinterpret_cast<const float4*>(p); }
+  __device__ static __forceinline__ void store(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+};
+template <> struct CacheVec<__nv_bfloat16> {
+  __device__ static __forceinline__ float4 load(const __nv_bfloat16* p) {
+    const uint2 u = *reinterpret_cast<const uint2*>(p);
+    return make_float4(bf16_lo(u.x), bf16_hi(u.x), bf16_lo(u.y), bf16_hi(u.y));
+  }
+  __device__ static __forceinline__ void store(__nv_bfloat16* p, float4 v) { OutVec<__nv_bfloat16>::store(p, v); }
+};
+
+template <typename T, typename C>
 __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restrict__ part_o,
                                                           const float* __restrict__ part_lse,
                                                           const int32_t* __restrict__ q_pos,
-                                                          const int32_t* __restrict__ seq_lens, float* cache_o,
+                                                          const int32_t* __restrict__ seq_lens, C* cache_o,
                                                           float* cache_lse, int32_t* cache_pos, T* __restrict__ out,
                                                           float* __restrict__ out_lse, int h_q, int D, int w) {
   const int b = blockIdx.y, x = blockIdx.x;
@@ -84,7 +97,7 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
   const bool cached = s_cached != 0;
   const int p_past = s_ppast;
   const bool evict = past >= 0 && p_past == t - w;   // popped after its last merge
-  float* c_o = cache_o + ((size_t)b * w + slot) * h_q * D;
+  C* c_o = cache_o + ((size_t)b * w + slot) * h_q * D;
   float* c_l = cache_lse + ((size_t)b * w + slot) * h_q;
   const float* po = part_o + ((size_t)b * R + (past >= 0 ? past : 0)) * h_q * D;
   const float* pl = part_lse + ((size_t)b * R + (past >= 0 ? past : 0)) * h_q;
@@ -99,7 +112,7 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
       if (i < n_vec) {
         const int hh = i / vec_per_row;
         if (past >= 0) { vp[u] = *reinterpret_cast<const float4*>(po + (size_t)i * 4); lp[u] = pl[hh]; }
-        if (past >= 0 && cached) { vc[u] = *reinterpret_cast<const float4*>(c_o + (size_t)i * 4); lc[u] = c_l[hh]; }
+        if (past >= 0 && cached) { vc[u] = CacheVec<C>::load(c_o + (size_t)i * 4); lc[u] = c_l[hh]; }
         if (cur >= 0) { vq[u] = *reinterpret_cast<const float4*>(qo + (size_t)i * 4); lq[u] = ql[hh]; }
       }
     }
@@ -129,7 +142,7 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
           lse = mx + __logf(wc + wp);
         }
         OutVec<T>::store(oo + (size_t)i * 4, res);
-        if (!evict) *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = res;
+        if (!evict) CacheVec<C>::store(c_o + (size_t)i * 4, res);
         if (head_lane) {
           if (out_lse != nullptr) out_lse[((size_t)b * R + past) * h_q + hh] = lse;
           if (!evict) c_l[hh] = lse;
@@ -138,7 +151,7 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
       if (cur >= 0) {   // push O_org of the current query (the popped row is already in registers)
         T* oo = out + ((size_t)b * R + cur) * h_q * D;
         OutVec<T>::store(oo + (size_t)i * 4, vq[u]);
-        *reinterpret_cast<float4*>(c_o + (size_t)i * 4) = vq[u];
+        CacheVec<C>::store(c_o + (size_t)i * 4, vq[u]);
         if (head_lane) {
           if (out_lse != nullptr) out_lse[((size_t)b * R + cur) * h_q + hh] = lq[u];
           c_l[hh] = lq[u];
@@ -153,17 +166,21 @@ __global__ void __launch_bounds__(256) merge_cache_kernel(const float* __restric
 }
 
 int launch_merge_output_cache(const retro_desc_t* d, const float* part_o, const float* part_lse,
-                              const int32_t* q_pos, const int32_t* seq_lens, float* cache_o, float* cache_lse,
+                              const int32_t* q_pos, const int32_t* seq_lens, void* cache_o, float* cache_lse,
                               int32_t* cache_pos, void* out, float* out_lse, cudaStream_t s) {
   dim3 grid(d->window + 1, d->batch);
-  if (d->dtype == RETRO_BF16)
-    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<__nv_bfloat16>, grid, dim3(256), 0, s, part_o, part_lse, q_pos,
-                                 seq_lens, cache_o, cache_lse, cache_pos, (__nv_bfloat16*)out, out_lse,
+  if (d->dtype == RETRO_BF16 && d->cache_dtype == RETRO_BF16)
+    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<__nv_bfloat16, __nv_bfloat16>, grid, dim3(256), 0, s, part_o,
+                                 part_lse, q_pos, seq_lens, (__nv_bfloat16*)cache_o, cache_lse, cache_pos,
+                                 (__nv_bfloat16*)out, out_lse, d->num_q_heads, d->head_dim, d->window));
+  else if (d->dtype == RETRO_BF16)
+    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<__nv_bfloat16, float>, grid, dim3(256), 0, s, part_o, part_lse,
+                                 q_pos, seq_lens, (float*)cache_o, cache_lse, cache_pos, (__nv_bfloat16*)out, out_lse,
                                  d->num_q_heads, d->head_dim, d->window));
   else
-    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<float>, grid, dim3(256), 0, s, part_o, part_lse, q_pos, seq_lens,
-                                 cache_o, cache_lse, cache_pos, (float*)out, out_lse, d->num_q_heads, d->head_dim,
-                                 d->window));
+    RETRO_CUDA_TRY(launch_kernel(merge_cache_kernel<float, float>, grid, dim3(256), 0, s, part_o, part_lse, q_pos,
+                                 seq_lens, (float*)cache_o, cache_lse, cache_pos, (float*)out, out_lse,
+                                 d->num_q_heads, d->head_dim, d->window));
   return RETRO_OK;
 }
 

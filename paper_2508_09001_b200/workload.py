@@ -290,3 +290,38 @@ def tensor_checksum(x: torch.Tensor) -> int:
     for chunk in raw.view(torch.int64).split(1 << 24):
         acc ^= int(np.bitwise_xor.reduce(chunk.cpu().numpy().view(np.uint64)))
     return acc
+
+
+def drift_step(inp: LayerInputs, step: int, rel_q: float = 0.05, rel_k: float = 0.05, rel_v: float = 0.10):
+    """"Drift" mode (in the full model the window tokens are re-embedded every step
+    and their Q / K move by < 5 %, V by < 10 % in relative l2 between adjacent steps; Alg. 1 line 2).
+
+    For decode step `step` returns the re-embedded tensors of the w past window tokens, seeded and deterministic:
+      positions [B][w] int32   t-w .. t-1, -1 where the position is not a decode-phase token yet
+      k_hat, v_hat [B][w][h_k][d], q_hat [B][w][h_q][d]   config dtype:  x_hat = x + rel * rms(x) * n,  n ~ N(0,1),
+    x the token's ORIGINAL value (so the drift stays bounded over a trajectory), rms over the head vector.
+    Pure data generation: nothing of the method is computed here."""
+    cfg = inp.cfg
+    B, w, P = cfg.batch, cfg.window, cfg.page_size
+    dt = inp.k_pages.dtype
+    positions = torch.full((B, max(w, 1)), -1, dtype=torch.int32)
+    k_hat = torch.zeros((B, max(w, 1), cfg.num_kv_heads, cfg.head_dim), dtype=dt)
+    v_hat = torch.zeros_like(k_hat)
+    q_hat = torch.zeros((B, max(w, 1), cfg.num_q_heads, cfg.head_dim), dtype=dt)
+    for b in range(B):
+        g = _gen("cpu", cfg.base_seed + 7919 * (step + 1) + 31 * b)
+        t = cfg.prompt_lens[b] + step
+        for i in range(w):
+            pos = t - w + i
+            s_of = pos - cfg.prompt_lens[b]                 # decode step that produced this token
+            if s_of < 0:
+                continue
+            positions[b, i] = pos
+            phys = int(inp.block_table[b, pos // P])
+            for src, dst, rel in ((inp.k_pages[phys, :, pos % P].float().cpu(), k_hat, rel_k),
+                                  (inp.v_pages[phys, :, pos % P].float().cpu(), v_hat, rel_v),
+                                  (inp.q_all[s_of, b].float().cpu(), q_hat, rel_q)):
+                n = torch.randn(src.shape, generator=g, dtype=torch.float32)
+                rms = src.pow(2).mean(dim=-1, keepdim=True).sqrt()
+                dst[b, i] = (src + rel * rms * n).to(dt)
+    return dict(positions=positions, k_hat=k_hat, v_hat=v_hat, q_hat=q_hat)

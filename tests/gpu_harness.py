@@ -236,7 +236,7 @@ def lockstep(inp: wl.LayerInputs, n_steps: int, budget_pages=None, start_step: i
         if cfg.window > 0:
             assert np.array_equal(sub_np(buf.cache_pos), layer.cache_pos), f"step {s} cache_pos"
             live = layer.cache_pos >= 0
-            co_g, cl_g = sub_np(buf.cache_o), sub_np(buf.cache_lse)
+            co_g, cl_g = sub_np(buf.cache_o.float()), sub_np(buf.cache_lse)
             errs["cache_o"] = max(errs["cache_o"], close(co_g[live], layer.cache_o[live], atol, rtol, f"step {s} cache_o"))
             close(cl_g[live], layer.cache_lse[live], atol, rtol, f"step {s} cache_lse")
     return errs

@@ -343,6 +343,68 @@ def test_update_kv_overwrite_and_digest_refresh_match_oracle():
         assert np.array_equal(buf.bounds[b, :, :n].double().cpu().numpy(), layer.bounds[b, :, :n])
 
 
+@pytest.mark.parametrize("name", ["c1", "c2"])
+def test_drift_trajectory_update_kv_inside_the_step_matches_oracle(name):
+    """NEXT-4 drift mode inside a trajectory (Alg. 1 lines 2-8): every step the w past window
+    tokens are re-embedded - their K / V rows are overwritten (retro_update_kv), the digests of the touched pages
+    refreshed (retro_update_page_bounds from t - w), the window queries replaced by their drifted versions - then
+    the whole step runs.  The oracle consumes the same arrays; selections bit-exact, outputs within tolerance."""
+    cfg = wl.c1() if name == "c1" else wl.shrink(wl.c2(), (1003, 700), 14, batch=2)
+    inp = wl.make_layer_inputs(cfg)
+    desc, buf = GH.make_device_layer(inp)
+    layer = H.oracle_layer(inp)
+    B, w, P = cfg.batch, cfg.window, cfg.page_size
+    prompt = np.asarray(cfg.prompt_lens)
+    layer.prefill_bounds(prompt)
+    buf.seq_lens.copy_(torch.from_numpy(prompt.astype(np.int32)))
+    buf.rebuild_bounds()
+    atol, rtol = GH.TOL[cfg.dtype]
+    n_touch = (w + P - 1) // P + 1
+    for s in range(cfg.n_steps):
+        seq_lens = inp.seq_lens_at(s).numpy()
+        dr = wl.drift_step(inp, s)
+        # Alg. 1 line 2 (UpdateKV) + digest refresh of the touched pages, both sides
+        buf.seq_lens.copy_(torch.from_numpy(seq_lens))
+        rb.retro_update_kv(desc, dr["k_hat"].cuda(), dr["v_hat"].cuda(), dr["positions"].cuda(), buf.block_table,
+                           buf.seq_lens, buf.k_pages, buf.v_pages)
+        pos_begin = torch.from_numpy(np.maximum(seq_lens - 1 - w, 0).astype(np.int32)).cuda()
+        rb.retro_update_page_bounds(desc, buf.k_pages, buf.block_table, buf.seq_lens, pos_begin, n_touch, buf.bounds)
+        orc.update_kv(layer.desc, layer.k_pages, layer.v_pages, layer.block_table, seq_lens, dr["positions"].numpy(),
+                      dr["k_hat"].double().numpy(), dr["v_hat"].double().numpy())
+        orc.update_page_bounds(layer.desc, layer.k_pages, layer.block_table, seq_lens,
+                               np.maximum(seq_lens - 1 - w, 0), layer.bounds)
+        # the window rows use the re-embedded queries (the current row its own query)
+        q_win, q_pos = wl.make_q_window(inp, s)
+        for b in range(B):
+            for i in range(w):
+                pos = int(dr["positions"][b, i])
+                if pos >= 0:
+                    q_win[b, wl.ring_slot(cfg, pos)] = dr["q_hat"][b, i]
+        res = layer.step(H.np64(q_win), q_pos.numpy(), H.np64(inp.q_all[s]), seq_lens,
+                         np.full(B, cfg.budget_pages, dtype=np.int32))
+        buf.q_win.copy_(q_win); buf.q_pos.copy_(q_pos); buf.q_cur.copy_(inp.q_all[s])
+        rb.retro_decode_step(desc, buf.state, buf.q_win, buf.q_pos, buf.q_cur, buf.out, buf.out_lse)
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.k_pages.double().cpu().numpy(), layer.k_pages), f"step {s} K pool after UpdateKV"
+        assert np.array_equal(buf.sel_pages.cpu().numpy(), res["sel_pages"]), f"step {s} sel_pages"
+        assert np.array_equal(buf.sel_prev.cpu().numpy(), res["sel_prev"]), f"step {s} sel_prev"
+        GH.close(buf.out.float().cpu().numpy(), res["out"], atol, rtol, f"drift step {s} out")
+        GH.close(buf.out_lse.cpu().numpy(), res["out_lse"], atol, rtol, f"drift step {s} out_lse")
+        assert np.array_equal(buf.cache_pos.cpu().numpy(), layer.cache_pos)
+
+
+@pytest.mark.parametrize("use_step", [False, True])
+def test_bf16_output_cache_matches_oracle_with_the_same_rounding(use_step):
+    """NEXT-3: 16-bit output cache + fp32 LSE, the paper's footprint (Eq. 12).  Merges run in fp32
+    and the row written back to the cache is rounded to bf16; the oracle rounds at the same place (round-to-nearest-
+    even), so outputs and cache contents agree within the usual bf16 tolerance over w = 8 consecutive merges."""
+    cfg = wl.shrink(wl.c5(8, 1024), (1500, 1490, 1333), 20, batch=3)
+    inp = wl.make_layer_inputs(cfg)
+    e = GH.lockstep(inp, 20, use_decode_step=use_step, desc_kw=dict(cache_dtype=rb.RETRO_BF16),
+                    oracle_kw=dict(cache_round="bf16"))
+    print("bf16 cache errs", e)
+
+
 def test_budget_policy_and_build_mask_match_oracle():
     """NEXT-2: device-side relative budget and Alg. 2 alone (external selector), bit-exact against the oracle."""
     cfg = wl.shrink(wl.c5(8, 1024), (1500, 40, 1714), 4, batch=3)

@@ -523,3 +523,26 @@ def test_step_diagnostics_effective_budget_is_the_union_size_and_mass_identity()
     for b in range(2):
         empty = [r for r in range(w + 1) if res[0]["q_pos"][b, r] < 0]
         assert len(empty) == w and np.all(diag[0][0][b][:, empty] == 0) and np.all(diag[0][1][b][empty] == 0)
+
+
+def test_bf16_cache_rounding_is_library_rounding_and_its_error_budget_over_w_merges():
+    """NEXT-3 (Eq. 12: 16-bit cached O + fp32 LSE).  (1) round_bf16 == torch's float32 -> bfloat16
+    conversion (round-to-nearest-even) on values over 40 binades; (2) error budget: a trajectory with the cache kept
+    in bf16 against the same trajectory with the full-precision cache: every merged output within
+    (w + 1) roundings of 2^-9 relative to the largest value, far inside the 2e-2 + 1e-2 |x| tolerance."""
+    import torch
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal(200000) * np.exp(rng.uniform(-14, 14, 200000))
+    assert np.array_equal(orc.round_bf16(x), torch.from_numpy(x).float().to(torch.bfloat16).double().numpy())
+    assert np.array_equal(orc.round_bf16(np.array([0.0, -0.0, 1.0, -2.5])), np.array([0.0, -0.0, 1.0, -2.5]))
+    cfg = wl.shrink(wl.c2(), (300,), 14, window=6, budget_tokens=96, num_q_heads=8, num_kv_heads=2)
+    inp = wl.make_layer_inputs(cfg)
+    _, ref = H.run_oracle_trajectory(inp, 14)
+    _, low = H.run_oracle_trajectory(inp, 14, cache_round="bf16")
+    worst = 0.0
+    for a, b in zip(ref, low):
+        assert np.array_equal(a["sel_pages"], b["sel_pages"])
+        scale = np.abs(a["out"]).max()
+        worst = max(worst, float(np.abs(a["out"] - b["out"]).max() / scale))
+        np.testing.assert_allclose(b["out"], a["out"], atol=2e-2, rtol=1e-2)
+    assert 0.0 < worst < (cfg.window + 1) * 2.0 ** -9
