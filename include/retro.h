@@ -13,7 +13,14 @@
  *     work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream) and is CUDA-graph
  *     capturable: every step-varying quantity (seq_lens, q_pos, budgets, cache_pos) lives in device memory
  *     and grids are sized from the descriptor's upper bounds only.
- *   - Device pointers must be 16-byte aligned.  Validation is host-side only (null / shape / alignment).
+ *     (One documented exception: retro_debug_status in the RETRO_DEBUG_CHECKS build synchronises `stream` and
+ *     reads two counters back.)
+ *   - Host-side state kept by the library (per process, one mutex, safe to call from several threads): the last
+ *     CUDA error, per-device facts (SM count, shared-memory limit), per-(device, kernel) shared-memory grants and
+ *     resident-cluster capacities, and a 64-entry cache of TMA tensor-map descriptors keyed by the K/V pool
+ *     addresses and shapes.  Nothing else survives a call.
+ *   - Device pointers must be 16-byte aligned.  Validation is host-side only (null / shape / alignment); the debug
+ *     build (libretro_dbg.so) adds device-side checks of every index the kernels consume.
  *   - `w` = desc->window counts PAST queries (the paper's window counts the current one: w_paper = w + 1);
  *     w = 0 is plain Quest sparse attention and needs no mask / cache buffers.
  *   - t_b = seq_lens[b] - 1 is the position of sequence b's current token.  "Decode step" and "position of the

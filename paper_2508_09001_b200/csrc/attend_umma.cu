@@ -18,15 +18,22 @@
 // when some logit exceeds it by more than 64 (log2 units: bf16 and fp32 share the exponent range, so P up to
 // 2^64 costs no precision), so the common block needs no reduction.
 //
-// One CTA per (split, KV head, sequence), 640 threads, warp-specialised:
+// One CTA per (split, row group, KV head, sequence), 640 threads, warp-specialised; the splits of a (unit, row
+// group) are the CTAs of one thread-block cluster (<= 8):
 //   warp 0, 1   TMA producers, one for K and one for V (separate rings of 32 KB slots = 8 pages = 128 keys, so a
 //               K block never queues behind the longer-lived V block): every selected (page, head) tile arrives
 //               as two 64-channel boxes with the 128-byte swizzle (cp.async.bulk.tensor.2d + mbarrier).
 //   warp 2      MMA issuer (converged warp, elect.sync: the operands stay in uniform registers), owns the TMEM
 //               allocation; tcgen05.commit signals mbarriers.
-//   warp 3      idle (keeps the softmax warps aligned to the TMEM lane quadrants)
+//   warp 3      S4 service (fused step only; also keeps the softmax warps aligned to the TMEM lane quadrants):
+//               prefetches this CTA's output-cache operands into shared memory, snapshots cache_pos, takes the
+//               cross-head arrival ticket whose last holder rewrites cache_pos.
 //   warps 4..19 softmax: TMEM lane quadrant = warp % 4 (32 keys), column group = (warp - 4) / 4 (a quarter of the rows).
-// Every page is read from HBM once and serves all rows.  Split partials are combined by the last CTA of the unit.
+// Every page is read from HBM once and serves all rows.  Epilogue: every split stages its normalised partial (fp16
+// tile + base-2 lse) in its own shared memory, one cluster barrier, then each CTA merges a share of the
+// (cache slot, q head) items, reading the other splits' rows through distributed shared memory (Eq. 8 over the
+// splits), and - inside retro_decode_step - merges with the cached (o, lse) and writes out / cache (S4, Eq. 8-9).
+// In the fused step everything that does not depend on this step's selection runs before griddepcontrol.wait.
 #include <cuda.h>
 #include <cuda_fp16.h>
 
