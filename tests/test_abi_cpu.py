@@ -56,3 +56,28 @@ def test_workspace_grows_with_window_and_batch():
     a = rb.retro_workspace_bytes(rb.make_desc(8, 32, 8, 128, 16, 2064, 256, 8 * 2064, 0, "bf16"))
     b = rb.retro_workspace_bytes(rb.make_desc(8, 32, 8, 128, 16, 2064, 256, 8 * 2064, 32, "bf16"))
     assert b > a
+
+
+def test_launch_plan_is_two_kernels_per_layer_step_where_the_fusion_applies():
+    """retro_launches_per_step is host logic (no device needed): the bf16 tensor-core path with one row group fuses
+    the split combine and S4 into the attend kernel (select + attend = 2 launches); fp32 (C1) and row blocks above
+    128 rows (w = 32 with G = 4) run S4 as a third launch."""
+    two = {
+        "c2": rb.make_desc(1, 32, 8, 128, 16, 2304, 64, 2304, 8, "bf16"),
+        "c3": rb.make_desc(16, 32, 8, 128, 16, 1536, 128, 16 * 1536, 16, "bf16"),
+        "c4": rb.make_desc(4, 28, 4, 128, 16, 8208, 256, 4 * 8208, 8, "bf16"),
+        "c5_w0": rb.make_desc(8, 32, 8, 128, 16, 2064, 256, 8 * 2064, 0, "bf16"),
+        "c2_bf16_cache": rb.make_desc(1, 32, 8, 128, 16, 2304, 64, 2304, 8, "bf16", cache_dtype=rb.RETRO_BF16),
+    }
+    three = {
+        "c1_fp32": rb.make_desc(1, 4, 4, 64, 16, 33, 8, 33, 4, "f32"),
+        "c5_w32": rb.make_desc(8, 32, 8, 128, 16, 2064, 256, 8 * 2064, 32, "bf16"),
+    }
+    for name, d in two.items():
+        assert rb.retro_launches_per_step(d) == 2, name
+    for name, d in three.items():
+        assert rb.retro_launches_per_step(d) == 3, name
+    # a 16-bit output cache needs bf16 inputs
+    with pytest.raises(rb.RetroError) as e:
+        rb.retro_workspace_bytes(rb.make_desc(1, 4, 4, 64, 16, 33, 8, 33, 4, "f32", cache_dtype=rb.RETRO_BF16))
+    assert e.value.code in (rb.RETRO_ERR_ARG, rb.RETRO_ERR_UNSUPPORTED)
