@@ -5,6 +5,8 @@
 The .so is git-ignored but travels to the GPU box with the gpurun snapshot."""
 from __future__ import annotations
 
+import contextlib
+import fcntl
 import os
 import subprocess
 import sys
@@ -37,11 +39,30 @@ def build_debug(force: bool = False) -> str:
     return build(force=force, lib_path=DBG_LIB_PATH, extra_flags=["-DRETRO_DEBUG_CHECKS"], obj_suffix=".dbg.o")
 
 
+@contextlib.contextmanager
+def _build_lock():
+    """One builder at a time per checkout: the ranks of a torchrun launch (or parallel test workers) that all find
+    the library stale take turns; every rank after the first then finds it up to date."""
+    os.makedirs(LIB_DIR, exist_ok=True)
+    with open(os.path.join(LIB_DIR, ".build.lock"), "w") as f:
+        fcntl.flock(f, fcntl.LOCK_EX)
+        try:
+            yield
+        finally:
+            fcntl.flock(f, fcntl.LOCK_UN)
+
+
 def build(force: bool = False, verbose: bool = False, lib_path: str = LIB_PATH, extra_flags=(),
           obj_suffix: str = ".o") -> str:
     if not force and not _stale(lib_path):
         return lib_path
-    os.makedirs(LIB_DIR, exist_ok=True)
+    with _build_lock():
+        if not force and not _stale(lib_path):      # another process built it while this one waited
+            return lib_path
+        return _build_locked(verbose, lib_path, extra_flags, obj_suffix)
+
+
+def _build_locked(verbose: bool, lib_path: str, extra_flags, obj_suffix: str) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
@@ -63,11 +84,14 @@ def build(force: bool = False, verbose: bool = False, lib_path: str = LIB_PATH, 
         failed |= pr.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed building libretro.so")
-    link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", lib_path] + objs
+    # link to a temporary name and rename: a process that has the old library mapped keeps a consistent file
+    tmp_path = lib_path + f".tmp{os.getpid()}"
+    link = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp_path] + objs
     r = subprocess.run(link, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:
         sys.stderr.write(r.stdout)
         raise RuntimeError("nvcc link failed for libretro.so")
+    os.replace(tmp_path, lib_path)
     return lib_path
 
 
