@@ -151,6 +151,28 @@ def time_graph(graph, iters: int):
     return start.elapsed_time(end)   # ms
 
 
+def replay_percentiles(graph, n_layers: int, iters: int = 48):
+    """p10 / median / p90 of single graph replays (one decode step of the whole stack each), us per layer-step;
+    a separate pass after the timed region (per-replay events leave gaps: the headline value is the K-step mean).
+    None if anything goes wrong: this is a side figure and must never cost the bench line."""
+    try:
+        import torch
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+        torch.cuda.synchronize()
+        for a, b in evs:
+            a.record()
+            graph.replay()
+            b.record()
+        torch.cuda.synchronize()
+        us = sorted(a.elapsed_time(b) * 1000.0 / n_layers for a, b in evs)
+        pick = lambda q: us[min(len(us) - 1, int(q * len(us)))]
+        return {"p10": pick(0.10), "p50": pick(0.50), "p90": pick(0.90), "replays": iters,
+                "unit": UNIT, "note": "single replays timed one by one (events around each): includes the launch gap "
+                                      "between replays that the K-step mean amortises"}
+    except Exception:
+        return None
+
+
 def run_stack(cfg, n_layers, steps, warmup, seed_offset, dist_barrier, keep_inputs=False):
     """Build the layer stack, warm up, time `steps` graph replays.  Returns (stack, graph, elapsed_ms)."""
     import torch
@@ -342,9 +364,9 @@ def main():
     warmup = max(args.warmup, 3)
     steps, L = args.steps, args.layers
     w_full = None
-    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 80)
+    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 160)
     warmup = max(warmup, cfg.window + 2)       # the retro window is full during the timed region
-    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 80)
+    cfg = workload_cfg(args.workload, n_steps=warmup + steps + 160)
     seed_off = hs.rank_layer_seed_offset(ri.rank)
 
     sampler = ClockSampler(ri.local_rank) if ri.rank == 0 else None
@@ -378,6 +400,7 @@ def main():
     }
 
     if not args.no_extras:
+        line["step_percentiles"] = replay_percentiles(graph, L)
         # ---- device time of the step's OWN kernels (retro_decode_step_part: the select kernel with S1 in line, the
         # attend kernel with the split combine and S4 in its epilogue), each as a CUDA graph of L back-to-back
         # launches (one per layer, different layer state) between CUDA events, from the state the timed steps left
@@ -465,7 +488,7 @@ def main():
         if ri.rank == 0 and ri.world_size == 1 and args.workload == "c2" and args.window is None:
             line["bandwidth_point"] = bandwidth_point(peak, dev)
         if cfg.window > 0 and not args.no_w0:
-            cfg0 = workload_cfg(args.workload, n_steps=warmup + steps + 80, window=0)
+            cfg0 = workload_cfg(args.workload, n_steps=warmup + steps + 160, window=0)
             stack0, graph0, ms0 = run_stack(cfg0, L, steps, warmup, seed_off, barrier)
             ms0 = hs.max_over_ranks(ms0, dev)
             us0 = ms0 * 1000.0 / (steps * L)
