@@ -29,7 +29,10 @@
  * Layouts (row-major, innermost last; T = desc->dtype element, P = page_size, d = head_dim):
  *   k_pages, v_pages [num_phys_pages][h_k][P][d] T   each (page, KV head) tile is contiguous (4 KB for bf16 d128).
  *                                                   Slots at positions >= seq_len are never used: they may hold
- *                                                   anything (unwritten memory, NaN, Inf).
+ *                                                   anything (unwritten memory, NaN, Inf).  bf16 path: VALID V values
+ *                                                   must satisfy |v| <= 65504 - the normalised partial of a KV split
+ *                                                   (a convex combination of V rows) is handed to the split combine
+ *                                                   as fp16; larger magnitudes overflow to Inf there.
  *   block_table      [B][max_pages_per_seq] int32   logical page j of sequence b -> physical page
  *   seq_lens         [B] int32                      tokens valid in sequence b, current token included
  *   bounds           [B][h_k][max_pages_per_seq][2][d] T   [..][0][:] = Kmax, [..][1][:] = Kmin
