@@ -436,6 +436,12 @@ def main():
                                              "traffic": ncu_traffic(wl_key, k.split("_")[0]) if wl_key else None}
                                          for k in step_k}
         line["attend_arith_intensity_flop_per_byte"] = hs.attend_flops(cfg, seq_now) / bytes_model["kv"]
+        # the same counting only the (row, page) pairs the retrospective mask leaves: every pair of the
+        # current query's G rows plus the unmasked share of the past rows' pairs (layer 0, last timed step)
+        f_unmasked = (workload_stats or {}).get("unmasked_past_row_page_pairs")
+        if f_unmasked is not None:
+            line["attend_arith_intensity_unmasked_flop_per_byte"] = (
+                line["attend_arith_intensity_flop_per_byte"] * (1.0 + cfg.window * f_unmasked) / (cfg.window + 1))
         # ---- the four stand-alone C-ABI entry points (S1, S2, S3, S4 launched alone), for reference ----
         # (they run after the select replays above: their mask state is "every selected page seen", i.e. the
         # stand-alone attend entry point is timed on the current row's work only; the step-kernel figures above are
