@@ -500,6 +500,21 @@ def main():
             us0 = ms0 * 1000.0 / (steps * L)
             line["w0_us_per_layer_step"] = us0
             line["overhead_vs_w0"] = us_layer / us0 - 1.0
+            del graph0, stack0
+            torch.cuda.empty_cache()
+        # ---- single layer, hot L2 (SURVEY 8(d) "also report the single-layer hot-L2 number, labelled"): the same
+        # step with ONE layer state, so that layer's digests and recurring pages stay in the 126 MB L2 from step to
+        # step.  A side figure: never the headline, and never allowed to cost the bench line.
+        if ri.world_size == 1:
+            try:
+                stack1, graph1, ms1 = run_stack(cfg, 1, steps, warmup, seed_off, barrier)
+                line["single_layer_hot_l2"] = {
+                    "value": ms1 * 1000.0 / steps, "unit": UNIT, "layers_per_step": 1,
+                    "note": "one layer state replayed every step: its digests and the pages that stay selected are "
+                            "L2 hits; NOT comparable with `value` (32 layer states, inputs larger than L2)"}
+                del graph1, stack1
+            except Exception as ex:      # noqa: BLE001
+                line["single_layer_hot_l2"] = {"value": None, "error": repr(ex)[:200]}
     else:
         line["e2e"] = None
 
