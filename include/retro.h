@@ -118,7 +118,9 @@ int retro_update_page_bounds(const retro_desc_t* desc, const void* k_pages, cons
                              int32_t max_touched_pages /*HOST*/, void* bounds, void* stream);
 
 /* S2 (Eq. 1; top-k PAPER.md:42, 248; Alg. 2).  Per (b, KV head):
- * score_j = reduce over the head's q heads g of sum_c max(q_gc * Kmin_jc, q_gc * Kmax_jc), accumulated in fp64;
+ * score_j = reduce over the head's q heads g of sum_c max(q_gc * Kmin_jc, q_gc * Kmax_jc).  The ranking is the one
+ * of the fp64 scores: the digest stream is scored in fp32 next to a proven bound on the fp32 error, and the pages the
+ * bound cannot decide are re-scored in fp64 and ranked exactly (reading Q7);
  * k = min(budget_pages[b], #pages, max_sel_pages); k == #pages selects every page, else the newest page (if
  * force_last_page) plus the best of the others ordered by (score desc, index asc); emitted ascending.
  * Then M_i = A[page_i] -> sel_prev and A[page_i] = seq_lens[b] - 1.  last_loaded may be NULL iff window == 0
