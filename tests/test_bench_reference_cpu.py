@@ -35,3 +35,16 @@ def test_reference_arm_prints_one_contract_line():
 def test_reference_arm_other_ranks_exit_quietly():
     r = _run({"RANK": "1", "WORLD_SIZE": "2"})
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_our_arm_fails_loudly_without_a_cuda_device():
+    """No CPU fallback: on a box without a GPU the product arm stops with a clear message, it does not time anything."""
+    import pytest
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("this box has a GPU: the arm would run the real benchmark")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "1"], cwd=ROOT,
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode != 0
+    assert "needs a CUDA device" in r.stderr
+    assert r.stdout.strip() == ""
