@@ -16,6 +16,7 @@ CSRC = os.path.join(PKG, "csrc")
 LIB_DIR = os.path.join(PKG, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libretro.so")
 DBG_LIB_PATH = os.path.join(LIB_DIR, "libretro_dbg.so")
+NVTX_LIB_PATH = os.path.join(LIB_DIR, "libretro_nvtx.so")
 INCLUDE = os.path.join(os.path.dirname(PKG), "include")
 
 
@@ -37,6 +38,11 @@ def _stale(lib_path: str = None) -> bool:
 def build_debug(force: bool = False) -> str:
     """The same library with -DRETRO_DEBUG_CHECKS (device-side index validation) -> lib/libretro_dbg.so."""
     return build(force=force, lib_path=DBG_LIB_PATH, extra_flags=["-DRETRO_DEBUG_CHECKS"], obj_suffix=".dbg.o")
+
+
+def build_nvtx(force: bool = False) -> str:
+    """The same library with -DRETRO_NVTX (every entry point is an NVTX range) -> lib/libretro_nvtx.so."""
+    return build(force=force, lib_path=NVTX_LIB_PATH, extra_flags=["-DRETRO_NVTX"], obj_suffix=".nvtx.o")
 
 
 @contextlib.contextmanager
@@ -99,3 +105,5 @@ if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
     if "--debug" in sys.argv:
         print(build_debug(force="--force" in sys.argv))
+    if "--nvtx" in sys.argv:
+        print(build_nvtx(force="--force" in sys.argv))

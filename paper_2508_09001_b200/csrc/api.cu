@@ -3,6 +3,24 @@
 
 #include "common.cuh"
 
+// -DRETRO_NVTX (lib/libretro_nvtx.so): every entry point that enqueues work is an NVTX range named after itself, so a
+// timeline tool shows the host side of a step (validation, launch calls) next to the kernels.  Header-only NVTX 3:
+// nothing is linked and the calls are no-ops until a tool attaches.  The release build compiles the macro away.
+#ifdef RETRO_NVTX
+#include <nvtx3/nvToolsExt.h>
+namespace {
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
+}  // namespace
+#define RETRO_RANGE(name) NvtxRange nvtx_range__(name)
+#else
+#define RETRO_RANGE(name) do {} while (0)
+#endif
+
 namespace retro {
 
 static std::atomic<int> g_last_cuda_error{0};
@@ -203,6 +221,7 @@ int retro_workspace_bytes(const retro_desc_t* desc, size_t* bytes) {
 }
 
 int retro_workspace_init(const retro_desc_t* desc, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_RANGE("retro_workspace_init");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(workspace);
   const WorkspaceLayout wl = workspace_layout(desc);
@@ -215,6 +234,7 @@ int retro_workspace_init(const retro_desc_t* desc, void* workspace, size_t ws_by
 int retro_update_page_bounds(const retro_desc_t* desc, const void* k_pages, const int32_t* block_table,
                              const int32_t* seq_lens, const int32_t* pos_begin, int32_t max_touched_pages,
                              void* bounds, void* stream) {
+  RETRO_RANGE("retro_update_page_bounds");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(bounds);
   if (pos_begin != nullptr && !aligned16(pos_begin)) return RETRO_ERR_ARG;
@@ -226,6 +246,7 @@ int retro_update_page_bounds(const retro_desc_t* desc, const void* k_pages, cons
 int retro_select_pages(const retro_desc_t* desc, const void* q_cur, const void* bounds, const int32_t* seq_lens,
                        const int32_t* budget_pages, int32_t* last_loaded, int32_t* sel_pages, int32_t* sel_prev,
                        int32_t* sel_count, double* scores_out, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_RANGE("retro_select_pages");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(q_cur); RETRO_CHECK_PTR(bounds); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(budget_pages);
   RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(workspace);
@@ -242,6 +263,7 @@ int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32
                         const void* v_pages, const int32_t* block_table, const int32_t* seq_lens,
                         const int32_t* sel_pages, const int32_t* sel_prev, const int32_t* sel_count, float* part_o,
                         float* part_lse, void* workspace, size_t ws_bytes, void* stream) {
+  RETRO_RANGE("retro_sparse_attend");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(q_win); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
   RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev);
@@ -255,6 +277,7 @@ int retro_sparse_attend(const retro_desc_t* desc, const void* q_win, const int32
 int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, const float* part_lse,
                              const int32_t* q_pos, const int32_t* seq_lens, void* cache_o, float* cache_lse,
                              int32_t* cache_pos, void* out, float* out_lse, void* stream) {
+  RETRO_RANGE("retro_merge_output_cache");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(part_o); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(q_pos); RETRO_CHECK_PTR(seq_lens);
   RETRO_CHECK_PTR(out);
@@ -266,6 +289,7 @@ int retro_merge_output_cache(const retro_desc_t* desc, const float* part_o, cons
 
 int retro_append_kv(const retro_desc_t* desc, const void* k_new, const void* v_new, const int32_t* block_table,
                     const int32_t* seq_lens, void* k_pages, void* v_pages, void* stream) {
+  RETRO_RANGE("retro_append_kv");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(k_new); RETRO_CHECK_PTR(v_new); RETRO_CHECK_PTR(block_table); RETRO_CHECK_PTR(seq_lens);
   RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
@@ -275,6 +299,7 @@ int retro_append_kv(const retro_desc_t* desc, const void* k_new, const void* v_n
 int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, int32_t* step_counter,
                          int32_t pool_steps, int32_t* seq_lens, void* q_win, int32_t* q_pos, void* q_cur_out,
                          void* stream) {
+  RETRO_RANGE("retro_window_advance");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(q_new_or_pool); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(q_win); RETRO_CHECK_PTR(q_pos);
   if (step_counter != nullptr && pool_steps < 1) return RETRO_ERR_ARG;
@@ -285,6 +310,7 @@ int retro_window_advance(const retro_desc_t* desc, const void* q_new_or_pool, in
 
 int retro_budget_policy(const retro_desc_t* desc, const int32_t* seq_lens, int32_t ratio_permille, int32_t min_tokens,
                         int32_t* budget_pages, void* stream) {
+  RETRO_RANGE("retro_budget_policy");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(budget_pages);
   if (ratio_permille < 0 || min_tokens < 0) return RETRO_ERR_ARG;
@@ -293,6 +319,7 @@ int retro_budget_policy(const retro_desc_t* desc, const int32_t* seq_lens, int32
 
 int retro_build_mask(const retro_desc_t* desc, const int32_t* sel_pages, const int32_t* sel_count,
                      const int32_t* seq_lens, int32_t* last_loaded, int32_t* sel_prev, void* stream) {
+  RETRO_RANGE("retro_build_mask");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(last_loaded);
   RETRO_CHECK_PTR(sel_prev);
@@ -303,6 +330,7 @@ int retro_step_diagnostics(const retro_desc_t* desc, const int32_t* sel_pages, c
                            const int32_t* sel_count, const int32_t* q_pos, const int32_t* seq_lens,
                            const float* part_lse, const float* out_lse, int32_t* supp_pages, float* supp_mass,
                            void* stream) {
+  RETRO_RANGE("retro_step_diagnostics");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(sel_pages); RETRO_CHECK_PTR(sel_prev); RETRO_CHECK_PTR(sel_count); RETRO_CHECK_PTR(q_pos);
   RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(part_lse); RETRO_CHECK_PTR(out_lse); RETRO_CHECK_PTR(supp_pages);
@@ -315,6 +343,7 @@ int retro_step_diagnostics(const retro_desc_t* desc, const int32_t* sel_pages, c
 int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_hat, const int32_t* positions,
                     int32_t n_upd, const int32_t* block_table, const int32_t* seq_lens, void* k_pages, void* v_pages,
                     void* stream) {
+  RETRO_RANGE("retro_update_kv");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(k_hat); RETRO_CHECK_PTR(v_hat); RETRO_CHECK_PTR(positions); RETRO_CHECK_PTR(block_table);
   RETRO_CHECK_PTR(seq_lens); RETRO_CHECK_PTR(k_pages); RETRO_CHECK_PTR(v_pages);
@@ -325,6 +354,7 @@ int retro_update_kv(const retro_desc_t* desc, const void* k_hat, const void* v_h
 
 int retro_window_advance_layers(const retro_desc_t* desc, const retro_advance_rec_t* table, int32_t n_layers,
                                 int32_t pool_steps, void* stream) {
+  RETRO_RANGE("retro_window_advance_layers");
   RETRO_CHECK_DESC(desc);
   RETRO_CHECK_PTR(table);
   if (n_layers < 1 || pool_steps < 1) return RETRO_ERR_ARG;
@@ -381,12 +411,14 @@ static int decode_step_parts(const retro_desc_t* desc, const retro_layer_state_t
 
 int retro_decode_step(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
                       const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, void* stream) {
+  RETRO_RANGE("retro_decode_step");
   return decode_step_parts(desc, st, q_win, q_pos, q_cur, out, out_lse, 3, stream);
 }
 
 int retro_decode_step_part(const retro_desc_t* desc, const retro_layer_state_t* st, const void* q_win,
                            const int32_t* q_pos, const void* q_cur, void* out, float* out_lse, int32_t part,
                            void* stream) {
+  RETRO_RANGE("retro_decode_step_part");
   if (part != 0 && part != 1) return RETRO_ERR_ARG;
   return decode_step_parts(desc, st, q_win, q_pos, q_cur, out, out_lse, 1 << part, stream);
 }
@@ -422,6 +454,7 @@ int retro_launches_per_step(const retro_desc_t* desc, int32_t* launches) {
 
 int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* st, const retro_step_io_t* io,
                            const void* host_qkv_new, void* host_out, void* stream) {
+  RETRO_RANGE("retro_decode_step_host");
   RETRO_CHECK_DESC(desc);
   int rc = check_state(desc, st);
   if (rc != RETRO_OK) return rc;
@@ -445,6 +478,7 @@ int retro_decode_step_host(const retro_desc_t* desc, const retro_layer_state_t* 
 
 int retro_decode_steps_host(const retro_desc_t* desc, const retro_layer_state_t* states, const retro_step_io_t* ios,
                             int32_t n_layers, const void* host_qkv_new, void* host_out, void* stream) {
+  RETRO_RANGE("retro_decode_steps_host");
   RETRO_CHECK_DESC(desc);
   if (states == nullptr || ios == nullptr || n_layers < 1 || host_qkv_new == nullptr || host_out == nullptr)
     return RETRO_ERR_ARG;

@@ -81,3 +81,21 @@ def test_launch_plan_is_two_kernels_per_layer_step_where_the_fusion_applies():
     with pytest.raises(rb.RetroError) as e:
         rb.retro_workspace_bytes(rb.make_desc(1, 4, 4, 64, 16, 33, 8, 33, 4, "f32", cache_dtype=rb.RETRO_BF16))
     assert e.value.code in (rb.RETRO_ERR_ARG, rb.RETRO_ERR_UNSUPPORTED)
+
+
+def test_nvtx_build_exports_the_same_abi_and_answers_on_the_host():
+    """-DRETRO_NVTX (NVTX ranges around the entry points): same symbols, header-only NVTX 3 inside
+    (nothing linked), and a range opened without a tool attached is a no-op."""
+    from paper_2508_09001_b200 import build as rbuild
+    path = rbuild.build_nvtx()
+    lib = C.CDLL(path)
+    for n in declared_symbols():
+        assert hasattr(lib, n), f"libretro_nvtx.so does not export {n}"
+    blob = open(path, "rb").read()
+    assert b"nvtxRangePushA" in blob and b"retro_select_pages" in blob
+    assert b"nvtxRangePushA" not in open(rb.library_path(), "rb").read()      # the release build has none of it
+    # an entry point that opens a range and returns from host-side validation: the range is pushed and popped
+    desc = rb.make_desc(1, 32, 8, 128, 16, 64, 8, 64, 2, "bf16")
+    lib.retro_workspace_init.restype = C.c_int
+    rc = lib.retro_workspace_init(C.byref(desc), C.c_void_p(0), C.c_size_t(0), C.c_void_p(0))
+    assert rc == rb.RETRO_ERR_ARG
